@@ -1,0 +1,181 @@
+/*
+ * glisse.h — C ABI of the B200-native GLISSE hot path.
+ *
+ * What the library computes (all fp64): N massless test particles are advanced through a
+ * star + N_p planet system with the fixed-time-step Wisdom–Holman mixed-variable symplectic
+ * step of Zhang & Gladman 2020 (§2.2 Eq. 1–2 and the 5-item step list at
+ * PAPER.md:91-95): kick ½ – Kepler drift 1 – kick ½ for the particles, the standard Jacobi
+ * WH step for the mutually interacting planets, close-encounter / escape tests
+ * that flag and freeze a particle.  DESIGN.md §2 lists every reading of the
+ * paper that this header relies on (step order, Kepler-solver form, flag priorities …).
+ *
+ * Every step of the path runs in hand-written CUDA kernels for sm_100a; there is no CPU
+ * fallback.  If no CUDA device is usable every entry point returns GLISSE_ECUDA.
+ *
+ * Conventions
+ *  - Return value: 0 (GLISSE_OK) on success, a negative GLISSE_E* status otherwise.  The
+ *    library never throws, aborts or prints.
+ *  - Units: the library is unit-agnostic; G is folded into the masses (gm = G·m).  The
+ *    benchmark configurations use AU, days, solar masses with G = k² (Gaussian constant).
+ *  - Pointers marked "host or device" are classified with cudaPointerGetAttributes; anything
+ *    that is not device/managed memory is treated as pageable or pinned host memory.
+ *  - Ownership: inputs are copied during glisse_create (the caller keeps its buffers); outputs
+ *    are caller-allocated.  The library owns its internal device state until glisse_destroy.
+ *  - Threading: one glisse_sim per host thread; no global mutable state.
+ */
+#ifndef GLISSE_H_
+#define GLISSE_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes ------------------------------------------------------------------------- */
+#define GLISSE_OK       0
+#define GLISSE_EINVAL  (-1)  /* null pointer, size <= 0, n_planets outside [0,32], dt == 0,
+                                non-finite input, bad params                                  */
+#define GLISSE_ECUDA   (-2)  /* a CUDA call failed (sticky: the sim is unusable afterwards)    */
+#define GLISSE_ENOMEM  (-3)  /* host or device allocation failed                              */
+#define GLISSE_EPLANET (-4)  /* a planet's Kepler drift failed (unbound / not converged): the
+                                paper requires encounter-free planets           */
+
+/* ---- per-particle flag values ("a flag that records which planet") ------------ */
+#define GLISSE_FLAG_ACTIVE    0
+#define GLISSE_FLAG_RMIN      1   /* |r| < r_min                     (BASELINE.json configs)  */
+#define GLISSE_FLAG_RMAX      2   /* |r| > r_max                     (BASELINE.json configs)  */
+#define GLISSE_FLAG_NONCONV   3   /* Kepler solve not converged           */
+#define GLISSE_FLAG_UNBOUND   4   /* 2μ/r − v² <= 0 at the drift     (reading S8)   */
+#define GLISSE_FLAG_PLANET0  16   /* 16 + j : |r − q_j| < rcrit_j       */
+
+#define GLISSE_MAX_PLANETS   32
+
+typedef struct glisse_sim glisse_sim; /* opaque */
+
+/* User-configurable quantities the paper names: Kepler iteration count (fn 5 at
+ * 135), planetary chunk size, resync interval.                   */
+typedef struct {
+  double r_min;         /* heliocentric inner removal radius; <= 0 disables the test           */
+  double r_max;         /* heliocentric outer removal radius; +inf (or <= 0) disables the test */
+  int    kepler_iters;  /* maximum number of Newton updates per Kepler solve, default 5        */
+  double kepler_tol;    /* |residual of Kepler's equation| above which a particle is flagged
+                           GLISSE_FLAG_NONCONV, default 1e-14                   */
+  int    chunk_steps;   /* K: steps per planet-log chunk = per particle-kernel launch,
+                           default 1024, 1..16384; performance only, results do not depend on it */
+  int    resync_chunks; /* R: survivor compaction every R chunks, 0 = never, default 1;
+                           performance only, results do not depend on it                       */
+  int    device;        /* CUDA device ordinal, default 0                                      */
+  void*  stream;        /* cudaStream_t on which the particle work is enqueued, or NULL for a
+                           stream owned by the library                                         */
+} glisse_params;
+
+/* Fill *p with the defaults listed above.  p == NULL is ignored. */
+void glisse_default_params(glisse_params* p);
+
+/*
+ * Create a simulation at step 0.
+ *   gm_star        G·m0.
+ *   n_planets      N_p in [0, 32]; planets are given in Jacobi order = order of increasing
+ *                  distance from the star.
+ *   gm_planet      [n_planets] host; G·m_j > 0.
+ *   planet_pos/vel [n_planets][3] host, row-major (x,y,z per planet), heliocentric.
+ *   planet_rcrit   [n_planets] host; absolute encounter radius of planet j in length units
+ *                  (e.g. k Hill radii); 0 disables the test for that planet.
+ *                  May be NULL (all tests off).
+ *   n_particles    N >= 1 (N < 2^31).
+ *   pos, vel       three pointers each (x,y,z / vx,vy,vz), every one an array of N doubles,
+ *                  struct-of-arrays, heliocentric, host or device (all six of the same kind).
+ *   dt             time step, non-zero; negative integrates backwards (time reversal).
+ *   params         NULL = defaults.
+ * On success *out holds the handle.  Work is enqueued on params->stream; create synchronises.
+ */
+int glisse_create(glisse_sim** out,
+                  double gm_star,
+                  int n_planets, const double* gm_planet,
+                  const double* planet_pos, const double* planet_vel,
+                  const double* planet_rcrit,
+                  long long n_particles,
+                  const double* const pos[3], const double* const vel[3],
+                  double dt, const glisse_params* params);
+
+/*
+ * Advance planets and particles by n_steps >= 0 steps of size dt.  Asynchronous: kernels are
+ * enqueued on the sim's stream (planet-history kernels on an internal second stream) and the
+ * call returns without waiting.  The sequence per chunk of <= K steps is: planet-history kernel
+ * (a1) -> particle kernel (a2–a7) -> every R chunks the compaction kernels (a8).
+ * A planet failure is reported by the next synchronising call as GLISSE_EPLANET.
+ */
+int glisse_advance(glisse_sim* sim, long long n_steps);
+
+/*
+ * Test hook / external planet history ("these planetary positions could be supplied
+ * using any method"): advance the PARTICLES by n_steps using a caller-supplied planet log
+ * instead of the planet-history kernel.  log holds n_steps+1 records (times t_s … t_{s+n}),
+ * host or device, each glisse_log_stride(n_planets) doubles:
+ *   [ q_0x q_0y q_0z  q_1x … q_{Np-1}z   h0x h0y h0z   (zero padding to an even count) ]
+ * with h0 = −Σ_j gm_j q_j/|q_j|³.  The internal planet state is NOT advanced.
+ */
+int glisse_advance_with_log(glisse_sim* sim, long long n_steps, const double* log);
+
+/* Doubles per planet-log record: 3·(n_planets+1) rounded up to a multiple of 2 (16-byte rows
+ * for bulk copies).  Returns 0 if n_planets is out of range. */
+int glisse_log_stride(int n_planets);
+
+/*
+ * Write the planet log the library itself would generate for the next n_steps steps
+ * (n_steps+1 records, layout above) into log (host or device) WITHOUT changing the simulation.
+ * Used to check the planet-history kernel (a1) against the oracle.  Synchronises.
+ */
+int glisse_planet_log(glisse_sim* sim, long long n_steps, double* log);
+
+/*
+ * Read the particle state in ORIGINAL particle order (compaction is invisible).
+ * Any of pos, vel, flag, removal_step may be NULL (skipped); pos/vel are three pointers to
+ * arrays of N doubles; flag is int[N]; removal_step is long long[N] (number of completed steps
+ * when the particle was flagged, −1 while active).  Buffers host or device.  Synchronises.
+ * A removed particle reports the state frozen at its removal.
+ */
+int glisse_read(glisse_sim* sim, double* const pos[3], double* const vel[3],
+                int* flag, long long* removal_step);
+
+/* Heliocentric planet positions and velocities at the current step, [n_planets][3] each, host
+ * or device, either may be NULL.  Synchronises. */
+int glisse_read_planets(glisse_sim* sim, double* pos, double* vel);
+
+/* Number of particles with flag == 0 at the current step (synchronises); < 0 on error. */
+long long glisse_active_count(glisse_sim* sim);
+
+/* Number of steps completed since create (host counter, no synchronisation); < 0 on error. */
+long long glisse_step(glisse_sim* sim);
+
+/* Particle-steps actually integrated so far = Σ over steps of the number of particles that were
+ * still active when the step began (the "useful work" of BASELINE.json's metric). Synchronises. */
+long long glisse_particle_steps(glisse_sim* sim);
+
+/* Number of kernels the library has launched for this sim so far (bench.py's gpu_launches). */
+long long glisse_launch_count(glisse_sim* sim);
+
+/* Block until all enqueued work of this sim has finished; returns its sticky status. */
+int glisse_sync(glisse_sim* sim);
+
+/* Device time in milliseconds spent in particle kernels since the last call (or since create),
+ * measured with CUDA events recorded on the sim's own stream around every particle-kernel
+ * launch, and the number of such launches.  Synchronises.  Used by bench.py's roofline. */
+int glisse_particle_kernel_time(glisse_sim* sim, double* ms, long long* launches);
+
+/*
+ * Measure this GPU's plain FP64 FMA rate with a register-resident DFMA loop (no memory
+ * traffic): returns the achieved FLOP/s (2 per DFMA) in *flops over a kernel of roughly
+ * `millis` milliseconds on `device`, `stream` may be NULL.  This is the roofline denominator
+ * of the ALU-bound particle kernel (MEASURED_PEAKS.json has no FP64 figure).
+ */
+int glisse_fp64_peak_probe(int device, void* stream, double millis, double* flops);
+
+void glisse_destroy(glisse_sim* sim);
+
+/* Static string for a status code. */
+const char* glisse_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GLISSE_H_ */

@@ -1,0 +1,501 @@
+/*
+ * glisse_oracle.cpp — the ORACLE: a plain, slow, single-threaded fp64 CPU implementation of the
+ * GLISSE test-particle integrator, written from the paper (Zhang & Gladman 2020, PAPER.md) and
+ * the readings listed in DESIGN.md §2.
+ *
+ * THIS IS TEST INFRASTRUCTURE.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * `--impl reference` legs may build, load or call it.  It shares no code, header, table or helper
+ * with the CUDA path under paper_2011_03484_b200/csrc/, and neither side includes the other.
+ *
+ * Style: the algorithm step by step in the paper's order and notation; no blocking, fusion,
+ * reordering, vectorisation or early exit.  Build: g++ -O2 -ffp-contract=off (no FMA
+ * contraction), libm sin/cos/sqrt.
+ *
+ * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): two-body closed form (T1), single-planet
+ * Kepler orbit (T2), finite-difference gradient of H_int vs the planet kick (T3), CR3BP Jacobi
+ * constant bounded and O(dt^2) (T4), time reversal (T5), order-2 convergence to a brute-force
+ * high-order direct integration (T6), the paper's 5-iteration / 1e-14 claim (T7),
+ * removal logic on crafted inputs (T8).  Parity unpinned: none of the functions below; the
+ * paper's application-level numbers (10.8 % librators …) are unpinned because the authors'
+ * initial conditions are not available.
+ *
+ * Notation: mu0 = G m0 (star); mu_j = G m_j, j = 0..Np-1 in Jacobi order (innermost first,
+ * PAPER.md:87); q_j, qd_j heliocentric planet position / velocity; r, v heliocentric particle
+ * position / velocity; dt the fixed step.
+ */
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+namespace {
+
+constexpr int kMaxPlanets = 32;
+constexpr int kPlanetKeplerIters = 10; /* generous count for planets, O3 */
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+
+enum Flag { ACTIVE = 0, RMIN = 1, RMAX = 2, NONCONV = 3, UNBOUND = 4, PLANET0 = 16 };
+
+struct Params {
+  double r_min, r_max;
+  int kepler_iters;
+  double kepler_tol;
+};
+
+/* ---------------------------------------------------------------------------------------------
+ * O2. Kepler drift (PAPER.md:92-94 steps 2–4 and the Kepler equation at).
+ * Advance (r, v) along the two-body orbit about a point mass mu for time dt.
+ * Differenced form of Kepler's equation in x = E(t) − E(t0) (reading S4):
+ *     dM = n dt = x − ec sin x + es (1 − cos x),   ec = e cos E0,  es = e sin E0,
+ * solved by exactly `iters` Newton updates from the initial guess of reading S5, followed by the
+ * Gauss f and g functions.  Returns ACTIVE, UNBOUND (alpha <= 0, reading S8) or NONCONV
+ * (|residual| > tol, reading S6).  On a non-zero return r, v are left untouched.
+ * ------------------------------------------------------------------------------------------- */
+int kepler_drift(double mu, double r[3], double v[3], double dt, int iters, double tol) {
+  const double r0 = std::sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+  const double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+  const double u = r[0] * v[0] + r[1] * v[1] + r[2] * v[2];
+  const double alpha = 2.0 * mu / r0 - v2; /* = mu / a */
+  if (!(alpha > 0.0)) return UNBOUND;
+  const double a = mu / alpha;
+  const double n = std::sqrt(mu / (a * a * a));
+  const double ec = 1.0 - r0 / a;
+  const double es = u / (n * a * a);
+  const double e = std::sqrt(ec * ec + es * es);
+  const double ndt = n * dt;
+  const double dM = ndt - kTwoPi * std::nearbyint(ndt / kTwoPi); /* reading S9 */
+
+  /* initial guess, reading S5 */
+  const double q = r0 / a; /* = 1 − ec */
+  const double x1 = dM / q;
+  double x;
+  if (std::fabs(es) * std::fabs(x1) < 0.25 * q && e * x1 * x1 < 0.25 * q) {
+    x = x1;
+  } else {
+    const double y = dM - es;
+    const double sg = es * std::cos(y) + ec * std::sin(y);
+    x = y + (sg >= 0.0 ? 0.85 : -0.85) * e;
+  }
+
+  /* fixed number of Newton updates */
+  for (int it = 0; it < iters; ++it) {
+    const double s = std::sin(x), c = std::cos(x);
+    const double f = x - ec * s + es * (1.0 - c) - dM;
+    const double fp = 1.0 - ec * c + es * s;
+    x = x - f / fp;
+  }
+  const double s = std::sin(x), c = std::cos(x);
+  const double res = x - ec * s + es * (1.0 - c) - dM;
+  if (!(std::fabs(res) <= tol)) return NONCONV;
+
+  /* Gauss f, g functions (BASELINE.json north_star; Danby, Fundamentals of Celestial Mechanics §6.7) */
+  const double p = 1.0 - ec * c + es * s; /* r(t)/a */
+  const double fg_f = 1.0 + (c - 1.0) * a / r0;
+  const double fg_g = (dM - x + s) / n; /* = dt + (s − x)/n with dM in place of n dt (S9) */
+  const double fg_fd = -n * s * a / (r0 * p);
+  const double fg_gd = 1.0 + (c - 1.0) / p;
+  for (int k = 0; k < 3; ++k) {
+    const double rk = r[k], vk = v[k];
+    r[k] = fg_f * rk + fg_g * vk;
+    v[k] = fg_fd * rk + fg_gd * vk;
+  }
+  return ACTIVE;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * h0, the common heliocentric term:  h0 = − sum_j mu_j q_j / |q_j|^3 .
+ * ------------------------------------------------------------------------------------------- */
+void common_term_h0(int np, const double* gm, const double* q, double h0[3]) {
+  h0[0] = h0[1] = h0[2] = 0.0;
+  for (int j = 0; j < np; ++j) {
+    const double* qj = q + 3 * j;
+    const double d2 = qj[0] * qj[0] + qj[1] * qj[1] + qj[2] * qj[2];
+    const double d = std::sqrt(d2);
+    const double w = gm[j] / (d2 * d);
+    for (int k = 0; k < 3; ++k) h0[k] -= w * qj[k];
+  }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O3. One Wisdom–Holman step of the planets ("standard Wisdom-Holman mixed-variable
+ * symplectic algorithm"), Jacobi coordinates, reading S14.
+ *   eta_k = m0 + sum_{i<=k} m_i  (eta_{-1} = m0); all masses enter as G m.
+ *   Jacobi position  r'_k = q_k − (sum_{i<k} m_i q_i) / eta_{k-1}   (same map for velocities)
+ *   inverse          q_k  = r'_k + sum_{i<k} (m_i / eta_i) r'_i
+ *   H_int = sum_k G m_k m0 (1/|r'_k| − 1/|q_k|) − sum_{i<j} G m_i m_j / |q_i − q_j|
+ *   kick  v'_k += h (eta_k/eta_{k-1}) [ mu0 r'_k/|r'_k|^3 + A_k + (1/eta_k) sum_{i>k} m_i A_i ],
+ *         A_i = − mu0 q_i/|q_i|^3 − sum_{j != i} mu_j (q_i − q_j)/|q_i − q_j|^3
+ *   drift of planet k: two-body motion in (r'_k, v'_k) with mu = mu0 eta_k / eta_{k-1}.
+ * Returns 0, or the 1-based index of the first planet whose drift failed.
+ * ------------------------------------------------------------------------------------------- */
+void helio_to_jacobi(int np, double gm0, const double* gm, const double* h, double* jac) {
+  double sum[3] = {0.0, 0.0, 0.0}; /* sum_{i<k} m_i h_i */
+  double eta = gm0;                /* eta_{k-1} */
+  for (int k = 0; k < np; ++k) {
+    for (int c = 0; c < 3; ++c) jac[3 * k + c] = h[3 * k + c] - sum[c] / eta;
+    for (int c = 0; c < 3; ++c) sum[c] += gm[k] * h[3 * k + c];
+    eta += gm[k];
+  }
+}
+
+void jacobi_to_helio(int np, double gm0, const double* gm, const double* jac, double* h) {
+  double sum[3] = {0.0, 0.0, 0.0}; /* sum_{i<k} (m_i/eta_i) r'_i */
+  double eta = gm0;
+  for (int k = 0; k < np; ++k) {
+    for (int c = 0; c < 3; ++c) h[3 * k + c] = jac[3 * k + c] + sum[c];
+    eta += gm[k]; /* eta_k */
+    for (int c = 0; c < 3; ++c) sum[c] += gm[k] / eta * jac[3 * k + c];
+  }
+}
+
+/* Jacobi accelerations dv'_k/dt = −(1/m'_k) dH_int/dr'_k, m'_k = m_k eta_{k-1}/eta_k. */
+void planet_kick_accel(int np, double gm0, const double* gm, const double* q, const double* rj,
+                       double* acc) {
+  std::vector<double> A(3 * np, 0.0);
+  for (int i = 0; i < np; ++i) {
+    const double* qi = q + 3 * i;
+    const double d2 = qi[0] * qi[0] + qi[1] * qi[1] + qi[2] * qi[2];
+    const double d = std::sqrt(d2);
+    const double w = gm0 / (d2 * d);
+    for (int c = 0; c < 3; ++c) A[3 * i + c] = -w * qi[c];
+    for (int j = 0; j < np; ++j) {
+      if (j == i) continue;
+      const double* qj = q + 3 * j;
+      const double dx[3] = {qi[0] - qj[0], qi[1] - qj[1], qi[2] - qj[2]};
+      const double s2 = dx[0] * dx[0] + dx[1] * dx[1] + dx[2] * dx[2];
+      const double s = std::sqrt(s2);
+      const double wj = gm[j] / (s2 * s);
+      for (int c = 0; c < 3; ++c) A[3 * i + c] -= wj * dx[c];
+    }
+  }
+  double eta_prev = gm0;
+  for (int k = 0; k < np; ++k) {
+    const double eta = eta_prev + gm[k];
+    const double* rk = rj + 3 * k;
+    const double d2 = rk[0] * rk[0] + rk[1] * rk[1] + rk[2] * rk[2];
+    const double d = std::sqrt(d2);
+    const double w = gm0 / (d2 * d);
+    double tail[3] = {0.0, 0.0, 0.0}; /* sum_{i>k} m_i A_i */
+    for (int i = k + 1; i < np; ++i)
+      for (int c = 0; c < 3; ++c) tail[c] += gm[i] * A[3 * i + c];
+    for (int c = 0; c < 3; ++c)
+      acc[3 * k + c] = (eta / eta_prev) * (w * rk[c] + A[3 * k + c] + tail[c] / eta);
+    eta_prev = eta;
+  }
+}
+
+int planet_step(int np, double gm0, const double* gm, double* q, double* qd, double dt) {
+  if (np == 0) return 0;
+  std::vector<double> rj(3 * np), vj(3 * np), acc(3 * np);
+  helio_to_jacobi(np, gm0, gm, q, rj.data());
+  helio_to_jacobi(np, gm0, gm, qd, vj.data());
+  /* kick 1/2 */
+  planet_kick_accel(np, gm0, gm, q, rj.data(), acc.data());
+  for (int i = 0; i < 3 * np; ++i) vj[i] += 0.5 * dt * acc[i];
+  /* drift 1 */
+  double eta_prev = gm0;
+  for (int k = 0; k < np; ++k) {
+    const double eta = eta_prev + gm[k];
+    const double mu = gm0 * eta / eta_prev;
+    const int st = kepler_drift(mu, &rj[3 * k], &vj[3 * k], dt, kPlanetKeplerIters, 1e-13);
+    if (st != ACTIVE) return k + 1;
+    eta_prev = eta;
+  }
+  /* kick 1/2 at the new positions */
+  jacobi_to_helio(np, gm0, gm, rj.data(), q);
+  planet_kick_accel(np, gm0, gm, q, rj.data(), acc.data());
+  for (int i = 0; i < 3 * np; ++i) vj[i] += 0.5 * dt * acc[i];
+  jacobi_to_helio(np, gm0, gm, vj.data(), qd);
+  return 0;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O1/O4/O5. One force evaluation on a particle with the tests of PAPER.md:125-127 ("while
+ * computing the acceleration").  Returns the flag that fires (priority: r_min, r_max, lowest
+ * planet index; reading S11) or ACTIVE with the acceleration
+ *     a = h0 − sum_j mu_j (r − q_j)/|r − q_j|^3
+ * ------------------------------------------------------------------------------------------- */
+int particle_accel(int np, const double* gm, const double* q, const double h0[3],
+                   const double* rcrit2, const Params& P, const double r[3], double a[3]) {
+  const double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+  if (P.r_min > 0.0 && r2 < P.r_min * P.r_min) return RMIN;
+  if (P.r_max > 0.0 && r2 > P.r_max * P.r_max) return RMAX;
+  a[0] = h0[0]; a[1] = h0[1]; a[2] = h0[2];
+  int hit = ACTIVE;
+  for (int j = 0; j < np; ++j) {
+    const double d[3] = {r[0] - q[3 * j], r[1] - q[3 * j + 1], r[2] - q[3 * j + 2]};
+    const double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    if (hit == ACTIVE && d2 < rcrit2[j]) hit = PLANET0 + j;
+    const double dd = std::sqrt(d2);
+    const double w = gm[j] / (d2 * dd);
+    for (int k = 0; k < 3; ++k) a[k] -= w * d[k];
+  }
+  return hit;
+}
+
+struct Sim {
+  double gm0 = 0.0;
+  int np = 0;
+  std::vector<double> gm, q, qd, rcrit2;
+  long long n = 0;
+  std::vector<double> x[3], v[3];
+  std::vector<int> flag;
+  std::vector<long long> rstep;
+  double dt = 0.0;
+  Params P{};
+  long long step = 0;
+  long long particle_steps = 0;
+};
+
+/* kick every active particle by h·a evaluated with planets (q, h0); `completed` = number of
+ * completed steps to record on a hit (reading S12) */
+void kick_particles(Sim& S, const double* q, const double h0[3], double h, long long completed) {
+  for (long long i = 0; i < S.n; ++i) {
+    if (S.flag[i] != ACTIVE) continue;
+    const double r[3] = {S.x[0][i], S.x[1][i], S.x[2][i]};
+    double a[3];
+    const int hit = particle_accel(S.np, S.gm.data(), q, h0, S.rcrit2.data(), S.P, r, a);
+    if (hit != ACTIVE) {
+      S.flag[i] = hit;
+      S.rstep[i] = completed;
+      continue; /* frozen: the kick of this evaluation is NOT applied (O5) */
+    }
+    for (int k = 0; k < 3; ++k) S.v[k][i] += h * a[k];
+  }
+}
+
+void drift_particles(Sim& S) {
+  for (long long i = 0; i < S.n; ++i) {
+    if (S.flag[i] != ACTIVE) continue;
+    double r[3] = {S.x[0][i], S.x[1][i], S.x[2][i]};
+    double v[3] = {S.v[0][i], S.v[1][i], S.v[2][i]};
+    const int st = kepler_drift(S.gm0, r, v, S.dt, S.P.kepler_iters, S.P.kepler_tol);
+    if (st != ACTIVE) {
+      S.flag[i] = st;
+      S.rstep[i] = S.step; /* flagged during step `step`: that many steps were completed */
+      continue;
+    }
+    for (int k = 0; k < 3; ++k) { S.x[k][i] = r[k]; S.v[k][i] = v[k]; }
+  }
+}
+
+long long count_active(const Sim& S) {
+  long long c = 0;
+  for (long long i = 0; i < S.n; ++i) c += (S.flag[i] == ACTIVE);
+  return c;
+}
+
+int log_stride(int np) { return (3 * (np + 1) + 1) & ~1; }
+
+bool all_finite(const double* p, long long n) {
+  for (long long i = 0; i < n; ++i)
+    if (!std::isfinite(p[i])) return false;
+  return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+struct oracle_sim;
+
+typedef struct {
+  double r_min, r_max;
+  int kepler_iters;
+  double kepler_tol;
+} oracle_params;
+
+void oracle_default_params(oracle_params* p) {
+  if (!p) return;
+  p->r_min = 0.0;
+  p->r_max = std::numeric_limits<double>::infinity();
+  p->kepler_iters = 5;
+  p->kepler_tol = 1e-14;
+}
+
+int oracle_log_stride(int n_planets) {
+  return (n_planets < 0 || n_planets > kMaxPlanets) ? 0 : log_stride(n_planets);
+}
+
+int oracle_create(oracle_sim** out, double gm_star, int n_planets, const double* gm_planet,
+                  const double* planet_pos, const double* planet_vel, const double* planet_rcrit,
+                  long long n_particles, const double* const pos[3], const double* const vel[3],
+                  double dt, const oracle_params* params) {
+  if (!out) return -1;
+  *out = nullptr;
+  if (n_planets < 0 || n_planets > kMaxPlanets || n_particles < 1 || !pos || !vel) return -1;
+  if (!(gm_star > 0.0) || !std::isfinite(gm_star) || dt == 0.0 || !std::isfinite(dt)) return -1;
+  if (n_planets > 0 && (!gm_planet || !planet_pos || !planet_vel)) return -1;
+  for (int k = 0; k < 3; ++k)
+    if (!pos[k] || !vel[k] || !all_finite(pos[k], n_particles) || !all_finite(vel[k], n_particles))
+      return -1;
+  if (n_planets > 0 && (!all_finite(gm_planet, n_planets) || !all_finite(planet_pos, 3 * n_planets) ||
+                        !all_finite(planet_vel, 3 * n_planets)))
+    return -1;
+  Sim* S = new (std::nothrow) Sim;
+  if (!S) return -3;
+  S->gm0 = gm_star;
+  S->np = n_planets;
+  S->gm.assign(gm_planet, gm_planet + n_planets);
+  for (int j = 0; j < n_planets; ++j)
+    if (!(S->gm[j] > 0.0)) { delete S; return -1; }
+  S->q.assign(planet_pos, planet_pos + 3 * n_planets);
+  S->qd.assign(planet_vel, planet_vel + 3 * n_planets);
+  S->rcrit2.assign(n_planets, 0.0);
+  if (planet_rcrit)
+    for (int j = 0; j < n_planets; ++j) S->rcrit2[j] = planet_rcrit[j] * planet_rcrit[j];
+  S->n = n_particles;
+  for (int k = 0; k < 3; ++k) {
+    S->x[k].assign(pos[k], pos[k] + n_particles);
+    S->v[k].assign(vel[k], vel[k] + n_particles);
+  }
+  S->flag.assign(n_particles, ACTIVE);
+  S->rstep.assign(n_particles, -1);
+  S->dt = dt;
+  oracle_params d;
+  oracle_default_params(&d);
+  if (params) d = *params;
+  if (d.kepler_iters < 0 || !(d.kepler_tol > 0.0)) { delete S; return -1; }
+  S->P.r_min = d.r_min;
+  S->P.r_max = (std::isfinite(d.r_max) ? d.r_max : 0.0);
+  S->P.kepler_iters = d.kepler_iters;
+  S->P.kepler_tol = d.kepler_tol;
+  *out = reinterpret_cast<oracle_sim*>(S);
+  return 0;
+}
+
+/* One full step s -> s+1 for everything, in the order O1, O2, O3, O4 of DESIGN.md §2. */
+int oracle_advance(oracle_sim* sim, long long n_steps) {
+  if (!sim || n_steps < 0) return -1;
+  Sim& S = *reinterpret_cast<Sim*>(sim);
+  const double h = 0.5 * S.dt;
+  double h0[3];
+  for (long long s = 0; s < n_steps; ++s) {
+    /* O1: opening half kick, planets at t_s */
+    common_term_h0(S.np, S.gm.data(), S.q.data(), h0);
+    kick_particles(S, S.q.data(), h0, h, S.step);
+    S.particle_steps += count_active(S);
+    /* O2: drift */
+    drift_particles(S);
+    /* O3: planets t_s -> t_{s+1} */
+    const int bad = planet_step(S.np, S.gm0, S.gm.data(), S.q.data(), S.qd.data(), S.dt);
+    if (bad) return -4;
+    /* O4: closing half kick, planets at t_{s+1} */
+    common_term_h0(S.np, S.gm.data(), S.q.data(), h0);
+    kick_particles(S, S.q.data(), h0, h, S.step + 1);
+    S.step += 1;
+  }
+  return 0;
+}
+
+/* Planet log for the next n_steps steps: n_steps+1 records of oracle_log_stride(np) doubles
+ * [q_0 … q_{Np-1}, h0, pad] at times t_s … t_{s+n}.  The simulation is not
+ * changed. */
+int oracle_planet_log(oracle_sim* sim, long long n_steps, double* log) {
+  if (!sim || n_steps < 0 || !log) return -1;
+  const Sim& S = *reinterpret_cast<Sim*>(sim);
+  std::vector<double> q = S.q, qd = S.qd;
+  const int st = log_stride(S.np);
+  for (long long s = 0; s <= n_steps; ++s) {
+    double* rec = log + s * st;
+    for (int i = 0; i < st; ++i) rec[i] = 0.0;
+    for (int i = 0; i < 3 * S.np; ++i) rec[i] = q[i];
+    common_term_h0(S.np, S.gm.data(), q.data(), rec + 3 * S.np);
+    if (s < n_steps) {
+      const int bad = planet_step(S.np, S.gm0, S.gm.data(), q.data(), qd.data(), S.dt);
+      if (bad) return -4;
+    }
+  }
+  return 0;
+}
+
+/* Particles only, planets taken from a caller-supplied log; planet state unchanged. */
+int oracle_advance_with_log(oracle_sim* sim, long long n_steps, const double* log) {
+  if (!sim || n_steps < 0 || !log) return -1;
+  Sim& S = *reinterpret_cast<Sim*>(sim);
+  const double h = 0.5 * S.dt;
+  const int st = log_stride(S.np);
+  for (long long s = 0; s < n_steps; ++s) {
+    const double* r0 = log + s * st;
+    const double* r1 = log + (s + 1) * st;
+    kick_particles(S, r0, r0 + 3 * S.np, h, S.step);
+    S.particle_steps += count_active(S);
+    drift_particles(S);
+    kick_particles(S, r1, r1 + 3 * S.np, h, S.step + 1);
+    S.step += 1;
+  }
+  return 0;
+}
+
+int oracle_read(oracle_sim* sim, double* const pos[3], double* const vel[3], int* flag,
+                long long* removal_step) {
+  if (!sim) return -1;
+  const Sim& S = *reinterpret_cast<Sim*>(sim);
+  for (int k = 0; k < 3; ++k) {
+    if (pos && pos[k]) std::memcpy(pos[k], S.x[k].data(), sizeof(double) * S.n);
+    if (vel && vel[k]) std::memcpy(vel[k], S.v[k].data(), sizeof(double) * S.n);
+  }
+  if (flag) std::memcpy(flag, S.flag.data(), sizeof(int) * S.n);
+  if (removal_step) std::memcpy(removal_step, S.rstep.data(), sizeof(long long) * S.n);
+  return 0;
+}
+
+int oracle_read_planets(oracle_sim* sim, double* pos, double* vel) {
+  if (!sim) return -1;
+  const Sim& S = *reinterpret_cast<Sim*>(sim);
+  if (pos) std::memcpy(pos, S.q.data(), sizeof(double) * 3 * S.np);
+  if (vel) std::memcpy(vel, S.qd.data(), sizeof(double) * 3 * S.np);
+  return 0;
+}
+
+long long oracle_active_count(oracle_sim* sim) {
+  return sim ? count_active(*reinterpret_cast<Sim*>(sim)) : -1;
+}
+long long oracle_step(oracle_sim* sim) { return sim ? reinterpret_cast<Sim*>(sim)->step : -1; }
+long long oracle_particle_steps(oracle_sim* sim) {
+  return sim ? reinterpret_cast<Sim*>(sim)->particle_steps : -1;
+}
+void oracle_destroy(oracle_sim* sim) { delete reinterpret_cast<Sim*>(sim); }
+
+/* ---- single functions exposed so the pins can test each part on its own -------------------- */
+
+/* O2 on one body; returns the flag (0, 3 or 4). */
+int oracle_kepler_drift(double mu, double* r, double* v, double dt, int iters, double tol) {
+  return kepler_drift(mu, r, v, dt, iters, tol);
+}
+
+/* O3 kick accelerations in Jacobi coordinates for heliocentric positions q [np][3]. */
+int oracle_planet_kick_accel(int np, double gm0, const double* gm, const double* q, double* acc) {
+  if (np < 0 || np > kMaxPlanets) return -1;
+  std::vector<double> rj(3 * np);
+  helio_to_jacobi(np, gm0, gm, q, rj.data());
+  planet_kick_accel(np, gm0, gm, q, rj.data(), acc);
+  return 0;
+}
+
+void oracle_helio_to_jacobi(int np, double gm0, const double* gm, const double* h, double* jac) {
+  helio_to_jacobi(np, gm0, gm, h, jac);
+}
+void oracle_jacobi_to_helio(int np, double gm0, const double* gm, const double* jac, double* h) {
+  jacobi_to_helio(np, gm0, gm, jac, h);
+}
+
+/* One O3 step on caller arrays. */
+int oracle_planet_step(int np, double gm0, const double* gm, double* q, double* qd, double dt) {
+  return planet_step(np, gm0, gm, q, qd, dt);
+}
+
+/* O1/O5 on one particle: returns the flag, fills a[3] when it is 0. */
+int oracle_particle_accel(int np, const double* gm, const double* q, const double* rcrit,
+                          double r_min, double r_max, const double* r, double* a) {
+  Params P{r_min, std::isfinite(r_max) ? r_max : 0.0, 5, 1e-14};
+  std::vector<double> rc2(np);
+  for (int j = 0; j < np; ++j) rc2[j] = rcrit ? rcrit[j] * rcrit[j] : 0.0;
+  double h0[3];
+  common_term_h0(np, gm, q, h0);
+  return particle_accel(np, gm, q, h0, rc2.data(), P, r, a);
+}
+
+}  // extern "C"

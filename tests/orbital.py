@@ -1,0 +1,32 @@
+"""Textbook two-body helpers used by the pins (independent of oracle/ and of the CUDA path)."""
+import numpy as np
+
+
+def cartesian_to_elements(mu, r, v):
+    """r, v: [...,3] -> dict of a, e, inc, Omega, omega, M (Murray & Dermott §2.8)."""
+    r = np.asarray(r, dtype=np.float64)
+    v = np.asarray(v, dtype=np.float64)
+    rn = np.linalg.norm(r, axis=-1)
+    v2 = np.sum(v * v, axis=-1)
+    h = np.cross(r, v)
+    hn = np.linalg.norm(h, axis=-1)
+    a = 1.0 / (2.0 / rn - v2 / mu)
+    evec = np.cross(v, h) / mu - r / rn[..., None]
+    e = np.linalg.norm(evec, axis=-1)
+    inc = np.arccos(np.clip(h[..., 2] / hn, -1, 1))
+    Omega = np.arctan2(h[..., 0], -h[..., 1])
+    node = np.stack([np.cos(Omega), np.sin(Omega), np.zeros_like(Omega)], axis=-1)
+    # argument of latitude of pericentre measured in the orbital plane
+    m = np.cross(h / hn[..., None], node)
+    omega = np.arctan2(np.sum(evec * m, axis=-1), np.sum(evec * node, axis=-1))
+    # eccentric anomaly from e cos E = 1 - r/a, e sin E = r.v / sqrt(mu a)
+    ecE = 1.0 - rn / a
+    esE = np.sum(r * v, axis=-1) / np.sqrt(mu * a)
+    E = np.arctan2(esE, ecE)
+    M = E - esE
+    return dict(a=a, e=e, inc=inc, Omega=np.mod(Omega, 2 * np.pi), omega=np.mod(omega, 2 * np.pi),
+                M=np.mod(M, 2 * np.pi))
+
+
+def angle_diff(a, b):
+    return np.abs((a - b + np.pi) % (2 * np.pi) - np.pi)
