@@ -170,6 +170,15 @@ int glisse_particle_kernel_time(glisse_sim* sim, double* ms, long long* launches
  */
 int glisse_fp64_peak_probe(int device, void* stream, double millis, double* flops);
 
+/*
+ * Test hook: evaluate one device primitive of the CUDA path on an array, on device 0.
+ * in/out are HOST or device arrays.  which = 0 rsqrt (in[n] -> out[n]), 1 reciprocal, 2 reciprocal
+ * to 2^-39 (Newton updates only), 3 sin x - x and cos x - 1 (in[n] -> out[2n], interleaved),
+ * 4 one Kepler drift (step a5) per body: in[10n] = {mu, dt, kepler_iters, kepler_tol, x, y, z, vx,
+ * vy, vz}, out[7n] = {flag, x, y, z, vx, vy, vz}.  Synchronises.
+ */
+int glisse_test_primitive(int which, long long n, const double* in, double* out);
+
 void glisse_destroy(glisse_sim* sim);
 
 /* Static string for a status code. */

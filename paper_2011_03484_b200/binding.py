@@ -1,0 +1,272 @@
+"""Thin ctypes binding over the C-ABI library (include/glisse.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; this module holds no arithmetic of the
+method and has no CPU fallback: if libglisse.so is missing and cannot be built with nvcc, or no
+CUDA device is usable, it raises.  Names follow the C ABI: GlisseSim.create/advance/read ...
+
+Host inputs are numpy float64 arrays; device inputs are torch CUDA float64 tensors (PyTorch is
+used for device memory and streams only).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_double, c_int, c_longlong, c_void_p
+
+import numpy as np
+
+from . import build as _build
+
+OK, EINVAL, ECUDA, ENOMEM, EPLANET = 0, -1, -2, -3, -4
+FLAG_ACTIVE, FLAG_RMIN, FLAG_RMAX, FLAG_NONCONV, FLAG_UNBOUND, FLAG_PLANET0 = 0, 1, 2, 3, 4, 16
+
+#: every symbol include/glisse.h declares (tests check that the library exports each one)
+EXPORTS = (
+    "glisse_default_params", "glisse_create", "glisse_advance", "glisse_advance_with_log",
+    "glisse_log_stride", "glisse_planet_log", "glisse_read", "glisse_read_planets",
+    "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_launch_count", "glisse_sync",
+    "glisse_particle_kernel_time", "glisse_fp64_peak_probe", "glisse_test_primitive", "glisse_destroy",
+    "glisse_strerror",
+)
+
+
+class GlisseParams(ctypes.Structure):
+    _fields_ = [("r_min", c_double), ("r_max", c_double), ("kepler_iters", c_int), ("kepler_tol", c_double),
+                ("chunk_steps", c_int), ("resync_chunks", c_int), ("device", c_int), ("stream", c_void_p)]
+
+
+class GlisseError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: {strerror(status)} (status {status})")
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load libglisse.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        P3 = POINTER(c_void_p)
+        L.glisse_default_params.argtypes = [POINTER(GlisseParams)]
+        L.glisse_default_params.restype = None
+        L.glisse_create.argtypes = [POINTER(c_void_p), c_double, c_int, c_void_p, c_void_p, c_void_p, c_void_p,
+                                    c_longlong, P3, P3, c_double, POINTER(GlisseParams)]
+        L.glisse_create.restype = c_int
+        L.glisse_advance.argtypes = [c_void_p, c_longlong]
+        L.glisse_advance.restype = c_int
+        L.glisse_advance_with_log.argtypes = [c_void_p, c_longlong, c_void_p]
+        L.glisse_advance_with_log.restype = c_int
+        L.glisse_log_stride.argtypes = [c_int]
+        L.glisse_log_stride.restype = c_int
+        L.glisse_planet_log.argtypes = [c_void_p, c_longlong, c_void_p]
+        L.glisse_planet_log.restype = c_int
+        L.glisse_read.argtypes = [c_void_p, P3, P3, c_void_p, c_void_p]
+        L.glisse_read.restype = c_int
+        L.glisse_read_planets.argtypes = [c_void_p, c_void_p, c_void_p]
+        L.glisse_read_planets.restype = c_int
+        for name in ("glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_launch_count"):
+            getattr(L, name).argtypes = [c_void_p]
+            getattr(L, name).restype = c_longlong
+        L.glisse_sync.argtypes = [c_void_p]
+        L.glisse_sync.restype = c_int
+        L.glisse_particle_kernel_time.argtypes = [c_void_p, POINTER(c_double), POINTER(c_longlong)]
+        L.glisse_particle_kernel_time.restype = c_int
+        L.glisse_fp64_peak_probe.argtypes = [c_int, c_void_p, c_double, POINTER(c_double)]
+        L.glisse_fp64_peak_probe.restype = c_int
+        L.glisse_test_primitive.argtypes = [c_int, c_longlong, c_void_p, c_void_p]
+        L.glisse_test_primitive.restype = c_int
+        L.glisse_destroy.argtypes = [c_void_p]
+        L.glisse_destroy.restype = None
+        L.glisse_strerror.argtypes = [c_int]
+        L.glisse_strerror.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return lib().glisse_strerror(int(status)).decode()
+
+
+def log_stride(n_planets: int) -> int:
+    return lib().glisse_log_stride(int(n_planets))
+
+
+def _check(status, where):
+    if status != OK:
+        raise GlisseError(status, where)
+
+
+def _is_torch(t) -> bool:
+    return type(t).__module__.startswith("torch")
+
+
+def _ptr(a):
+    """Raw address of a numpy array or torch tensor (None -> NULL)."""
+    if a is None:
+        return None
+    if _is_torch(a):
+        return c_void_p(a.data_ptr())
+    return c_void_p(a.ctypes.data)
+
+
+def _rows(a, n_rows):
+    """Three (or n_rows) contiguous float64 rows of a [n_rows, N] numpy array or torch tensor."""
+    if _is_torch(a):
+        import torch
+        assert a.dtype == torch.float64 and a.shape[0] == n_rows
+        a = a.contiguous()
+        return a, [a[k] for k in range(n_rows)]
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    assert a.shape[0] == n_rows
+    return a, [a[k] for k in range(n_rows)]
+
+
+def _p3(rows):
+    return (c_void_p * 3)(*[(r.data_ptr() if _is_torch(r) else r.ctypes.data) for r in rows])
+
+
+class GlisseSim:
+    """glisse_create / glisse_advance / glisse_read with the C ABI's argument order."""
+
+    def __init__(self, gm_star, gm_planet, planet_pos, planet_vel, planet_rcrit, pos, vel, dt, *, r_min=0.0,
+                 r_max=float("inf"), kepler_iters=5, kepler_tol=1e-14, chunk_steps=1024, resync_chunks=1,
+                 device=0, stream=None):
+        L = lib()
+        gm_planet = np.ascontiguousarray(gm_planet, dtype=np.float64).reshape(-1)
+        self.n_planets = int(gm_planet.shape[0])
+        planet_pos = np.ascontiguousarray(planet_pos, dtype=np.float64).reshape(self.n_planets, 3)
+        planet_vel = np.ascontiguousarray(planet_vel, dtype=np.float64).reshape(self.n_planets, 3)
+        rcrit = None if planet_rcrit is None else np.ascontiguousarray(planet_rcrit, dtype=np.float64).reshape(
+            self.n_planets)
+        keep_p, prow = _rows(pos, 3)
+        keep_v, vrow = _rows(vel, 3)
+        self.n = int(prow[0].shape[0])
+        self.device = int(device)
+        prm = GlisseParams()
+        L.glisse_default_params(byref(prm))
+        prm.r_min, prm.r_max = float(r_min), float(r_max)
+        prm.kepler_iters, prm.kepler_tol = int(kepler_iters), float(kepler_tol)
+        prm.chunk_steps, prm.resync_chunks = int(chunk_steps), int(resync_chunks)
+        prm.device = self.device
+        prm.stream = None if stream is None else c_void_p(int(stream))
+        h = c_void_p()
+        st = L.glisse_create(byref(h), float(gm_star), self.n_planets, _ptr(gm_planet), _ptr(planet_pos),
+                             _ptr(planet_vel), _ptr(rcrit), self.n, _p3(prow), _p3(vrow), float(dt), byref(prm))
+        self._h = None
+        _check(st, "glisse_create")
+        self._h = h
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        kw.setdefault("chunk_steps", w.chunk_steps)
+        return cls(w.gm_star, w.gm_planet, w.planet_pos, w.planet_vel, w.planet_rcrit, w.pos, w.vel, w.dt,
+                   r_min=w.r_min, r_max=w.r_max, **kw)
+
+    # ---- the calls of include/glisse.h ---------------------------------------------------------
+    def advance(self, n_steps):
+        _check(lib().glisse_advance(self._h, int(n_steps)), "glisse_advance")
+
+    def advance_with_log(self, n_steps, log):
+        if not _is_torch(log):
+            log = np.ascontiguousarray(log, dtype=np.float64)
+        assert log.shape[0] >= n_steps + 1
+        _check(lib().glisse_advance_with_log(self._h, int(n_steps), _ptr(log)), "glisse_advance_with_log")
+
+    def planet_log(self, n_steps):
+        out = np.zeros((int(n_steps) + 1, log_stride(self.n_planets)), dtype=np.float64)
+        _check(lib().glisse_planet_log(self._h, int(n_steps), _ptr(out)), "glisse_planet_log")
+        return out
+
+    def read(self, out=None):
+        """Returns (pos[3,N], vel[3,N], flag[N] int32, removal_step[N] int64) as host numpy arrays,
+        or fills the given (pos, vel, flag, removal_step) numpy arrays / torch CUDA tensors."""
+        if out is None:
+            pos = np.empty((3, self.n), dtype=np.float64)
+            vel = np.empty((3, self.n), dtype=np.float64)
+            flag = np.empty(self.n, dtype=np.int32)
+            rstep = np.empty(self.n, dtype=np.int64)
+        else:
+            pos, vel, flag, rstep = out
+        prow = None if pos is None else [pos[k] for k in range(3)]
+        vrow = None if vel is None else [vel[k] for k in range(3)]
+        st = lib().glisse_read(self._h, None if prow is None else _p3(prow), None if vrow is None else _p3(vrow),
+                               _ptr(flag), _ptr(rstep))
+        _check(st, "glisse_read")
+        return pos, vel, flag, rstep
+
+    def read_planets(self):
+        pos = np.empty((self.n_planets, 3), dtype=np.float64)
+        vel = np.empty((self.n_planets, 3), dtype=np.float64)
+        _check(lib().glisse_read_planets(self._h, _ptr(pos), _ptr(vel)), "glisse_read_planets")
+        return pos, vel
+
+    def _count(self, fn, where):
+        v = int(fn(self._h))
+        if v < 0:
+            raise GlisseError(v, where)
+        return v
+
+    def active_count(self):
+        return self._count(lib().glisse_active_count, "glisse_active_count")
+
+    def step(self):
+        return self._count(lib().glisse_step, "glisse_step")
+
+    def particle_steps(self):
+        return self._count(lib().glisse_particle_steps, "glisse_particle_steps")
+
+    def launch_count(self):
+        return self._count(lib().glisse_launch_count, "glisse_launch_count")
+
+    def sync(self):
+        _check(lib().glisse_sync(self._h), "glisse_sync")
+
+    def particle_kernel_time(self):
+        """(milliseconds, launches) spent in particle kernels since the last call."""
+        ms, n = c_double(), c_longlong()
+        _check(lib().glisse_particle_kernel_time(self._h, byref(ms), byref(n)), "glisse_particle_kernel_time")
+        return ms.value, n.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().glisse_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def fp64_peak_probe(device=0, millis=200.0, stream=None) -> float:
+    """Measured FP64 FMA rate of the device in FLOP/s (register-resident DFMA loop)."""
+    out = c_double()
+    st = lib().glisse_fp64_peak_probe(int(device), None if stream is None else c_void_p(int(stream)), float(millis),
+                                      byref(out))
+    _check(st, "glisse_fp64_peak_probe")
+    return out.value
+
+
+_PRIM = {"rsqrt": (0, 1, 1), "rcp": (1, 1, 1), "rcp1": (2, 1, 1), "sincosm": (3, 1, 2), "kepler_drift": (4, 10, 7)}
+
+
+def test_primitive(name, x):
+    """Evaluate one device primitive on a host array (test hook of include/glisse.h)."""
+    which, n_in, n_out = _PRIM[name]
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    n = x.size // n_in
+    out = np.empty(n * n_out, dtype=np.float64)
+    _check(lib().glisse_test_primitive(which, n, _ptr(x), _ptr(out)), "glisse_test_primitive")
+    return out.reshape(n, n_out) if n_out > 1 else out
+
+
+test_primitive.__test__ = False  # not a pytest test

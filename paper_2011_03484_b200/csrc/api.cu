@@ -1,0 +1,704 @@
+// api.cu — the C ABI of include/glisse.h and the host driver behind it (layers A and B of
+// DESIGN.md §1): per-chunk schedule planet-history kernel (own stream, one chunk ahead, two log
+// buffers) -> particle kernel -> survivor compaction every R chunks
+// (PAPER.md:127), with CUDA events for the dependencies and no host synchronisation inside
+// glisse_advance.  Every step of the path runs in the kernels; there is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstddef>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+
+#include "glisse_internal.cuh"
+
+using namespace glisse;
+
+namespace {
+
+struct LogBuffer {
+  double* log = nullptr;    // [(K+1) * stride]
+  double* jlog = nullptr;   // [(K+1) * 6 Np]   Jacobi state of the planets at every record
+  long long start = 0;      // step index of record 0
+  cudaEvent_t ready = nullptr;     // planet-history kernel that fills it has finished   (stream P)
+  cudaEvent_t consumed = nullptr;  // last particle kernel that reads it has finished    (stream Q)
+};
+
+struct TimedLaunch {
+  cudaEvent_t t0, t1;
+};
+
+}  // namespace
+
+struct glisse_sim {
+  int device = 0;
+  cudaStream_t q = nullptr;  // particle stream (the caller's, or owned)
+  cudaStream_t p = nullptr;  // planet-history stream (owned)
+  bool own_q = false;
+  int np = 0;
+  long long n = 0;
+  double dt = 0.0, gm0 = 0.0;
+  glisse_params prm{};
+  int K = 1024;
+  int stride = 0;
+  int status = GLISSE_OK;  // sticky
+
+  PlanetSystem* d_sys = nullptr;
+  double* d_j0 = nullptr;  // Jacobi state at create
+  LogBuffer buf[2];
+  int cur = 0;
+  long long step = 0;
+  bool external_log_used = false;
+
+  // particle state: two working sets (ping-pong for compaction) + original-order assembly arrays
+  double* work[2][6] = {};
+  int* id[2] = {};
+  int* flag[2] = {};
+  long long* rstep[2] = {};
+  double* fin[6] = {};
+  int* fin_flag = nullptr;
+  long long* fin_rstep = nullptr;
+  int* d_nslots = nullptr;  // [2], indexed like the working sets
+  int* d_block_counts = nullptr;
+  int w = 0;                // working set in use
+  int nslots_upper = 0;     // host upper bound of d_nslots[w]
+  int* h_nslots = nullptr;  // pinned
+  cudaEvent_t nslots_ready = nullptr;
+  bool nslots_pending = false;
+  int chunks_since_resync = 0;
+
+  unsigned long long* d_counters = nullptr;  // [0] particle-steps, [1] scratch for counts
+  long long launches = 0;
+
+  ParticleArgs pa{};
+  std::vector<TimedLaunch> timed_free, timed_busy;
+  double timed_ms = 0.0;
+  long long timed_launches = 0;
+};
+
+namespace {
+
+#define CK(call)                                 \
+  do {                                           \
+    cudaError_t e__ = (call);                    \
+    if (e__ != cudaSuccess) {                    \
+      (void)cudaGetLastError();                  \
+      return (e__ == cudaErrorMemoryAllocation) ? GLISSE_ENOMEM : GLISSE_ECUDA; \
+    }                                            \
+  } while (0)
+
+// same, for use after the sim exists: a failure is sticky
+#define CKS(sim, call)                           \
+  do {                                           \
+    cudaError_t e__ = (call);                    \
+    if (e__ != cudaSuccess) {                    \
+      (void)cudaGetLastError();                  \
+      (sim)->status = (e__ == cudaErrorMemoryAllocation) ? GLISSE_ENOMEM : GLISSE_ECUDA; \
+      return (sim)->status;                      \
+    }                                            \
+  } while (0)
+
+bool all_finite_host(const double* p, long long n) {
+  for (long long i = 0; i < n; ++i)
+    if (!std::isfinite(p[i])) return false;
+  return true;
+}
+
+bool is_device_pointer(const void* p) {
+  cudaPointerAttributes at{};
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return false;
+  }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+void free_sim(glisse_sim* s) {
+  if (!s) return;
+  cudaSetDevice(s->device);
+  if (s->q) cudaStreamSynchronize(s->q);
+  if (s->p) cudaStreamSynchronize(s->p);
+  for (int b = 0; b < 2; ++b) {
+    cudaFree(s->buf[b].log);
+    cudaFree(s->buf[b].jlog);
+    if (s->buf[b].ready) cudaEventDestroy(s->buf[b].ready);
+    if (s->buf[b].consumed) cudaEventDestroy(s->buf[b].consumed);
+    for (int k = 0; k < 6; ++k) cudaFree(s->work[b][k]);
+    cudaFree(s->id[b]);
+    cudaFree(s->flag[b]);
+    cudaFree(s->rstep[b]);
+  }
+  for (int k = 0; k < 6; ++k) cudaFree(s->fin[k]);
+  cudaFree(s->fin_flag);
+  cudaFree(s->fin_rstep);
+  cudaFree(s->d_nslots);
+  cudaFree(s->d_block_counts);
+  cudaFree(s->d_counters);
+  cudaFree(s->d_sys);
+  cudaFree(s->d_j0);
+  if (s->h_nslots) cudaFreeHost(s->h_nslots);
+  if (s->nslots_ready) cudaEventDestroy(s->nslots_ready);
+  for (auto& t : s->timed_free) { cudaEventDestroy(t.t0); cudaEventDestroy(t.t1); }
+  for (auto& t : s->timed_busy) { cudaEventDestroy(t.t0); cudaEventDestroy(t.t1); }
+  if (s->p) cudaStreamDestroy(s->p);
+  if (s->own_q && s->q) cudaStreamDestroy(s->q);
+  (void)cudaGetLastError();
+  delete s;
+}
+
+// collect finished timed launches (non-blocking unless `block`)
+void harvest_timings(glisse_sim* s, bool block) {
+  size_t kept = 0;
+  for (size_t i = 0; i < s->timed_busy.size(); ++i) {
+    TimedLaunch t = s->timed_busy[i];
+    cudaError_t e = block ? cudaEventSynchronize(t.t1) : cudaEventQuery(t.t1);
+    if (e == cudaSuccess) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, t.t0, t.t1) == cudaSuccess) {
+        s->timed_ms += ms;
+        s->timed_launches += 1;
+      }
+      s->timed_free.push_back(t);
+    } else {
+      (void)cudaGetLastError();
+      s->timed_busy[kept++] = t;
+    }
+  }
+  s->timed_busy.resize(kept);
+}
+
+int launch_particles(glisse_sim* s, const double* log, int nsteps) {
+  ParticleArgs& a = s->pa;
+  const int w = s->w;
+  for (int k = 0; k < 6; ++k) a.st[k] = s->work[w][k];
+  a.flag = s->flag[w];
+  a.rstep = s->rstep[w];
+  a.n_slots = s->d_nslots + w;
+  a.log = log;
+  a.step0 = s->step;
+  a.nsteps = nsteps;
+  // a newer survivor count may have arrived from the last compaction: shrink the grid (never blocks)
+  if (s->nslots_pending && cudaEventQuery(s->nslots_ready) == cudaSuccess) {
+    s->nslots_upper = *s->h_nslots;
+    s->nslots_pending = false;
+  }
+  (void)cudaGetLastError();
+  TimedLaunch t{};
+  bool timed = false;
+  if (s->timed_free.empty() && s->timed_busy.size() >= 256) harvest_timings(s, false);
+  if (!s->timed_free.empty()) {
+    t = s->timed_free.back();
+    s->timed_free.pop_back();
+    timed = true;
+  } else if (s->timed_busy.size() < 256) {
+    if (cudaEventCreate(&t.t0) == cudaSuccess && cudaEventCreate(&t.t1) == cudaSuccess) timed = true;
+  }
+  if (timed) cudaEventRecord(t.t0, s->q);
+  CKS(s, launch_particle_kernel(a, s->nslots_upper, s->q));
+  s->launches += 1;
+  if (timed) {
+    cudaEventRecord(t.t1, s->q);
+    s->timed_busy.push_back(t);
+  }
+  return GLISSE_OK;
+}
+
+int run_compaction(glisse_sim* s) {
+  const int w = s->w, o = w ^ 1;
+  CompactArgs c{};
+  for (int k = 0; k < 6; ++k) {
+    c.src[k] = s->work[w][k];
+    c.dst[k] = s->work[o][k];
+    c.fin[k] = s->fin[k];
+  }
+  c.src_id = s->id[w]; c.dst_id = s->id[o];
+  c.src_flag = s->flag[w]; c.src_rstep = s->rstep[w];
+  c.dst_flag = s->flag[o]; c.dst_rstep = s->rstep[o];
+  c.fin_flag = s->fin_flag; c.fin_rstep = s->fin_rstep;
+  c.n_in = s->d_nslots + w;
+  c.n_out = s->d_nslots + o;
+  c.block_counts = s->d_block_counts;
+  CKS(s, launch_compaction(c, s->nslots_upper, s->q, &s->launches));
+  s->w = o;
+  // survivor count to the host without blocking; the next launches use it once it has arrived
+  if (s->nslots_pending) {
+    // an older copy may still be in flight into the same pinned word: order behind it on stream q
+  }
+  CKS(s, cudaMemcpyAsync(s->h_nslots, s->d_nslots + o, sizeof(int), cudaMemcpyDeviceToHost, s->q));
+  CKS(s, cudaEventRecord(s->nslots_ready, s->q));
+  s->nslots_pending = true;
+  s->chunks_since_resync = 0;
+  return GLISSE_OK;
+}
+
+// planet-history kernel into buffer b, starting from the Jacobi state `jin` at step `start`
+int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
+  LogBuffer& B = s->buf[b];
+  CKS(s, cudaStreamWaitEvent(s->p, B.consumed, 0));
+  CKS(s, launch_planet_kernel(s->d_sys, jin, B.log, B.jlog, s->K, s->dt, s->p));
+  s->launches += 1;
+  CKS(s, cudaEventRecord(B.ready, s->p));
+  B.start = start;
+  return GLISSE_OK;
+}
+
+int sync_all(glisse_sim* s) {
+  CKS(s, cudaStreamSynchronize(s->q));
+  CKS(s, cudaStreamSynchronize(s->p));
+  if (s->nslots_pending) {
+    s->nslots_upper = *s->h_nslots;
+    s->nslots_pending = false;
+  }
+  harvest_timings(s, true);
+  if (s->status == GLISSE_OK) {
+    int pst = 0;
+    CKS(s, cudaMemcpy(&pst, reinterpret_cast<char*>(s->d_sys) + offsetof(PlanetSystem, status), sizeof(int),
+                      cudaMemcpyDeviceToHost));
+    if (pst != 0) s->status = GLISSE_EPLANET;
+  }
+  return s->status;
+}
+
+template <class T>
+cudaError_t dmalloc(T** p, size_t count) {
+  return cudaMalloc(reinterpret_cast<void**>(p), (count ? count : 1) * sizeof(T));
+}
+
+}  // namespace
+
+extern "C" {
+
+void glisse_default_params(glisse_params* p) {
+  if (!p) return;
+  p->r_min = 0.0;
+  p->r_max = std::numeric_limits<double>::infinity();
+  p->kepler_iters = 5;
+  p->kepler_tol = 1e-14;
+  p->chunk_steps = 1024;
+  p->resync_chunks = 1;
+  p->device = 0;
+  p->stream = nullptr;
+}
+
+int glisse_log_stride(int n_planets) {
+  return (n_planets < 0 || n_planets > kMaxPlanets) ? 0 : log_stride(n_planets);
+}
+
+const char* glisse_strerror(int status) {
+  switch (status) {
+    case GLISSE_OK: return "ok";
+    case GLISSE_EINVAL: return "invalid argument";
+    case GLISSE_ECUDA: return "CUDA failure";
+    case GLISSE_ENOMEM: return "out of memory";
+    case GLISSE_EPLANET: return "a planet's Kepler drift failed (planets must be encounter-free and bound)";
+    default: return "unknown status";
+  }
+}
+
+int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double* gm_planet, const double* planet_pos,
+                  const double* planet_vel, const double* planet_rcrit, long long n_particles,
+                  const double* const pos[3], const double* const vel[3], double dt, const glisse_params* params) {
+  if (!out) return GLISSE_EINVAL;
+  *out = nullptr;
+  if (n_planets < 0 || n_planets > kMaxPlanets || n_particles < 1 || n_particles >= (1LL << 31) || !pos || !vel)
+    return GLISSE_EINVAL;
+  if (!(gm_star > 0.0) || !std::isfinite(gm_star) || dt == 0.0 || !std::isfinite(dt)) return GLISSE_EINVAL;
+  if (n_planets > 0 && (!gm_planet || !planet_pos || !planet_vel)) return GLISSE_EINVAL;
+  for (int k = 0; k < 3; ++k)
+    if (!pos[k] || !vel[k]) return GLISSE_EINVAL;
+  if (n_planets > 0) {
+    if (!all_finite_host(gm_planet, n_planets) || !all_finite_host(planet_pos, 3LL * n_planets) ||
+        !all_finite_host(planet_vel, 3LL * n_planets))
+      return GLISSE_EINVAL;
+    for (int j = 0; j < n_planets; ++j)
+      if (!(gm_planet[j] > 0.0)) return GLISSE_EINVAL;
+    if (planet_rcrit && !all_finite_host(planet_rcrit, n_planets)) return GLISSE_EINVAL;
+  }
+  glisse_params prm;
+  glisse_default_params(&prm);
+  if (params) prm = *params;
+  if (prm.kepler_iters < 0 || !(prm.kepler_tol > 0.0) || prm.chunk_steps < 1 || prm.chunk_steps > 16384 ||
+      prm.resync_chunks < 0 || prm.device < 0 || std::isnan(prm.r_min) || std::isnan(prm.r_max))
+    return GLISSE_EINVAL;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || prm.device >= ndev) {
+    (void)cudaGetLastError();
+    return GLISSE_ECUDA;
+  }
+  CK(cudaSetDevice(prm.device));
+
+  glisse_sim* s = new (std::nothrow) glisse_sim;
+  if (!s) return GLISSE_ENOMEM;
+  s->device = prm.device;
+  s->prm = prm;
+  s->np = n_planets;
+  s->n = n_particles;
+  s->dt = dt;
+  s->gm0 = gm_star;
+  s->K = prm.chunk_steps;
+  s->stride = log_stride(n_planets);
+  const long long N = n_particles;
+  const int np = n_planets;
+
+#define CKF(call)                         \
+  do {                                    \
+    cudaError_t e2__ = (call);            \
+    if (e2__ != cudaSuccess) {            \
+      (void)cudaGetLastError();           \
+      free_sim(s);                        \
+      return (e2__ == cudaErrorMemoryAllocation) ? GLISSE_ENOMEM : GLISSE_ECUDA; \
+    }                                     \
+  } while (0)
+
+  if (prm.stream) {
+    s->q = static_cast<cudaStream_t>(prm.stream);
+  } else {
+    CKF(cudaStreamCreateWithFlags(&s->q, cudaStreamNonBlocking));
+    s->own_q = true;
+  }
+  CKF(cudaStreamCreateWithFlags(&s->p, cudaStreamNonBlocking));
+  CKF(configure_particle_kernels());
+
+  // ---- allocations ------------------------------------------------------------------------------
+  for (int b = 0; b < 2; ++b) {
+    CKF(dmalloc(&s->buf[b].log, static_cast<size_t>(s->K + 1) * s->stride));
+    CKF(dmalloc(&s->buf[b].jlog, static_cast<size_t>(s->K + 1) * 6 * np));
+    CKF(cudaEventCreateWithFlags(&s->buf[b].ready, cudaEventDisableTiming));
+    CKF(cudaEventCreateWithFlags(&s->buf[b].consumed, cudaEventDisableTiming));
+    for (int k = 0; k < 6; ++k) CKF(dmalloc(&s->work[b][k], N));
+    CKF(dmalloc(&s->id[b], N));
+    CKF(dmalloc(&s->flag[b], N));
+    CKF(dmalloc(&s->rstep[b], N));
+  }
+  for (int k = 0; k < 6; ++k) CKF(dmalloc(&s->fin[k], N));
+  CKF(dmalloc(&s->fin_flag, N));
+  CKF(dmalloc(&s->fin_rstep, N));
+  CKF(dmalloc(&s->d_nslots, 2));
+  CKF(dmalloc(&s->d_block_counts, static_cast<size_t>((N + 255) / 256 + 1)));
+  CKF(dmalloc(&s->d_counters, 2));
+  CKF(dmalloc(&s->d_sys, 1));
+  CKF(dmalloc(&s->d_j0, static_cast<size_t>(6 * np)));
+  CKF(cudaMallocHost(reinterpret_cast<void**>(&s->h_nslots), sizeof(int)));
+  CKF(cudaEventCreateWithFlags(&s->nslots_ready, cudaEventDisableTiming));
+
+  // ---- planet system ----------------------------------------------------------------------------
+  PlanetSystem hs{};
+  hs.np = np;
+  hs.gm0 = gm_star;
+  double eta = gm_star;
+  for (int j = 0; j < np; ++j) {
+    hs.gm[j] = gm_planet[j];
+    hs.eta_prev[j] = eta;
+    eta += gm_planet[j];
+    hs.eta[j] = eta;
+  }
+  hs.status = 0;
+  CKF(cudaMemcpyAsync(s->d_sys, &hs, sizeof(hs), cudaMemcpyHostToDevice, s->p));
+  if (np > 0) {
+    double *d_q = nullptr, *d_qd = nullptr;
+    CKF(dmalloc(&d_q, static_cast<size_t>(3 * np)));
+    cudaError_t e = dmalloc(&d_qd, static_cast<size_t>(3 * np));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_q, planet_pos, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_qd, planet_vel, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p);
+    if (e == cudaSuccess) e = launch_planet_init(s->d_sys, d_q, d_qd, s->d_j0, s->p);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->p);
+    cudaFree(d_q);
+    cudaFree(d_qd);
+    s->launches += 1;
+    CKF(e);
+  } else {
+    CKF(cudaStreamSynchronize(s->p));
+  }
+  // chunk 0 into buffer 0, chunk 1 into buffer 1 (one chunk ahead from the start)
+  if (fill_log_buffer(s, 0, s->d_j0, 0) != GLISSE_OK ||
+      fill_log_buffer(s, 1, s->buf[0].jlog + static_cast<size_t>(s->K) * 6 * np, s->K) != GLISSE_OK) {
+    const int st = s->status;
+    free_sim(s);
+    return st;
+  }
+
+  // ---- particle state ---------------------------------------------------------------------------
+  const bool dev_in = is_device_pointer(pos[0]);
+  for (int k = 0; k < 3; ++k) {
+    if (!dev_in) {
+      if (!all_finite_host(pos[k], N) || !all_finite_host(vel[k], N)) {
+        free_sim(s);
+        return GLISSE_EINVAL;
+      }
+    }
+    CKF(cudaMemcpyAsync(s->work[0][k], pos[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
+    CKF(cudaMemcpyAsync(s->work[0][3 + k], vel[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
+  }
+  CKF(cudaMemsetAsync(s->d_counters, 0, 2 * sizeof(unsigned long long), s->q));
+  if (dev_in) {
+    for (int k = 0; k < 6; ++k) {
+      CKF(launch_count_nonfinite(s->work[0][k], N, s->d_counters + 1, s->q));
+      s->launches += 1;
+    }
+    unsigned long long bad = 0;
+    CKF(cudaMemcpyAsync(&bad, s->d_counters + 1, sizeof(bad), cudaMemcpyDeviceToHost, s->q));
+    CKF(cudaStreamSynchronize(s->q));
+    if (bad) {
+      free_sim(s);
+      return GLISSE_EINVAL;
+    }
+  }
+  CKF(launch_init_ids(s->id[0], s->flag[0], s->rstep[0], s->fin_flag, s->fin_rstep, static_cast<int>(N), s->q));
+  s->launches += 1;
+  const int nsl[2] = {static_cast<int>(N), 0};
+  CKF(cudaMemcpyAsync(s->d_nslots, nsl, sizeof(nsl), cudaMemcpyHostToDevice, s->q));
+  s->nslots_upper = static_cast<int>(N);
+  s->w = 0;
+
+  // ---- constant part of the particle-kernel arguments --------------------------------------------
+  ParticleArgs& a = s->pa;
+  a.pstep_counter = s->d_counters;
+  a.stride = s->stride;
+  a.stage_recs = stage_records(np);
+  a.np = np;
+  a.iters = prm.kepler_iters;
+  a.hdt = 0.5 * dt;
+  a.mu = gm_star;
+  a.inv_mu = 1.0 / gm_star;
+  a.inv_mu_dt = dt / gm_star;
+  a.rmin2 = (prm.r_min > 0.0) ? prm.r_min * prm.r_min : 0.0;
+  a.rmax2 = (prm.r_max > 0.0 && std::isfinite(prm.r_max)) ? prm.r_max * prm.r_max
+                                                           : std::numeric_limits<double>::infinity();
+  a.tol = prm.kepler_tol;
+  for (int j = 0; j < kMaxPlanets; ++j) {
+    a.gm[j] = (j < np) ? gm_planet[j] : 0.0;
+    a.rc2[j] = (j < np && planet_rcrit) ? planet_rcrit[j] * planet_rcrit[j] : 0.0;
+  }
+  CKF(cudaStreamSynchronize(s->q));
+  CKF(cudaStreamSynchronize(s->p));
+#undef CKF
+  *out = s;
+  return GLISSE_OK;
+}
+
+int glisse_advance(glisse_sim* s, long long n_steps) {
+  if (!s || n_steps < 0) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (s->external_log_used) return GLISSE_EINVAL;  // the internal planet clock is stale
+  CKS(s, cudaSetDevice(s->device));
+  const int np = s->np;
+  while (n_steps > 0) {
+    long long off = s->step - s->buf[s->cur].start;
+    if (off == s->K) {
+      // this buffer is used up: hand it back to the planet stream, which refills it with the chunk
+      // after the next one while the particles work through the next one
+      const int old = s->cur;
+      CKS(s, cudaEventRecord(s->buf[old].consumed, s->q));
+      s->cur ^= 1;
+      const LogBuffer& nxt = s->buf[s->cur];
+      const int st = fill_log_buffer(s, old, nxt.jlog + static_cast<size_t>(s->K) * 6 * np, nxt.start + s->K);
+      if (st != GLISSE_OK) return st;
+      off = 0;
+    }
+    const LogBuffer& B = s->buf[s->cur];
+    CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+    const int m = static_cast<int>(std::min<long long>(n_steps, s->K - off));
+    const int st = launch_particles(s, B.log + static_cast<size_t>(off) * s->stride, m);
+    if (st != GLISSE_OK) return st;
+    s->step += m;
+    n_steps -= m;
+    if (s->prm.resync_chunks > 0 && ++s->chunks_since_resync >= s->prm.resync_chunks) {
+      const int sc = run_compaction(s);
+      if (sc != GLISSE_OK) return sc;
+    }
+  }
+  return GLISSE_OK;
+}
+
+int glisse_advance_with_log(glisse_sim* s, long long n_steps, const double* log) {
+  if (!s || n_steps < 0 || !log) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (n_steps == 0) return GLISSE_OK;
+  CKS(s, cudaSetDevice(s->device));
+  const size_t count = static_cast<size_t>(n_steps + 1) * s->stride;
+  double* d_log = nullptr;
+  CKS(s, dmalloc(&d_log, count));
+  cudaError_t e = cudaMemcpyAsync(d_log, log, count * sizeof(double), cudaMemcpyDefault, s->q);
+  int st = (e == cudaSuccess) ? GLISSE_OK : GLISSE_ECUDA;
+  long long done = 0;
+  while (st == GLISSE_OK && done < n_steps) {
+    const int m = static_cast<int>(std::min<long long>(n_steps - done, s->K));
+    st = launch_particles(s, d_log + static_cast<size_t>(done) * s->stride, m);
+    if (st != GLISSE_OK) break;
+    s->step += m;
+    done += m;
+    if (s->prm.resync_chunks > 0 && ++s->chunks_since_resync >= s->prm.resync_chunks) st = run_compaction(s);
+  }
+  cudaStreamSynchronize(s->q);
+  cudaFree(d_log);
+  s->external_log_used = true;
+  if (st != GLISSE_OK) s->status = st;
+  return st;
+}
+
+int glisse_planet_log(glisse_sim* s, long long n_steps, double* log) {
+  if (!s || n_steps < 0 || !log || n_steps > (1LL << 24)) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (s->external_log_used) return GLISSE_EINVAL;
+  CKS(s, cudaSetDevice(s->device));
+  const int np = s->np;
+  const LogBuffer& B = s->buf[s->cur];
+  const long long off = s->step - B.start;
+  double *d_log = nullptr, *d_jlog = nullptr;
+  const size_t count = static_cast<size_t>(n_steps + 1) * s->stride;
+  CKS(s, dmalloc(&d_log, count));
+  cudaError_t e = dmalloc(&d_jlog, static_cast<size_t>(n_steps + 1) * 6 * np);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s->q, B.ready, 0);
+  if (e == cudaSuccess)
+    e = launch_planet_kernel(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_log, d_jlog,
+                             static_cast<int>(n_steps), s->dt, s->q);
+  s->launches += 1;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(log, d_log, count * sizeof(double), cudaMemcpyDefault, s->q);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->q);
+  cudaFree(d_log);
+  cudaFree(d_jlog);
+  CKS(s, e);
+  return sync_all(s);
+}
+
+int glisse_read(glisse_sim* s, double* const pos[3], double* const vel[3], int* flag, long long* removal_step) {
+  if (!s) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  ScatterArgs g{};
+  const int w = s->w;
+  for (int k = 0; k < 6; ++k) {
+    g.st[k] = s->work[w][k];
+    g.fin[k] = s->fin[k];
+  }
+  g.id = s->id[w]; g.flag = s->flag[w]; g.rstep = s->rstep[w];
+  g.n_slots = s->d_nslots + w;
+  g.fin_flag = s->fin_flag; g.fin_rstep = s->fin_rstep;
+  CKS(s, launch_scatter_to_original(g, s->nslots_upper, s->q));
+  s->launches += 1;
+  const size_t N = static_cast<size_t>(s->n);
+  for (int k = 0; k < 3; ++k) {
+    if (pos && pos[k]) CKS(s, cudaMemcpyAsync(pos[k], s->fin[k], N * sizeof(double), cudaMemcpyDefault, s->q));
+    if (vel && vel[k]) CKS(s, cudaMemcpyAsync(vel[k], s->fin[3 + k], N * sizeof(double), cudaMemcpyDefault, s->q));
+  }
+  if (flag) CKS(s, cudaMemcpyAsync(flag, s->fin_flag, N * sizeof(int), cudaMemcpyDefault, s->q));
+  if (removal_step)
+    CKS(s, cudaMemcpyAsync(removal_step, s->fin_rstep, N * sizeof(long long), cudaMemcpyDefault, s->q));
+  return sync_all(s);
+}
+
+int glisse_read_planets(glisse_sim* s, double* pos, double* vel) {
+  if (!s) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (s->external_log_used) return GLISSE_EINVAL;
+  CKS(s, cudaSetDevice(s->device));
+  const int np = s->np;
+  if (np == 0 || (!pos && !vel)) return sync_all(s);
+  const LogBuffer& B = s->buf[s->cur];
+  const long long off = s->step - B.start;
+  double* d_out = nullptr;
+  CKS(s, dmalloc(&d_out, static_cast<size_t>(6 * np)));
+  cudaError_t e = cudaStreamWaitEvent(s->q, B.ready, 0);
+  if (e == cudaSuccess)
+    e = launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q);
+  s->launches += 1;
+  if (e == cudaSuccess && pos) e = cudaMemcpyAsync(pos, d_out, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q);
+  if (e == cudaSuccess && vel)
+    e = cudaMemcpyAsync(vel, d_out + 3 * np, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->q);
+  cudaFree(d_out);
+  CKS(s, e);
+  return sync_all(s);
+}
+
+long long glisse_active_count(glisse_sim* s) {
+  if (!s) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (cudaSetDevice(s->device) != cudaSuccess) return GLISSE_ECUDA;
+  unsigned long long c = 0;
+  cudaError_t e = cudaMemsetAsync(s->d_counters + 1, 0, sizeof(unsigned long long), s->q);
+  if (e == cudaSuccess) e = launch_count_active(s->flag[s->w], s->d_nslots + s->w, s->nslots_upper, s->d_counters + 1, s->q);
+  s->launches += 1;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&c, s->d_counters + 1, sizeof(c), cudaMemcpyDeviceToHost, s->q);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->q);
+  if (e != cudaSuccess) {
+    (void)cudaGetLastError();
+    s->status = GLISSE_ECUDA;
+    return GLISSE_ECUDA;
+  }
+  const int st = sync_all(s);
+  return st == GLISSE_OK ? static_cast<long long>(c) : st;
+}
+
+long long glisse_step(glisse_sim* s) { return s ? s->step : GLISSE_EINVAL; }
+
+long long glisse_particle_steps(glisse_sim* s) {
+  if (!s) return GLISSE_EINVAL;
+  const int st = sync_all(s);
+  if (st != GLISSE_OK) return st;
+  unsigned long long c = 0;
+  if (cudaMemcpy(&c, s->d_counters, sizeof(c), cudaMemcpyDeviceToHost) != cudaSuccess) {
+    (void)cudaGetLastError();
+    s->status = GLISSE_ECUDA;
+    return GLISSE_ECUDA;
+  }
+  return static_cast<long long>(c);
+}
+
+long long glisse_launch_count(glisse_sim* s) { return s ? s->launches : GLISSE_EINVAL; }
+
+int glisse_sync(glisse_sim* s) {
+  if (!s) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  return sync_all(s);
+}
+
+int glisse_particle_kernel_time(glisse_sim* s, double* ms, long long* launches) {
+  if (!s) return GLISSE_EINVAL;
+  const int st = glisse_sync(s);
+  if (ms) *ms = s->timed_ms;
+  if (launches) *launches = s->timed_launches;
+  s->timed_ms = 0.0;
+  s->timed_launches = 0;
+  return st;
+}
+
+int glisse_fp64_peak_probe(int device, void* stream, double millis, double* flops) {
+  if (!flops || device < 0) return GLISSE_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) {
+    (void)cudaGetLastError();
+    return GLISSE_ECUDA;
+  }
+  CK(cudaSetDevice(device));
+  CK(run_fp64_probe(static_cast<cudaStream_t>(stream), millis, flops));
+  return GLISSE_OK;
+}
+
+int glisse_test_primitive(int which, long long n, const double* in, double* out) {
+  if (which < 0 || which > 4 || n < 1 || !in || !out) return GLISSE_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    (void)cudaGetLastError();
+    return GLISSE_ECUDA;
+  }
+  const size_t in_per = (which == 4) ? 10 : 1, out_per = (which == 4) ? 7 : (which == 3 ? 2 : 1);
+  double *d_in = nullptr, *d_out = nullptr;
+  CK(dmalloc(&d_in, static_cast<size_t>(n) * in_per));
+  cudaError_t e = dmalloc(&d_out, static_cast<size_t>(n) * out_per);
+  if (e == cudaSuccess) e = cudaMemcpy(d_in, in, sizeof(double) * n * in_per, cudaMemcpyDefault);
+  if (e == cudaSuccess) e = run_primitive(which, n, d_in, d_out, nullptr);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) e = cudaMemcpy(out, d_out, sizeof(double) * n * out_per, cudaMemcpyDefault);
+  cudaFree(d_in);
+  cudaFree(d_out);
+  CK(e);
+  return GLISSE_OK;
+}
+
+void glisse_destroy(glisse_sim* s) { free_sim(s); }
+
+}  // extern "C"

@@ -1,0 +1,178 @@
+// compact.cu — survivor compaction ("resync", step a8 of DESIGN.md) and the small
+// bookkeeping kernels around it.
+//
+// The paper runs a stable partition that moves deactivated particles to the array tail so later
+// launches cover only active ones, keeping the relative order of the survivors.  Here: a
+// warp-ballot + prefix-sum stable partition in three small kernels (per-block count, scan of the
+// block counts, scatter).  Survivors go, in order, to the prefix of the other working buffer; a
+// removed particle's frozen state goes to its ORIGINAL index in the `fin` arrays, which is where
+// glisse_read assembles the result, so compaction is invisible to the caller (reading S16).
+#include "glisse_internal.cuh"
+
+namespace glisse {
+namespace {
+
+constexpr int kBlock = 256;
+constexpr unsigned kFull = 0xffffffffu;
+
+__global__ void __launch_bounds__(kBlock) count_block_actives(const int* __restrict__ flag,
+                                                               const int* __restrict__ n_in,
+                                                               int* __restrict__ block_counts) {
+  const int n = *n_in;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  const bool act = (i < n) && (flag[i] == 0);
+  const int c = __syncthreads_count(act);
+  if (threadIdx.x == 0) block_counts[blockIdx.x] = c;
+}
+
+// exclusive scan of block_counts[0..nb) in place (one block), total -> *n_out
+__global__ void __launch_bounds__(1024) scan_block_counts(int* __restrict__ block_counts, int nb,
+                                                           int* __restrict__ n_out) {
+  __shared__ int warp_sums[32];
+  __shared__ int carry_s;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < nb; base += 1024) {
+    const int i = base + threadIdx.x;
+    const int v = (i < nb) ? block_counts[i] : 0;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(kFull, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_sums[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+      int w = warp_sums[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(kFull, w, o);
+        if (lane >= o) w += t;
+      }
+      warp_sums[lane] = w;  // inclusive over warps
+    }
+    __syncthreads();
+    const int carry = carry_s;
+    const int warp_off = warp ? warp_sums[warp - 1] : 0;
+    if (i < nb) block_counts[i] = carry + warp_off + inc - v;
+    __syncthreads();
+    if (threadIdx.x == 0) carry_s = carry + warp_sums[31];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *n_out = carry_s;
+}
+
+__global__ void __launch_bounds__(kBlock) scatter_partition(const CompactArgs a) {
+  __shared__ int warp_counts[kBlock / 32];
+  const int n = *a.n_in;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool in = i < n;
+  const int fl = in ? a.src_flag[i] : -1;
+  const bool act = fl == 0;
+  const unsigned m = __ballot_sync(kFull, act);
+  if (lane == 0) warp_counts[warp] = __popc(m);
+  __syncthreads();
+  int off = a.block_counts[blockIdx.x];
+  for (int w = 0; w < warp; ++w) off += warp_counts[w];
+  if (!in) return;
+  const int id = a.src_id[i];
+  if (act) {
+    const int d = off + __popc(m & ((1u << lane) - 1u));
+#pragma unroll
+    for (int k = 0; k < 6; ++k) a.dst[k][d] = a.src[k][i];
+    a.dst_id[d] = id;
+    a.dst_flag[d] = 0;
+    a.dst_rstep[d] = -1;
+  } else {
+#pragma unroll
+    for (int k = 0; k < 6; ++k) a.fin[k][id] = a.src[k][i];
+    a.fin_flag[id] = fl;
+    a.fin_rstep[id] = a.src_rstep[i];
+  }
+}
+
+__global__ void __launch_bounds__(kBlock) scatter_to_original(const ScatterArgs a) {
+  const int n = *a.n_slots;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n) return;
+  const int id = a.id[i];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) a.fin[k][id] = a.st[k][i];
+  a.fin_flag[id] = a.flag[i];
+  a.fin_rstep[id] = a.rstep[i];
+}
+
+__global__ void __launch_bounds__(kBlock) count_active_kernel(const int* __restrict__ flag,
+                                                               const int* __restrict__ n_slots,
+                                                               unsigned long long* __restrict__ out) {
+  const int n = *n_slots;
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  const bool act = (i < n) && (flag[i] == 0);
+  const int c = __syncthreads_count(act);
+  if (threadIdx.x == 0 && c) atomicAdd(out, static_cast<unsigned long long>(c));
+}
+
+__global__ void __launch_bounds__(kBlock) init_ids_kernel(int* id, int* flag, long long* rstep, int* fin_flag,
+                                                           long long* fin_rstep, int n) {
+  const int i = blockIdx.x * kBlock + threadIdx.x;
+  if (i >= n) return;
+  id[i] = i;
+  flag[i] = 0;
+  rstep[i] = -1;
+  fin_flag[i] = 0;
+  fin_rstep[i] = -1;
+}
+
+__global__ void __launch_bounds__(kBlock) count_nonfinite_kernel(const double* __restrict__ p, long long n,
+                                                                  unsigned long long* __restrict__ out) {
+  long long bad = 0;
+  for (long long i = static_cast<long long>(blockIdx.x) * kBlock + threadIdx.x; i < n;
+       i += static_cast<long long>(gridDim.x) * kBlock)
+    bad += !isfinite(p[i]);
+  const int c = __syncthreads_count(bad != 0);
+  if (threadIdx.x == 0 && c) atomicAdd(out, static_cast<unsigned long long>(c));
+}
+
+}  // namespace
+
+cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStream_t s, long long* launches) {
+  if (n_slots_upper < 1) n_slots_upper = 1;
+  const int nb = (n_slots_upper + kBlock - 1) / kBlock;
+  count_block_actives<<<nb, kBlock, 0, s>>>(a.src_flag, a.n_in, a.block_counts);
+  scan_block_counts<<<1, 1024, 0, s>>>(a.block_counts, nb, a.n_out);
+  scatter_partition<<<nb, kBlock, 0, s>>>(a);
+  if (launches) *launches += 3;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_to_original(const ScatterArgs& a, int n_slots_upper, cudaStream_t s) {
+  if (n_slots_upper < 1) n_slots_upper = 1;
+  scatter_to_original<<<(n_slots_upper + kBlock - 1) / kBlock, kBlock, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_count_active(const int* flag, const int* n_slots, int n_slots_upper, unsigned long long* out,
+                                cudaStream_t s) {
+  if (n_slots_upper < 1) n_slots_upper = 1;
+  count_active_kernel<<<(n_slots_upper + kBlock - 1) / kBlock, kBlock, 0, s>>>(flag, n_slots, out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_init_ids(int* id, int* flag, long long* rstep, int* fin_flag, long long* fin_rstep, int n,
+                            cudaStream_t s) {
+  init_ids_kernel<<<(n + kBlock - 1) / kBlock, kBlock, 0, s>>>(id, flag, rstep, fin_flag, fin_rstep, n);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_count_nonfinite(const double* p, long long n, unsigned long long* out, cudaStream_t s) {
+  long long nb = (n + kBlock - 1) / kBlock;
+  if (nb > 148 * 16) nb = 148 * 16;
+  if (nb < 1) nb = 1;
+  count_nonfinite_kernel<<<static_cast<int>(nb), kBlock, 0, s>>>(p, n, out);
+  return cudaGetLastError();
+}
+
+}  // namespace glisse

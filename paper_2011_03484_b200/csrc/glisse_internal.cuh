@@ -10,16 +10,17 @@ namespace glisse {
 
 constexpr int kMaxPlanets = GLISSE_MAX_PLANETS;
 constexpr int kParticleBlock = 128;  // threads per particle-kernel block (one particle per thread)
-constexpr int kRingStages = 3;       // planet-log ring buffers in shared memory per block
+constexpr int kParticleWarps = kParticleBlock / 32;
+constexpr int kRingSlots = 2;        // planet-log stages resident in shared memory per WARP
 
 // Doubles per planet-log record (include/glisse.h: glisse_log_stride).
 __host__ __device__ inline int log_stride(int np) { return (3 * (np + 1) + 1) & ~1; }
 
-// Records per shared-memory ring stage: about 4 KB per stage.
+// Records per shared-memory ring stage (one cp.async.bulk each): about 1 KB per stage.
 inline int stage_records(int np) {
-  int s = 4096 / (log_stride(np) * 8);
-  if (s > 32) s = 32;
-  if (s < 4) s = 4;
+  int s = 1024 / (log_stride(np) * 8);
+  if (s > 16) s = 16;
+  if (s < 2) s = 2;
   return s;
 }
 
@@ -29,7 +30,7 @@ struct ParticleArgs {
   int* flag;                           // 0 = active
   long long* rstep;                    // removal step
   const int* n_slots;                  // device: length of the working prefix in use
-  const double* log;                   // (nsteps + 1) records of `stride` doubles
+  const double* log;                   // (nsteps + 1) records of `stride` doubles, 16-byte aligned
   unsigned long long* pstep_counter;   // device: += number of drifts started
   long long step0;                     // completed steps at record 0
   int nsteps;
@@ -37,53 +38,68 @@ struct ParticleArgs {
   int stage_recs;
   int np;
   int iters;
-  double dt, hdt, mu, inv_mu, rmin2, rmax2, tol;
+  double hdt, mu, inv_mu, inv_mu_dt, rmin2, rmax2, tol;
   double gm[kMaxPlanets];
   double rc2[kMaxPlanets];
 };
 
-// ---- planet system constants + state, resident in device memory --------------------------------
+// ---- planet system constants, resident in device memory -----------------------------------------
 struct PlanetSystem {
   int np;
   double gm0;
   double gm[kMaxPlanets];
   double eta[kMaxPlanets];       // eta_k = gm0 + sum_{i<=k} gm_i
   double eta_prev[kMaxPlanets];  // eta_{k-1}
-  double rj[3 * kMaxPlanets];    // Jacobi positions   (persisted between chunks)
-  double vj[3 * kMaxPlanets];    // Jacobi velocities
   int status;                    // 0, or 1-based index of the first planet whose drift failed
 };
 
-// launchers (each returns the cudaError_t of the launch)
+// Jacobi state record: [r'_0 .. r'_{Np-1} | v'_0 .. v'_{Np-1}], 6·Np doubles.
+inline int jstate_stride(int np) { return 6 * np; }
+
+// launchers (each returns the cudaError_t of the launch); *launches += kernels launched
 cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_slots_upper, cudaStream_t s);
-cudaError_t launch_planet_kernel(PlanetSystem* sys, double* log, int nsteps, double dt, bool save_state,
-                                 cudaStream_t s);
-cudaError_t launch_planet_init(PlanetSystem* sys, const double* q, const double* qd, cudaStream_t s);
-cudaError_t launch_planet_read(const PlanetSystem* sys, double* q, double* qd, cudaStream_t s);
+cudaError_t configure_particle_kernels();
+
+// Planet-history kernel (a1): from the Jacobi state `jin` write nsteps+1 log records and nsteps+1
+// Jacobi state records (record 0 = the input state).
+cudaError_t launch_planet_kernel(PlanetSystem* sys, const double* jin, double* log, double* jlog, int nsteps,
+                                 double dt, cudaStream_t s);
+// heliocentric (q, qd) [np][3] -> Jacobi state record
+cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const double* qd, double* jstate,
+                               cudaStream_t s);
+// Jacobi state record -> heliocentric q, qd [np][3] (either may be null)
+cudaError_t launch_planet_read(const PlanetSystem* sys, const double* jstate, double* q, double* qd,
+                               cudaStream_t s);
 
 struct CompactArgs {
-  double* src[6];
+  const double* src[6];
   double* dst[6];
   double* fin[6];          // original order: frozen state of compacted-away particles
-  int* src_id;  int* dst_id;
-  int* src_flag; long long* src_rstep;
+  const int* src_id;  int* dst_id;
+  const int* src_flag; const long long* src_rstep;
+  int* dst_flag; long long* dst_rstep;
   int* fin_flag; long long* fin_rstep;
-  int* n_slots;            // in: prefix length; out: number of survivors
-  int* block_counts;       // scratch [ceil(n/256)]
+  const int* n_in;         // prefix length of src
+  int* n_out;              // number of survivors = prefix length of dst
+  int* block_counts;       // scratch [ceil(n_upper/256) + 1]
 };
-cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStream_t s, int* launches);
+cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStream_t s, long long* launches);
 
-struct GatherArgs {
+struct ScatterArgs {
   const double* st[6];
   const int* id; const int* flag; const long long* rstep;
   const int* n_slots;
-  double* out[6];          // original order, may be null individually
-  int* out_flag; long long* out_rstep;
+  double* fin[6];          // original order
+  int* fin_flag; long long* fin_rstep;
 };
-cudaError_t launch_scatter_to_original(const GatherArgs& a, int n_slots_upper, cudaStream_t s);
-cudaError_t launch_count_active(const int* flag, const int* n_slots, int n_slots_upper, int* out, cudaStream_t s);
-cudaError_t launch_init_ids(int* id, int* flag, long long* rstep, int n, cudaStream_t s);
+cudaError_t launch_scatter_to_original(const ScatterArgs& a, int n_slots_upper, cudaStream_t s);
+cudaError_t launch_count_active(const int* flag, const int* n_slots, int n_slots_upper,
+                                unsigned long long* out, cudaStream_t s);
+cudaError_t launch_init_ids(int* id, int* flag, long long* rstep, int* fin_flag, long long* fin_rstep, int n,
+                            cudaStream_t s);
+cudaError_t launch_count_nonfinite(const double* p, long long n, unsigned long long* out, cudaStream_t s);
 
 cudaError_t run_fp64_probe(cudaStream_t s, double millis, double* flops);
+cudaError_t run_primitive(int which, long long n, const double* in, double* out, cudaStream_t s);
 
 }  // namespace glisse

@@ -1,0 +1,219 @@
+// planets.cu — the planet-history kernel (step a1 of DESIGN.md; "standard
+// Wisdom-Holman" for the mutually interacting planets, PAPER.md:109-115 planet log and h0).
+//
+// The paper integrates the planets on the CPU and ships each chunk over PCIe; here
+// one warp advances them on the device, lane k = planet k in Jacobi order, and writes the chunk of
+// K+1 log records straight to HBM, one chunk ahead of the particle kernel on its own stream.
+// The step is serial in time, so what matters is latency: all sums over planets run through
+// register shuffles, in the index order of the definition (O3).
+//
+//   eta_k = gm0 + sum_{i<=k} gm_i ;  Jacobi r'_k = q_k − (sum_{i<k} gm_i q_i)/eta_{k-1}
+//   q_k = r'_k + sum_{i<k} (gm_i/eta_i) r'_i
+//   kick:  v'_k += h (eta_k/eta_{k-1}) [ gm0 r'_k/|r'_k|^3 + A_k + (1/eta_k) sum_{i>k} gm_i A_i ]
+//          A_i = − gm0 q_i/|q_i|^3 − sum_{j != i} gm_j (q_i − q_j)/|q_i − q_j|^3
+//   drift: two-body motion of (r'_k, v'_k) about mu_k = gm0 eta_k/eta_{k-1}
+#include "glisse_internal.cuh"
+#include "kepler.cuh"
+
+namespace glisse {
+namespace {
+
+constexpr int kPlanetKeplerIters = 10;
+constexpr double kPlanetKeplerTol = 1e-13;
+
+struct Lane {
+  int np, lane;
+  bool live;
+  double gm0, gm, eta, eta_prev, wj;  // wj = gm/eta
+  double mu, inv_mu;
+};
+
+__device__ __forceinline__ double shfl(double v, int src) { return __shfl_sync(kFullMask, v, src); }
+
+// exclusive prefix sum over lanes i < lane of c_i, added in increasing i
+__device__ __forceinline__ void prefix3(const Lane& L, double cx, double cy, double cz, double& sx, double& sy,
+                                        double& sz) {
+  sx = sy = sz = 0.0;
+  for (int i = 0; i + 1 < L.np; ++i) {
+    const double tx = shfl(cx, i), ty = shfl(cy, i), tz = shfl(cz, i);
+    if (i < L.lane) { sx += tx; sy += ty; sz += tz; }
+  }
+}
+
+// q from r' (Jacobi -> heliocentric); the same linear map serves velocities
+__device__ __forceinline__ void jacobi_to_helio(const Lane& L, double rx, double ry, double rz, double& qx,
+                                                double& qy, double& qz) {
+  double sx, sy, sz;
+  prefix3(L, L.wj * rx, L.wj * ry, L.wj * rz, sx, sy, sz);
+  qx = rx + sx; qy = ry + sy; qz = rz + sz;
+}
+
+// r' from q (heliocentric -> Jacobi)
+__device__ __forceinline__ void helio_to_jacobi(const Lane& L, double qx, double qy, double qz, double& rx,
+                                                double& ry, double& rz) {
+  double sx, sy, sz;
+  prefix3(L, L.gm * qx, L.gm * qy, L.gm * qz, sx, sy, sz);
+  const double ie = 1.0 / L.eta_prev;
+  rx = qx - sx * ie; ry = qy - sy * ie; rz = qz - sz * ie;
+}
+
+// Jacobi acceleration of this lane's planet, and h0 (the same on every lane)
+__device__ __forceinline__ void kick_accel(const Lane& L, double qx, double qy, double qz, double rx, double ry,
+                                           double rz, double& ax, double& ay, double& az, double& hx, double& hy,
+                                           double& hz) {
+  // star term of A_i and this planet's contribution to h0
+  const double q2 = fma(qx, qx, fma(qy, qy, qz * qz));
+  const double qi = rsqrt_f64(q2);
+  const double qi3 = qi * qi * qi;
+  double Ax = -(L.gm0 * qi3) * qx, Ay = -(L.gm0 * qi3) * qy, Az = -(L.gm0 * qi3) * qz;
+  const double tx = (L.gm * qi3) * qx, ty = (L.gm * qi3) * qy, tz = (L.gm * qi3) * qz;
+  hx = hy = hz = 0.0;
+  for (int j = 0; j < L.np; ++j) {
+    const double gj = shfl(L.gm, j);
+    const double qjx = shfl(qx, j), qjy = shfl(qy, j), qjz = shfl(qz, j);
+    hx -= shfl(tx, j); hy -= shfl(ty, j); hz -= shfl(tz, j);
+    const bool self = (j == L.lane);
+    const double dx = qx - qjx, dy = qy - qjy, dz = qz - qjz;
+    const double d2 = self ? 1.0 : fma(dx, dx, fma(dy, dy, dz * dz));
+    const double di = rsqrt_f64(d2);
+    const double w = self ? 0.0 : (gj * di) * (di * di);
+    Ax = fma(-w, dx, Ax); Ay = fma(-w, dy, Ay); Az = fma(-w, dz, Az);
+  }
+  // tail_k = sum_{i>k} gm_i A_i, added in increasing i
+  const double mx = L.gm * Ax, my = L.gm * Ay, mz = L.gm * Az;
+  double Tx = 0.0, Ty = 0.0, Tz = 0.0;
+  for (int i = 1; i < L.np; ++i) {
+    const double ux = shfl(mx, i), uy = shfl(my, i), uz = shfl(mz, i);
+    if (i > L.lane) { Tx += ux; Ty += uy; Tz += uz; }
+  }
+  const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
+  const double ri = rsqrt_f64(r2);
+  const double w0 = L.gm0 * (ri * ri * ri);
+  const double ie = 1.0 / L.eta;
+  const double sc = L.eta / L.eta_prev;
+  ax = sc * (fma(w0, rx, Ax) + Tx * ie);
+  ay = sc * (fma(w0, ry, Ay) + Ty * ie);
+  az = sc * (fma(w0, rz, Az) + Tz * ie);
+}
+
+__device__ __forceinline__ Lane make_lane(const PlanetSystem* sys) {
+  Lane L;
+  L.np = sys->np;
+  L.lane = threadIdx.x & 31;
+  L.live = L.lane < L.np;
+  L.gm0 = sys->gm0;
+  L.gm = L.live ? sys->gm[L.lane] : 0.0;
+  L.eta = L.live ? sys->eta[L.lane] : 1.0;
+  L.eta_prev = L.live ? sys->eta_prev[L.lane] : 1.0;
+  L.wj = L.gm / L.eta;
+  L.mu = L.gm0 * L.eta / L.eta_prev;
+  L.inv_mu = 1.0 / L.mu;
+  return L;
+}
+
+__device__ __forceinline__ void write_record(const Lane& L, double* log, double* jlog, int rec, int stride,
+                                             double qx, double qy, double qz, double hx, double hy, double hz,
+                                             double rx, double ry, double rz, double vx, double vy, double vz) {
+  double* r = log + static_cast<size_t>(rec) * stride;
+  if (L.live) {
+    r[3 * L.lane] = qx; r[3 * L.lane + 1] = qy; r[3 * L.lane + 2] = qz;
+    double* js = jlog + static_cast<size_t>(rec) * 6 * L.np;
+    js[3 * L.lane] = rx; js[3 * L.lane + 1] = ry; js[3 * L.lane + 2] = rz;
+    js[3 * L.np + 3 * L.lane] = vx; js[3 * L.np + 3 * L.lane + 1] = vy; js[3 * L.np + 3 * L.lane + 2] = vz;
+  }
+  if (L.lane == 0) {
+    r[3 * L.np] = hx; r[3 * L.np + 1] = hy; r[3 * L.np + 2] = hz;
+    for (int c = 3 * L.np + 3; c < stride; ++c) r[c] = 0.0;
+  }
+}
+
+__global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, const double* __restrict__ jin,
+                                                             double* __restrict__ log, double* __restrict__ jlog,
+                                                             int nsteps, double dt) {
+  const Lane L = make_lane(sys);
+  const int stride = log_stride(L.np);
+  const double hdt = 0.5 * dt;
+  const double inv_mu_dt = L.inv_mu * dt;
+  // dead lanes carry a harmless circular-orbit state
+  double rx = 1.0 + L.lane, ry = 0.0, rz = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+  if (L.live) {
+    rx = jin[3 * L.lane]; ry = jin[3 * L.lane + 1]; rz = jin[3 * L.lane + 2];
+    vx = jin[3 * L.np + 3 * L.lane]; vy = jin[3 * L.np + 3 * L.lane + 1]; vz = jin[3 * L.np + 3 * L.lane + 2];
+  }
+  double qx, qy, qz, ax, ay, az, hx, hy, hz;
+  jacobi_to_helio(L, rx, ry, rz, qx, qy, qz);
+  kick_accel(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
+  write_record(L, log, jlog, 0, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
+  int bad = 0;
+  for (int s = 0; s < nsteps; ++s) {
+    if (L.live) { vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz); }
+    const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
+    const int st = kepler_drift_warp(L.live, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2,
+                                     rx, ry, rz, vx, vy, vz);
+    const unsigned failed = __ballot_sync(kFullMask, st != 0);
+    if (failed && !bad) bad = __ffs(failed);
+    jacobi_to_helio(L, rx, ry, rz, qx, qy, qz);
+    kick_accel(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
+    if (L.live) { vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz); }
+    write_record(L, log, jlog, s + 1, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
+  }
+  if (bad && L.lane == 0 && sys->status == 0) sys->status = bad;
+}
+
+__global__ void __launch_bounds__(32) planet_init_kernel(const PlanetSystem* sys, const double* q, const double* qd,
+                                                          double* jstate) {
+  const Lane L = make_lane(sys);
+  double qx = 0, qy = 0, qz = 0, wx = 0, wy = 0, wz = 0;
+  if (L.live) {
+    qx = q[3 * L.lane]; qy = q[3 * L.lane + 1]; qz = q[3 * L.lane + 2];
+    wx = qd[3 * L.lane]; wy = qd[3 * L.lane + 1]; wz = qd[3 * L.lane + 2];
+  }
+  double rx, ry, rz, vx, vy, vz;
+  helio_to_jacobi(L, qx, qy, qz, rx, ry, rz);
+  helio_to_jacobi(L, wx, wy, wz, vx, vy, vz);
+  if (L.live) {
+    jstate[3 * L.lane] = rx; jstate[3 * L.lane + 1] = ry; jstate[3 * L.lane + 2] = rz;
+    jstate[3 * L.np + 3 * L.lane] = vx; jstate[3 * L.np + 3 * L.lane + 1] = vy;
+    jstate[3 * L.np + 3 * L.lane + 2] = vz;
+  }
+}
+
+__global__ void __launch_bounds__(32) planet_read_kernel(const PlanetSystem* sys, const double* jstate, double* q,
+                                                          double* qd) {
+  const Lane L = make_lane(sys);
+  double rx = 0, ry = 0, rz = 0, vx = 0, vy = 0, vz = 0;
+  if (L.live) {
+    rx = jstate[3 * L.lane]; ry = jstate[3 * L.lane + 1]; rz = jstate[3 * L.lane + 2];
+    vx = jstate[3 * L.np + 3 * L.lane]; vy = jstate[3 * L.np + 3 * L.lane + 1];
+    vz = jstate[3 * L.np + 3 * L.lane + 2];
+  }
+  double qx, qy, qz, wx, wy, wz;
+  jacobi_to_helio(L, rx, ry, rz, qx, qy, qz);
+  jacobi_to_helio(L, vx, vy, vz, wx, wy, wz);
+  if (L.live) {
+    if (q) { q[3 * L.lane] = qx; q[3 * L.lane + 1] = qy; q[3 * L.lane + 2] = qz; }
+    if (qd) { qd[3 * L.lane] = wx; qd[3 * L.lane + 1] = wy; qd[3 * L.lane + 2] = wz; }
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_planet_kernel(PlanetSystem* sys, const double* jin, double* log, double* jlog, int nsteps,
+                                 double dt, cudaStream_t s) {
+  planet_history_kernel<<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const double* qd, double* jstate,
+                               cudaStream_t s) {
+  planet_init_kernel<<<1, 32, 0, s>>>(sys, q, qd, jstate);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_planet_read(const PlanetSystem* sys, const double* jstate, double* q, double* qd,
+                               cudaStream_t s) {
+  planet_read_kernel<<<1, 32, 0, s>>>(sys, jstate, q, qd);
+  return cudaGetLastError();
+}
+
+}  // namespace glisse

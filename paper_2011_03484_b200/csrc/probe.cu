@@ -1,0 +1,124 @@
+// probe.cu — (i) the FP64-FMA peak probe that gives the roofline denominator of this ALU-bound path
+// (MEASURED_PEAKS.json has no FP64 figure) and (ii) a test hook that evaluates the
+// device primitives of kepler.cuh on arrays, so the tests can check them one by one.
+#include "glisse_internal.cuh"
+#include "kepler.cuh"
+
+namespace glisse {
+namespace {
+
+constexpr int kProbeBlock = 256;
+constexpr int kChains = 8;
+
+// Register-resident DFMA chains: kChains independent accumulators per thread, no memory traffic.
+__global__ void __launch_bounds__(kProbeBlock) dfma_probe_kernel(double* sink, long long iters, double a, double b) {
+  double acc[kChains];
+#pragma unroll
+  for (int c = 0; c < kChains; ++c) acc[c] = 1.0 + 1e-3 * (threadIdx.x + c);
+  for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int c = 0; c < kChains; ++c) acc[c] = fma(acc[c], a, b);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int c = 0; c < kChains; ++c) s += acc[c];
+  if (s == 123.456) sink[0] = s;  // never true; keeps the chains alive
+}
+
+__global__ void primitive_kernel(int which, long long n, const double* __restrict__ in, double* __restrict__ out) {
+  const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  const bool live = i < n;
+  const long long ii = live ? i : 0;
+  switch (which) {
+    case 0: {  // rsqrt_f64
+      const double v = rsqrt_f64(in[ii]);
+      if (live) out[i] = v;
+      break;
+    }
+    case 1: {  // rcp_f64
+      const double v = rcp_f64(in[ii]);
+      if (live) out[i] = v;
+      break;
+    }
+    case 2: {  // rcp_f64_1
+      const double v = rcp_f64_1(in[ii]);
+      if (live) out[i] = v;
+      break;
+    }
+    case 3: {  // sincosm_warp: out[2i] = sin x − x, out[2i+1] = cos x − 1
+      double sm, cm;
+      sincosm_warp(live, in[ii], sm, cm);
+      if (live) { out[2 * i] = sm; out[2 * i + 1] = cm; }
+      break;
+    }
+    case 4: {  // kepler drift: in = [mu, dt, iters, tol, x,y,z,vx,vy,vz] per body; out = [flag, x..vz]
+      const double* p = in + 10 * ii;
+      const double mu = p[0], dt = p[1];
+      double x = p[4], y = p[5], z = p[6], vx = p[7], vy = p[8], vz = p[9];
+      const double r2 = fma(x, x, fma(y, y, z * z));
+      const int st = kepler_drift_warp(live, mu, 1.0 / mu, dt / mu, static_cast<int>(p[2]), p[3], r2, x, y, z, vx,
+                                       vy, vz);
+      if (live) {
+        double* o = out + 7 * i;
+        o[0] = st; o[1] = x; o[2] = y; o[3] = z; o[4] = vx; o[5] = vy; o[6] = vz;
+      }
+      break;
+    }
+    default:
+      break;
+  }
+}
+
+}  // namespace
+
+cudaError_t run_fp64_probe(cudaStream_t s, double millis, double* flops) {
+  cudaError_t e;
+  int dev = 0, sms = 0;
+  if ((e = cudaGetDevice(&dev))) return e;
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev))) return e;
+  double* sink = nullptr;
+  if ((e = cudaMalloc(&sink, 8))) return e;
+  cudaEvent_t t0, t1;
+  cudaEventCreate(&t0);
+  cudaEventCreate(&t1);
+  const int blocks = sms * 8;  // 2048 threads per SM: every FP64 lane has eight warps to draw from
+  auto run = [&](long long iters, float* ms) -> cudaError_t {
+    cudaEventRecord(t0, s);
+    dfma_probe_kernel<<<blocks, kProbeBlock, 0, s>>>(sink, iters, 0.999999, 1e-6);
+    cudaEventRecord(t1, s);
+    cudaError_t er = cudaEventSynchronize(t1);
+    if (er) return er;
+    return cudaEventElapsedTime(ms, t0, t1);
+  };
+  float ms = 0.f;
+  long long iters = 2000;
+  e = run(iters, &ms);  // warm-up and calibration
+  if (!e) e = run(iters, &ms);
+  if (!e) {
+    if (millis < 1.0) millis = 1.0;
+    const double scale = millis / (ms > 1e-3f ? ms : 1e-3f);
+    long long it2 = static_cast<long long>(iters * scale);
+    if (it2 < 100) it2 = 100;
+    e = run(it2, &ms);
+    if (!e) {
+      const double fl = 2.0 * 8.0 * kChains * static_cast<double>(it2) * blocks * kProbeBlock;
+      *flops = fl / (ms * 1e-3);
+    }
+  }
+  cudaEventDestroy(t0);
+  cudaEventDestroy(t1);
+  cudaFree(sink);
+  return e;
+}
+
+cudaError_t run_primitive(int which, long long n, const double* in, double* out, cudaStream_t s) {
+  const int block = 128;
+  const long long nb = (n + block - 1) / block;
+  primitive_kernel<<<static_cast<int>(nb < 1 ? 1 : nb), block, 0, s>>>(which, n, in, out);
+  return cudaGetLastError();
+}
+
+}  // namespace glisse
