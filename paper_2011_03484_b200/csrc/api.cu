@@ -46,6 +46,7 @@ struct glisse_sim {
 
   PlanetSystem* d_sys = nullptr;
   double* d_j0 = nullptr;  // Jacobi state at create
+  double* d_ptmp = nullptr;  // [6 Np] scratch: heliocentric planet state in / out
   LogBuffer buf[2];
   int cur = 0;
   long long step = 0;
@@ -71,6 +72,7 @@ struct glisse_sim {
   unsigned long long* d_counters = nullptr;  // [0] particle-steps, [1] scratch for counts
   long long launches = 0;
 
+  void* arena = nullptr;  // one device allocation behind every pointer above
   ParticleArgs pa{};
   std::vector<TimedLaunch> timed_free, timed_busy;
   double timed_ms = 0.0;
@@ -120,23 +122,10 @@ void free_sim(glisse_sim* s) {
   if (s->q) cudaStreamSynchronize(s->q);
   if (s->p) cudaStreamSynchronize(s->p);
   for (int b = 0; b < 2; ++b) {
-    cudaFree(s->buf[b].log);
-    cudaFree(s->buf[b].jlog);
     if (s->buf[b].ready) cudaEventDestroy(s->buf[b].ready);
     if (s->buf[b].consumed) cudaEventDestroy(s->buf[b].consumed);
-    for (int k = 0; k < 6; ++k) cudaFree(s->work[b][k]);
-    cudaFree(s->id[b]);
-    cudaFree(s->flag[b]);
-    cudaFree(s->rstep[b]);
   }
-  for (int k = 0; k < 6; ++k) cudaFree(s->fin[k]);
-  cudaFree(s->fin_flag);
-  cudaFree(s->fin_rstep);
-  cudaFree(s->d_nslots);
-  cudaFree(s->d_block_counts);
-  cudaFree(s->d_counters);
-  cudaFree(s->d_sys);
-  cudaFree(s->d_j0);
+  cudaFree(s->arena);
   if (s->h_nslots) cudaFreeHost(s->h_nslots);
   if (s->nslots_ready) cudaEventDestroy(s->nslots_ready);
   for (auto& t : s->timed_free) { cudaEventDestroy(t.t0); cudaEventDestroy(t.t1); }
@@ -361,25 +350,43 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   CKF(cudaStreamCreateWithFlags(&s->p, cudaStreamNonBlocking));
   CKF(configure_particle_kernels());
 
-  // ---- allocations ------------------------------------------------------------------------------
+  // ---- allocations: one device arena, carved at 256-byte boundaries ------------------------------
+  {
+    struct Req { void** p; size_t bytes; };
+    std::vector<Req> reqs;
+    auto need = [&](auto** p, size_t count) {
+      reqs.push_back({reinterpret_cast<void**>(p), (count ? count : 1) * sizeof(**p)});
+    };
+    for (int b = 0; b < 2; ++b) {
+      need(&s->buf[b].log, static_cast<size_t>(s->K + 1) * s->stride);
+      need(&s->buf[b].jlog, static_cast<size_t>(s->K + 1) * 6 * np);
+      for (int k = 0; k < 6; ++k) need(&s->work[b][k], N);
+      need(&s->id[b], N);
+      need(&s->flag[b], N);
+      need(&s->rstep[b], N);
+    }
+    for (int k = 0; k < 6; ++k) need(&s->fin[k], N);
+    need(&s->fin_flag, N);
+    need(&s->fin_rstep, N);
+    need(&s->d_nslots, 2);
+    need(&s->d_block_counts, static_cast<size_t>((N + 255) / 256 + 1));
+    need(&s->d_counters, 2);
+    need(&s->d_sys, 1);
+    need(&s->d_j0, static_cast<size_t>(6 * np));
+    need(&s->d_ptmp, static_cast<size_t>(6 * np));
+    size_t total = 0;
+    for (auto& r : reqs) total += (r.bytes + 255) & ~static_cast<size_t>(255);
+    CKF(cudaMalloc(&s->arena, total));
+    size_t off = 0;
+    for (auto& r : reqs) {
+      *r.p = static_cast<char*>(s->arena) + off;
+      off += (r.bytes + 255) & ~static_cast<size_t>(255);
+    }
+  }
   for (int b = 0; b < 2; ++b) {
-    CKF(dmalloc(&s->buf[b].log, static_cast<size_t>(s->K + 1) * s->stride));
-    CKF(dmalloc(&s->buf[b].jlog, static_cast<size_t>(s->K + 1) * 6 * np));
     CKF(cudaEventCreateWithFlags(&s->buf[b].ready, cudaEventDisableTiming));
     CKF(cudaEventCreateWithFlags(&s->buf[b].consumed, cudaEventDisableTiming));
-    for (int k = 0; k < 6; ++k) CKF(dmalloc(&s->work[b][k], N));
-    CKF(dmalloc(&s->id[b], N));
-    CKF(dmalloc(&s->flag[b], N));
-    CKF(dmalloc(&s->rstep[b], N));
   }
-  for (int k = 0; k < 6; ++k) CKF(dmalloc(&s->fin[k], N));
-  CKF(dmalloc(&s->fin_flag, N));
-  CKF(dmalloc(&s->fin_rstep, N));
-  CKF(dmalloc(&s->d_nslots, 2));
-  CKF(dmalloc(&s->d_block_counts, static_cast<size_t>((N + 255) / 256 + 1)));
-  CKF(dmalloc(&s->d_counters, 2));
-  CKF(dmalloc(&s->d_sys, 1));
-  CKF(dmalloc(&s->d_j0, static_cast<size_t>(6 * np)));
   CKF(cudaMallocHost(reinterpret_cast<void**>(&s->h_nslots), sizeof(int)));
   CKF(cudaEventCreateWithFlags(&s->nslots_ready, cudaEventDisableTiming));
 
@@ -397,20 +404,14 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   hs.status = 0;
   CKF(cudaMemcpyAsync(s->d_sys, &hs, sizeof(hs), cudaMemcpyHostToDevice, s->p));
   if (np > 0) {
-    double *d_q = nullptr, *d_qd = nullptr;
-    CKF(dmalloc(&d_q, static_cast<size_t>(3 * np)));
-    cudaError_t e = dmalloc(&d_qd, static_cast<size_t>(3 * np));
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_q, planet_pos, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_qd, planet_vel, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p);
-    if (e == cudaSuccess) e = launch_planet_init(s->d_sys, d_q, d_qd, s->d_j0, s->p);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s->p);
-    cudaFree(d_q);
-    cudaFree(d_qd);
+    double* d_q = s->d_ptmp;
+    double* d_qd = s->d_ptmp + 3 * np;
+    CKF(cudaMemcpyAsync(d_q, planet_pos, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p));
+    CKF(cudaMemcpyAsync(d_qd, planet_vel, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p));
+    CKF(launch_planet_init(s->d_sys, d_q, d_qd, s->d_j0, s->p));
     s->launches += 1;
-    CKF(e);
-  } else {
-    CKF(cudaStreamSynchronize(s->p));
   }
+  CKF(cudaStreamSynchronize(s->p));  // the caller's planet arrays and `hs` are consumed
   // chunk 0 into buffer 0, chunk 1 into buffer 1 (one chunk ahead from the start)
   if (fill_log_buffer(s, 0, s->d_j0, 0) != GLISSE_OK ||
       fill_log_buffer(s, 1, s->buf[0].jlog + static_cast<size_t>(s->K) * 6 * np, s->K) != GLISSE_OK) {
@@ -471,8 +472,9 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     a.gm[j] = (j < np) ? gm_planet[j] : 0.0;
     a.rc2[j] = (j < np && planet_rcrit) ? planet_rcrit[j] * planet_rcrit[j] : 0.0;
   }
+  // the caller's buffers are free again once the copies on q are done; the planet stream keeps
+  // running (a planet failure is reported by the next synchronising call)
   CKF(cudaStreamSynchronize(s->q));
-  CKF(cudaStreamSynchronize(s->p));
 #undef CKF
   *out = s;
   return GLISSE_OK;
@@ -598,18 +600,12 @@ int glisse_read_planets(glisse_sim* s, double* pos, double* vel) {
   if (np == 0 || (!pos && !vel)) return sync_all(s);
   const LogBuffer& B = s->buf[s->cur];
   const long long off = s->step - B.start;
-  double* d_out = nullptr;
-  CKS(s, dmalloc(&d_out, static_cast<size_t>(6 * np)));
-  cudaError_t e = cudaStreamWaitEvent(s->q, B.ready, 0);
-  if (e == cudaSuccess)
-    e = launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q);
+  double* d_out = s->d_ptmp;
+  CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+  CKS(s, launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q));
   s->launches += 1;
-  if (e == cudaSuccess && pos) e = cudaMemcpyAsync(pos, d_out, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q);
-  if (e == cudaSuccess && vel)
-    e = cudaMemcpyAsync(vel, d_out + 3 * np, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s->q);
-  cudaFree(d_out);
-  CKS(s, e);
+  if (pos) CKS(s, cudaMemcpyAsync(pos, d_out, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q));
+  if (vel) CKS(s, cudaMemcpyAsync(vel, d_out + 3 * np, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q));
   return sync_all(s);
 }
 
