@@ -13,7 +13,8 @@ def cartesian_to_elements(mu, r, v):
     a = 1.0 / (2.0 / rn - v2 / mu)
     evec = np.cross(v, h) / mu - r / rn[..., None]
     e = np.linalg.norm(evec, axis=-1)
-    inc = np.arccos(np.clip(h[..., 2] / hn, -1, 1))
+    # atan2 form: arccos(h_z/h) loses all precision for the near-planar orbits of the configs
+    inc = np.arctan2(np.hypot(h[..., 0], h[..., 1]), h[..., 2])
     Omega = np.arctan2(h[..., 0], -h[..., 1])
     node = np.stack([np.cos(Omega), np.sin(Omega), np.zeros_like(Omega)], axis=-1)
     # argument of latitude of pericentre measured in the orbital plane
