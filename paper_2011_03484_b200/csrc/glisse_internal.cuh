@@ -12,6 +12,9 @@ constexpr int kMaxPlanets = GLISSE_MAX_PLANETS;
 constexpr int kParticleBlock = 128;  // threads per particle-kernel block (one particle per thread)
 constexpr int kParticleWarps = kParticleBlock / 32;
 constexpr int kRingSlots = 2;        // planet-log stages resident in shared memory per WARP
+#ifndef GL_MIN_BLOCKS
+#define GL_MIN_BLOCKS 6
+#endif
 
 // Doubles per planet-log record (include/glisse.h: glisse_log_stride).
 __host__ __device__ inline int log_stride(int np) { return (3 * (np + 1) + 1) & ~1; }

@@ -71,6 +71,12 @@ __device__ __forceinline__ double rcp_f64_1(double a) {
   return fma(y, e, y);
 }
 
+// The polynomial coefficients live in the constant bank so that every DFMA of the Horner chains takes
+// its coefficient as a c[3][..] operand: as 64-bit immediates they cost two UMOV each per use, which
+// competes with the FP64 pipe for issue slots (profiles/r01: 54 UMOV per particle-step).
+static __constant__ double kSinCoef[6] = {GL_S0, GL_S1, GL_S2, GL_S3, GL_S4, GL_S5};
+static __constant__ double kCosCoef[6] = {GL_C0, GL_C1, GL_C2, GL_C3, GL_C4, GL_C5};
+
 __device__ __forceinline__ int hi_word(double x) { return __double2hiint(x); }
 
 // |x| <= pi/4, decided on the high word (integer pipe, not the FP64 pipe).  NaN/Inf -> false.
@@ -83,16 +89,16 @@ __device__ __forceinline__ bool is_small_angle(double x) {
 // in the two places the drift needs them: g ~ dM − x + sin x and f − 1 ~ cos x − 1.
 __device__ __forceinline__ void sincosm_small(double x, double& sm, double& cm1) {
   const double t = x * x;
-  double ps = fma(t, GL_S5, GL_S4);
-  double pc = fma(t, GL_C5, GL_C4);
-  ps = fma(t, ps, GL_S3);
-  pc = fma(t, pc, GL_C3);
-  ps = fma(t, ps, GL_S2);
-  pc = fma(t, pc, GL_C2);
-  ps = fma(t, ps, GL_S1);
-  pc = fma(t, pc, GL_C1);
-  ps = fma(t, ps, GL_S0);
-  pc = fma(t, pc, GL_C0);
+  double ps = fma(t, kSinCoef[5], kSinCoef[4]);
+  double pc = fma(t, kCosCoef[5], kCosCoef[4]);
+  ps = fma(t, ps, kSinCoef[3]);
+  pc = fma(t, pc, kCosCoef[3]);
+  ps = fma(t, ps, kSinCoef[2]);
+  pc = fma(t, pc, kCosCoef[2]);
+  ps = fma(t, ps, kSinCoef[1]);
+  pc = fma(t, pc, kCosCoef[1]);
+  ps = fma(t, ps, kSinCoef[0]);
+  pc = fma(t, pc, kCosCoef[0]);
   const double x3 = t * x;
   const double t2 = t * t;
   const double mh = -0.5 * t;

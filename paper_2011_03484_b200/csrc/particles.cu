@@ -59,7 +59,7 @@ __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier
 
 // NP > 0: compile-time planet count (fully unrolled kick); NP == 0: run-time count a.np.
 template <int NP>
-__global__ void __launch_bounds__(kParticleBlock) particle_kernel(const __grid_constant__ ParticleArgs a) {
+__global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel(const __grid_constant__ ParticleArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31;
   const int warp = threadIdx.x >> 5;
