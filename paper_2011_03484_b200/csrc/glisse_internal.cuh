@@ -9,7 +9,14 @@
 namespace glisse {
 
 constexpr int kMaxPlanets = GLISSE_MAX_PLANETS;
-constexpr int kParticleBlock = 128;  // threads per particle-kernel block (one particle per thread)
+#ifndef GL_BLOCK
+#define GL_BLOCK 128
+#endif
+#ifndef GL_PPT
+#define GL_PPT 1
+#endif
+constexpr int kParticleBlock = GL_BLOCK;     // threads per particle-kernel block
+constexpr int kParticlesPerThread = GL_PPT;  // particles per thread (independent instruction streams)
 constexpr int kParticleWarps = kParticleBlock / 32;
 constexpr int kRingSlots = 2;        // planet-log stages resident in shared memory per WARP
 #ifndef GL_MIN_BLOCKS

@@ -106,116 +106,189 @@ __device__ __forceinline__ void sincosm_small(double x, double& sm, double& cm1)
   cm1 = fma(t2, pc, mh);
 }
 
-// sm, cm1 for any x.  Must be called by all 32 lanes; `live` lanes whose |x| > pi/4 take the
-// library sincos (full argument reduction), chosen per lane, skipped when no lane needs it.
-__device__ __forceinline__ void sincosm_warp(bool live, double x, double& sm, double& cm1) {
-  sincosm_small(x, sm, cm1);
-  const bool big = live && !is_small_angle(x);
-  if (__any_sync(kFullMask, big)) {
-    if (big) {
-      double s, c;
-      sincos(x, &s, &c);
-      sm = s - x;
-      cm1 = c - 1.0;
+// sm, cm1 for any x, P bodies per lane.  Must be called by all 32 lanes; `live` bodies whose |x| > pi/4
+// take the library sincos (full argument reduction), chosen per body, skipped when no lane needs it.
+template <int P>
+__device__ __forceinline__ void sincosm_warp(const bool (&live)[P], const double (&x)[P], double (&sm)[P],
+                                             double (&cm1)[P]) {
+  bool big[P];
+  bool any_big = false;
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    sincosm_small(x[p], sm[p], cm1[p]);
+    big[p] = live[p] && !is_small_angle(x[p]);
+    any_big = any_big || big[p];
+  }
+  if (__any_sync(kFullMask, any_big)) {
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+      if (big[p]) {
+        double s, c;
+        sincos(x[p], &s, &c);
+        sm[p] = s - x[p];
+        cm1[p] = c - 1.0;
+      }
     }
   }
 }
 
-// Kepler drift of one body per lane about a point mass mu for time dt.  All 32 lanes must call;
-// `live` marks lanes whose body is to be advanced.  r2 = |r|^2 on entry; inv_mu = 1/mu and
-// inv_mu_dt = dt/mu are passed in because they are constants of the run.  Returns 0,
-// GLISSE_FLAG_NONCONV (3) or GLISSE_FLAG_UNBOUND (4); on a non-zero return, or for !live lanes,
-// the state is untouched.
-__device__ __forceinline__ int kepler_drift_warp(bool live, double mu, double inv_mu, double inv_mu_dt,
-                                                 int iters, double tol, double r2, double& x, double& y,
-                                                 double& z, double& vx, double& vy, double& vz) {
-  const double v2 = fma(vx, vx, fma(vy, vy, vz * vz));
-  const double u = fma(x, vx, fma(y, vy, z * vz));
-  const double rinv = rsqrt_f64(r2);
-  const double r0 = r2 * rinv;
-  const double alpha = fma(2.0 * mu, rinv, -v2);  // mu / a
-  const bool live_in = live;
-  const bool unbound = !(alpha > 0.0);
-  live = live && !unbound;
-  const double al = live ? alpha : 1.0;  // dead lanes stay finite so they never trigger slow paths
-  const double rsa = rsqrt_f64(al);
-  const double sqa = al * rsa;        // sqrt(alpha) = n a
-  const double inva = rsa * rsa;      // 1 / alpha
-  const double q = r0 * (al * inv_mu);  // r0 / a = 1 − ec
-  const double ec = 1.0 - q;
-  const double es = u * (sqa * inv_mu);
-  const double ndt = (al * sqa) * inv_mu_dt;                   // n dt
-  const double dM = fma(-rint(ndt * kInvTwoPi), kTwoPi, ndt);  // reading S9
-  const double a = mu * inva;
-  const double invq = a * rinv;  // a / r0
+// Kepler drift of P bodies per lane about a point mass mu for time dt.  The P bodies of a lane are
+// independent instruction streams that the compiler interleaves: the drift of one body is a serial
+// chain of dependent FP64 operations (8 cycles each on sm_100), so P = 2 doubles the work in flight
+// per warp and halves the per-body share of every warp-wide vote, branch and constant load.
+// All 32 lanes must call; `live[p]` marks bodies to be advanced.  r2 = |r|^2 on entry; inv_mu = 1/mu
+// and inv_mu_dt = dt/mu are constants of the run.  st[p] returns 0, GLISSE_FLAG_NONCONV (3) or
+// GLISSE_FLAG_UNBOUND (4); on a non-zero status, or for !live bodies, the state is untouched.
+// A body's arithmetic never depends on the other bodies of its lane or warp.
+template <int P>
+__device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], double mu, double inv_mu,
+                                                  double inv_mu_dt, int iters, double tol, const double (&r2)[P],
+                                                  double (&x)[P], double (&y)[P], double (&z)[P], double (&vx)[P],
+                                                  double (&vy)[P], double (&vz)[P], int (&st)[P]) {
+  bool live[P], unbound[P], simple[P], rough[P];
+  double rinv[P], sqa[P], rsa[P], q[P], ec[P], es[P], dM[P], a[P], invq[P], e2[P], xk[P];
+  bool any_rough = false;
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    const double v2 = fma(vx[p], vx[p], fma(vy[p], vy[p], vz[p] * vz[p]));
+    const double u = fma(x[p], vx[p], fma(y[p], vy[p], z[p] * vz[p]));
+    rinv[p] = rsqrt_f64(r2[p]);
+    const double r0 = r2[p] * rinv[p];
+    const double alpha = fma(2.0 * mu, rinv[p], -v2);  // mu / a
+    unbound[p] = !(alpha > 0.0);
+    live[p] = live_in[p] && !unbound[p];
+    const double al = live[p] ? alpha : 1.0;  // dead bodies stay finite so they never trigger slow paths
+    rsa[p] = rsqrt_f64(al);
+    sqa[p] = al * rsa[p];                    // sqrt(alpha) = n a
+    const double inva = rsa[p] * rsa[p];     // 1 / alpha
+    q[p] = r0 * (al * inv_mu);               // r0 / a = 1 − ec
+    ec[p] = 1.0 - q[p];
+    es[p] = u * (sqa[p] * inv_mu);
+    const double ndt = (al * sqa[p]) * inv_mu_dt;                   // n dt
+    dM[p] = fma(-rint(ndt * kInvTwoPi), kTwoPi, ndt);               // reading S9
+    a[p] = mu * inva;
+    invq[p] = a[p] * rinv[p];  // a / r0
 
-  // initial guess (reading S5): x1 = dM/q if |es| |x1| < q/4 and e x1^2 < q/4, compared squared
-  const double x1 = dM * invq;
-  const double e2 = fma(ec, ec, es * es);
-  const double t1 = x1 * x1;
-  const double q16 = (0.25 * q) * (0.25 * q);
-  const bool simple = ((es * es) * t1 < q16) && ((e2 * t1) * t1 < q16);
-  double xk = x1;
-  if (__any_sync(kFullMask, live && !simple)) {
-    const double yy = dM - es;
-    double sy, cy;
-    sincosm_warp(live && !simple, yy, sy, cy);
-    const double sg = fma(es, 1.0 + cy, ec * (yy + sy));
-    const double e = sqrt(e2);
-    if (!simple) xk = yy + (sg >= 0.0 ? 0.85 : -0.85) * e;
+    // initial guess (reading S5): x1 = dM/q if |es| |x1| < q/4 and e x1^2 < q/4, compared squared
+    const double x1 = dM[p] * invq[p];
+    e2[p] = fma(ec[p], ec[p], es[p] * es[p]);
+    const double t1 = x1 * x1;
+    const double q16 = (0.25 * q[p]) * (0.25 * q[p]);
+    simple[p] = ((es[p] * es[p]) * t1 < q16) && ((e2[p] * t1) * t1 < q16);
+    xk[p] = x1;
+    rough[p] = live[p] && !simple[p];
+    any_rough = any_rough || rough[p];
   }
-  if (!live) xk = 0.0;
-
-  // Newton updates, warp-uniform exit.  After a lane's last update d (|d| <= eps)
-  // its sin/cos at x − d follow from those at x by angle addition instead of a fresh evaluation.
-  bool conv = !live;
-  double sm = 0.0, cm1 = 0.0;  // sin x − x, cos x − 1 at the current xk
-  for (int it = 0; it < iters; ++it) {
-    double smk, cmk;
-    sincosm_warp(!conv, xk, smk, cmk);
-    const double s = xk + smk;
-    const double f = fma(-es, cmk, fma(-ec, s, xk - dM));
-    const double fp = fma(es, s, fma(-ec, cmk, q));
-    const double d = f * rcp_f64_1(fp);
-    if (!conv) {
-      conv = fabs(d) <= kExitEps;
-      // sin(x − d) − (x − d), cos(x − d) − 1 to O(d^3); exact enough only once |d| <= eps
-      const double c = 1.0 + cmk;
-      const double hd = 0.5 * d;
-      sm = fma(-d, fma(hd, s, cmk), smk);
-      cm1 = fma(d, fma(-hd, c, s), cmk);
-      xk -= d;
+  if (__any_sync(kFullMask, any_rough)) {
+    double yy[P], sy[P], cy[P];
+#pragma unroll
+    for (int p = 0; p < P; ++p) yy[p] = dM[p] - es[p];
+    sincosm_warp<P>(rough, yy, sy, cy);
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+      const double sg = fma(es[p], 1.0 + cy[p], ec[p] * (yy[p] + sy[p]));
+      const double e = sqrt(e2[p]);
+      if (!simple[p]) xk[p] = yy[p] + (sg >= 0.0 ? 0.85 : -0.85) * e;
     }
-    if (__all_sync(kFullMask, conv)) break;
   }
-  // lanes that ran out of updates (or iters == 0) need a fresh evaluation at the final x
-  if (__any_sync(kFullMask, !conv)) {
-    double smk, cmk;
-    sincosm_warp(!conv, xk, smk, cmk);
-    if (!conv) { sm = smk; cm1 = cmk; }
-  }
-  const double s = xk + sm;
-  const double rho = fma(-es, cm1, fma(-ec, s, xk - dM));  // residual of Kepler's equation
-  const bool nonconv = !(fabs(rho) <= tol);
 
-  // Gauss f, g (PAPER.md:94 step 4), applied as r += (f−1) r + g v, v += fdot r + (gdot−1) v
-  const double p = fma(es, s, fma(-ec, cm1, q));  // r(t)/a
-  const double invp = rcp_f64(p);
-  const double fm1 = cm1 * invq;
-  const double g = (dM + sm) * (a * rsa);  // (dM − x + sin x) / n
-  const double fd = -(s * invp) * (sqa * rinv);
-  const double gm1 = cm1 * invp;
-  if (live && !nonconv) {
-    const double nx = fma(fm1, x, fma(g, vx, x));
-    const double ny = fma(fm1, y, fma(g, vy, y));
-    const double nz = fma(fm1, z, fma(g, vz, z));
-    vx = fma(fd, x, fma(gm1, vx, vx));
-    vy = fma(fd, y, fma(gm1, vy, vy));
-    vz = fma(fd, z, fma(gm1, vz, vz));
-    x = nx; y = ny; z = nz;
+  // Newton updates, warp-uniform exit.  After a body's last update d (|d| <= eps)
+  // its sin/cos at x − d follow from those at x by angle addition instead of a fresh evaluation.
+  bool conv[P], open[P];
+  double sm[P], cm1[P];  // sin x − x, cos x − 1 at the current xk
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    if (!live[p]) xk[p] = 0.0;
+    conv[p] = !live[p];
+    sm[p] = 0.0;
+    cm1[p] = 0.0;
   }
-  if (!live_in) return 0;
-  return unbound ? GLISSE_FLAG_UNBOUND : (nonconv ? GLISSE_FLAG_NONCONV : 0);
+  for (int it = 0; it < iters; ++it) {
+    double smk[P], cmk[P];
+#pragma unroll
+    for (int p = 0; p < P; ++p) open[p] = !conv[p];
+    sincosm_warp<P>(open, xk, smk, cmk);
+    bool all_conv = true;
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+      const double s = xk[p] + smk[p];
+      const double f = fma(-es[p], cmk[p], fma(-ec[p], s, xk[p] - dM[p]));
+      const double fp = fma(es[p], s, fma(-ec[p], cmk[p], q[p]));
+      const double d = f * rcp_f64_1(fp);
+      if (!conv[p]) {
+        conv[p] = fabs(d) <= kExitEps;
+        // sin(x − d) − (x − d), cos(x − d) − 1 to O(d^3); exact enough only once |d| <= eps
+        const double c = 1.0 + cmk[p];
+        const double hd = 0.5 * d;
+        sm[p] = fma(-d, fma(hd, s, cmk[p]), smk[p]);
+        cm1[p] = fma(d, fma(-hd, c, s), cmk[p]);
+        xk[p] -= d;
+      }
+      all_conv = all_conv && conv[p];
+    }
+    if (__all_sync(kFullMask, all_conv)) break;
+  }
+  // bodies that ran out of updates (or iters == 0) need a fresh evaluation at the final x
+  bool any_open = false;
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    open[p] = !conv[p];
+    any_open = any_open || open[p];
+  }
+  if (__any_sync(kFullMask, any_open)) {
+    double smk[P], cmk[P];
+    sincosm_warp<P>(open, xk, smk, cmk);
+#pragma unroll
+    for (int p = 0; p < P; ++p)
+      if (open[p]) { sm[p] = smk[p]; cm1[p] = cmk[p]; }
+  }
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    const double s = xk[p] + sm[p];
+    const double rho = fma(-es[p], cm1[p], fma(-ec[p], s, xk[p] - dM[p]));  // residual of Kepler's equation
+    const bool nonconv = !(fabs(rho) <= tol);
+
+    // Gauss f, g (PAPER.md:94 step 4), applied as r += (f−1) r + g v, v += fdot r + (gdot−1) v
+    const double pr = fma(es[p], s, fma(-ec[p], cm1[p], q[p]));  // r(t)/a
+    const double invp = rcp_f64(pr);
+    const double fm1 = cm1[p] * invq[p];
+    const double g = (dM[p] + sm[p]) * (a[p] * rsa[p]);  // (dM − x + sin x) / n
+    const double fd = -(s * invp) * (sqa[p] * rinv[p]);
+    const double gm1 = cm1[p] * invp;
+    if (live[p] && !nonconv) {
+      const double nx = fma(fm1, x[p], fma(g, vx[p], x[p]));
+      const double ny = fma(fm1, y[p], fma(g, vy[p], y[p]));
+      const double nz = fma(fm1, z[p], fma(g, vz[p], z[p]));
+      vx[p] = fma(fd, x[p], fma(gm1, vx[p], vx[p]));
+      vy[p] = fma(fd, y[p], fma(gm1, vy[p], vy[p]));
+      vz[p] = fma(fd, z[p], fma(gm1, vz[p], vz[p]));
+      x[p] = nx; y[p] = ny; z[p] = nz;
+    }
+    st[p] = !live_in[p] ? 0 : (unbound[p] ? GLISSE_FLAG_UNBOUND : (nonconv ? GLISSE_FLAG_NONCONV : 0));
+  }
+}
+
+// One body per lane (the planet-history kernel and the primitive test hook).
+__device__ __forceinline__ int kepler_drift_warp(bool live, double mu, double inv_mu, double inv_mu_dt, int iters,
+                                                 double tol, double r2, double& x, double& y, double& z,
+                                                 double& vx, double& vy, double& vz) {
+  const bool l1[1] = {live};
+  const double r21[1] = {r2};
+  double x1[1] = {x}, y1[1] = {y}, z1[1] = {z}, vx1[1] = {vx}, vy1[1] = {vy}, vz1[1] = {vz};
+  int st[1];
+  kepler_drift_warp<1>(l1, mu, inv_mu, inv_mu_dt, iters, tol, r21, x1, y1, z1, vx1, vy1, vz1, st);
+  x = x1[0]; y = y1[0]; z = z1[0]; vx = vx1[0]; vy = vy1[0]; vz = vz1[0];
+  return st[0];
+}
+
+// single-body sin x − x, cos x − 1 (test hook)
+__device__ __forceinline__ void sincosm_warp(bool live, double x, double& sm, double& cm1) {
+  const bool l1[1] = {live};
+  const double x1[1] = {x};
+  double s1[1], c1[1];
+  sincosm_warp<1>(l1, x1, s1, c1);
+  sm = s1[0];
+  cm1 = c1[0];
 }
 
 }  // namespace glisse

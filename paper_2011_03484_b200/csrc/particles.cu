@@ -58,7 +58,8 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 // NP > 0: compile-time planet count (fully unrolled kick); NP == 0: run-time count a.np.
-template <int NP>
+// P = particles per thread (kParticlesPerThread): independent instruction streams, see kepler.cuh.
+template <int NP, int P>
 __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel(const __grid_constant__ ParticleArgs a) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31;
@@ -70,21 +71,32 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   const int stage_doubles = R * stride;
 
   const int n = *a.n_slots;
-  const long long i = static_cast<long long>(blockIdx.x) * kParticleBlock + threadIdx.x;
-  const bool in_range = i < n;
+  // particle p of this thread: consecutive threads hold consecutive particles (coalesced), the P
+  // particles of a thread lie kParticleBlock apart
+  const long long i0 = static_cast<long long>(blockIdx.x) * (kParticleBlock * P) + threadIdx.x;
 
   // ---- a2: load ------------------------------------------------------------------------------
-  double x = 1.0, y = 0.0, z = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
-  int flag = -1;
-  if (in_range) {
-    flag = a.flag[i];
-    x = a.st[0][i]; y = a.st[1][i]; z = a.st[2][i];
-    vx = a.st[3][i]; vy = a.st[4][i]; vz = a.st[5][i];
+  double x[P], y[P], z[P], vx[P], vy[P], vz[P];
+  int flag[P];
+  bool was_alive[P], alive[P];
+  long long rs[P];
+  bool any_alive_t = false;
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    const long long i = i0 + p * kParticleBlock;
+    x[p] = 1.0; y[p] = 0.0; z[p] = 0.0; vx[p] = 0.0; vy[p] = 0.0; vz[p] = 0.0;
+    flag[p] = -1;
+    if (i < n) {
+      flag[p] = a.flag[i];
+      x[p] = a.st[0][i]; y[p] = a.st[1][i]; z[p] = a.st[2][i];
+      vx[p] = a.st[3][i]; vy[p] = a.st[4][i]; vz[p] = a.st[5][i];
+    }
+    was_alive[p] = (flag[p] == 0);
+    alive[p] = was_alive[p];
+    any_alive_t = any_alive_t || alive[p];
+    rs[p] = -1;
   }
-  const bool was_alive = (flag == 0);
-  bool alive = was_alive;
-  if (!__any_sync(kFullMask, alive)) return;  // nothing to do in this warp: leave before any copy
-  long long rs = -1;
+  if (!__any_sync(kFullMask, any_alive_t)) return;  // nothing to do in this warp: leave before any copy
   unsigned drifts = 0;
 
   // ---- warp-private ring ------------------------------------------------------------------------
@@ -119,46 +131,65 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
     for (int kk = 0; kk < recs; ++kk, ++k) {
       const double* rec = stage + kk * stride;
       // ---- a3/a4: force evaluation with the tests (O1/O4/O5) at time t_{step0+k} ----------------
-      const double r2 = fma(x, x, fma(y, y, z * z));
-      double ax = rec[3 * np], ay = rec[3 * np + 1], az = rec[3 * np + 2];  // h0
-      int hit = 0;
+      double r2[P], ax[P], ay[P], az[P];
+      int hit[P];
+#pragma unroll
+      for (int p = 0; p < P; ++p) {
+        r2[p] = fma(x[p], x[p], fma(y[p], y[p], z[p] * z[p]));
+        ax[p] = rec[3 * np]; ay[p] = rec[3 * np + 1]; az[p] = rec[3 * np + 2];  // h0
+        hit[p] = 0;
+      }
 #pragma unroll
       for (int jj = 0; jj < np; ++jj) {
         const int j = np - 1 - jj;  // descending, so the lowest index wins (reading S11)
-        const double dx = x - rec[3 * j], dy = y - rec[3 * j + 1], dz = z - rec[3 * j + 2];
-        const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        hit = (d2 < a.rc2[j]) ? (GLISSE_FLAG_PLANET0 + j) : hit;
-        const double ri = rsqrt_f64(d2);
-        const double w = (a.gm[j] * ri) * (ri * ri);
-        ax = fma(-w, dx, ax);
-        ay = fma(-w, dy, ay);
-        az = fma(-w, dz, az);
+        const double qx = rec[3 * j], qy = rec[3 * j + 1], qz = rec[3 * j + 2];
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+          const double dx = x[p] - qx, dy = y[p] - qy, dz = z[p] - qz;
+          const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
+          hit[p] = (d2 < a.rc2[j]) ? (GLISSE_FLAG_PLANET0 + j) : hit[p];
+          const double ri = rsqrt_f64(d2);
+          const double w = (a.gm[j] * ri) * (ri * ri);
+          ax[p] = fma(-w, dx, ax[p]);
+          ay[p] = fma(-w, dy, ay[p]);
+          az[p] = fma(-w, dz, az[p]);
+        }
       }
-      hit = (r2 > a.rmax2) ? GLISSE_FLAG_RMAX : hit;
-      hit = (r2 < a.rmin2) ? GLISSE_FLAG_RMIN : hit;
-      if (alive && hit != 0) {
-        flag = hit;
-        rs = a.step0 + k;
-        alive = false;
-      }
-      if (alive) {
-        vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
-        if (k > 0 && k < nsteps) {  // interior: closing half kick of step k-1 and opening of step k
-          vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
+      bool any_alive_k = false;
+#pragma unroll
+      for (int p = 0; p < P; ++p) {
+        hit[p] = (r2[p] > a.rmax2) ? GLISSE_FLAG_RMAX : hit[p];
+        hit[p] = (r2[p] < a.rmin2) ? GLISSE_FLAG_RMIN : hit[p];
+        if (alive[p] && hit[p] != 0) {
+          flag[p] = hit[p];
+          rs[p] = a.step0 + k;
+          alive[p] = false;
+        }
+        if (alive[p]) {
+          vx[p] = fma(ax[p], hdt, vx[p]); vy[p] = fma(ay[p], hdt, vy[p]); vz[p] = fma(az[p], hdt, vz[p]);
+          if (k > 0 && k < nsteps) {  // interior: closing half kick of step k-1 and opening of step k
+            vx[p] = fma(ax[p], hdt, vx[p]); vy[p] = fma(ay[p], hdt, vy[p]); vz[p] = fma(az[p], hdt, vz[p]);
+          }
         }
       }
       // ---- a5/a6: drift (O2) --------------------------------------------------------------------
       if (k < nsteps) {
-        drifts += alive ? 1u : 0u;
-        const int st_d = kepler_drift_warp(alive, a.mu, a.inv_mu, a.inv_mu_dt, a.iters, a.tol, r2, x, y, z,
-                                           vx, vy, vz);
-        if (st_d != 0) {
-          flag = st_d;
-          rs = a.step0 + k;
-          alive = false;
+        int st_d[P];
+#pragma unroll
+        for (int p = 0; p < P; ++p) drifts += alive[p] ? 1u : 0u;
+        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, a.inv_mu_dt, a.iters, a.tol, r2, x, y, z, vx, vy, vz, st_d);
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+          if (st_d[p] != 0) {
+            flag[p] = st_d[p];
+            rs[p] = a.step0 + k;
+            alive[p] = false;
+          }
         }
       }
-      any_alive = __any_sync(kFullMask, alive);
+#pragma unroll
+      for (int p = 0; p < P; ++p) any_alive_k = any_alive_k || alive[p];
+      any_alive = __any_sync(kFullMask, any_alive_k);
       if (!any_alive) break;
     }
     if (!any_alive) break;
@@ -179,12 +210,16 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   }
 
   // ---- a7: store --------------------------------------------------------------------------------
-  if (was_alive) {  // particles that were already removed at load are untouched
-    a.st[0][i] = x; a.st[1][i] = y; a.st[2][i] = z;
-    a.st[3][i] = vx; a.st[4][i] = vy; a.st[5][i] = vz;
-    if (flag != 0) {
-      a.flag[i] = flag;
-      a.rstep[i] = rs;
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    if (was_alive[p]) {  // particles that were already removed at load are untouched
+      const long long i = i0 + p * kParticleBlock;
+      a.st[0][i] = x[p]; a.st[1][i] = y[p]; a.st[2][i] = z[p];
+      a.st[3][i] = vx[p]; a.st[4][i] = vy[p]; a.st[5][i] = vz[p];
+      if (flag[p] != 0) {
+        a.flag[i] = flag[p];
+        a.rstep[i] = rs[p];
+      }
     }
   }
   unsigned tot = __reduce_add_sync(kFullMask, drifts);
@@ -201,19 +236,22 @@ size_t particle_smem_bytes(const ParticleArgs& a) {
 cudaError_t configure_particle_kernels() {
   cudaError_t e;
   const int carve = cudaSharedmemCarveoutMaxShared;
-  if ((e = cudaFuncSetAttribute(particle_kernel<0>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  if ((e = cudaFuncSetAttribute(particle_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  if ((e = cudaFuncSetAttribute(particle_kernel<8>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
+  constexpr int P = kParticlesPerThread;
+  if ((e = cudaFuncSetAttribute(particle_kernel<0, P>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
+  if ((e = cudaFuncSetAttribute(particle_kernel<4, P>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
+  if ((e = cudaFuncSetAttribute(particle_kernel<8, P>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
   return cudaSuccess;
 }
 
 cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_slots_upper, cudaStream_t s) {
   if (n_slots_upper < 1) n_slots_upper = 1;
-  const int blocks = (n_slots_upper + kParticleBlock - 1) / kParticleBlock;
+  constexpr int P = kParticlesPerThread;
+  const int per_block = kParticleBlock * P;
+  const int blocks = (n_slots_upper + per_block - 1) / per_block;
   const size_t smem = particle_smem_bytes(a);
-  if (a.np == 4) particle_kernel<4><<<blocks, kParticleBlock, smem, s>>>(a);
-  else if (a.np == 8) particle_kernel<8><<<blocks, kParticleBlock, smem, s>>>(a);
-  else particle_kernel<0><<<blocks, kParticleBlock, smem, s>>>(a);
+  if (a.np == 4) particle_kernel<4, P><<<blocks, kParticleBlock, smem, s>>>(a);
+  else if (a.np == 8) particle_kernel<8, P><<<blocks, kParticleBlock, smem, s>>>(a);
+  else particle_kernel<0, P><<<blocks, kParticleBlock, smem, s>>>(a);
   return cudaGetLastError();
 }
 
