@@ -39,12 +39,24 @@ CHUNK = 1024                     # BASELINE.json configs[1]: "planet-history chu
 METRIC = "particle-steps/sec (fp64, 1 B200)"
 UNIT = "particle-steps/s"
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
+# dram__bytes_read.sum + dram__bytes_write.sum per particle-kernel launch, from the ncu --set full
+# captures under profiles/ (the kernel is ALU-bound; this only shows that state traffic is negligible)
+TRAFFIC_BYTES_PER_LAUNCH = {"c2": 6.7e6, "1m_x4": 5.3e7}
 
 # Counted fp64 flops per particle-step of the particle kernel (DFMA = 2, DADD/DMUL = 1, compares,
-# MUFU seeds and integer work = 0), from the ncu instruction counters of profiles/ on the bench
-# workload (DESIGN.md §6 states the derivation): N_p = 4 and N_p = 8.
-FLOPS_PER_PSTEP = {4: 352.0, 8: 472.0}
-FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz
+# MUFU seeds and integer work = 0): the ncu instruction counters of the current kernel
+# (profiles/*_particle_kernel_*.md, "Derived per launch") divided by the thread-steps of the launch;
+# DESIGN.md §7 states the derivation.  N_p = 4 is measured; other N_p add 25 flops per planet (the
+# kick's per-planet instruction count).
+FLOPS_PER_PSTEP_NP4 = 328.0
+FLOPS_PER_PLANET = 25.0
+# FP64 peak: ncu reports sm__sass_thread_inst_executed_op_dfma_pred_on.sum.peak_sustained = 64 per SM
+# per cycle; x 148 SMs x 2 flops x 1.965 GHz (clocks.max.sm of B200_PROFILING.md)
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
+def flops_per_pstep(n_planets: int) -> float:
+    return FLOPS_PER_PSTEP_NP4 + FLOPS_PER_PLANET * (n_planets - 4)
 
 WORKLOADS = {
     "c2": ("BASELINE.json configs[1]: 4 giants, 131,072 particles a~U[20,28], dt=180 d, K=1024", lambda n: inputs.config(2, n)),
@@ -293,17 +305,18 @@ def main():
     value = psteps / (ms * 1e-3)
 
     # roofline of the dominant kernel (rank 0's launches)
-    fl = FLOPS_PER_PSTEP.get(w.n_planets, FLOPS_PER_PSTEP[4] + 30.0 * (w.n_planets - 4))
+    fl = flops_per_pstep(w.n_planets)
     k_ms = res["kernel_ms"] / max(res["kernel_launches"], 1)
     achieved = fl * (res["psteps"] / max(res["kernel_launches"], 1)) / (k_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "achieved": achieved, "peak": peak / 1e12, "unit": "TFLOP/s",
-                "frac": achieved / (peak / 1e12), "traffic": None,
+    roofline = {"bound": "alu", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved / FP64_NOMINAL_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload),
                 "kernel": "particle_kernel", "kernel_ms_per_launch": k_ms,
                 "kernel_share_of_step": res["kernel_ms"] / res["ms"],
                 "flops_per_particle_step": fl,
-                "peak_source": "measured in this run: glisse_fp64_peak_probe (register-resident DFMA loop); "
-                               f"nominal 148 SM x 64 lanes x 2 x 1.965 GHz = {FP64_NOMINAL_TFLOPS:.1f} TFLOP/s",
-                "frac_of_nominal": achieved / FP64_NOMINAL_TFLOPS}
+                "peak_source": "nominal FP64 FMA rate: 148 SMs x 64 DFMA lanes (ncu peak_sustained) x 2 x "
+                               "1.965 GHz; MEASURED_PEAKS.json has no FP64 figure",
+                "probe_tflops": peak / 1e12, "frac_of_probe": achieved / (peak / 1e12),
+                "probe": "glisse_fp64_peak_probe: register-resident DFMA chains timed in this run"}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -335,10 +348,11 @@ def main():
                 _, wt = make_workload("1m_x4")
                 rt = time_resident(binding, torch, wt, max(3, args.steps // 4), 3, device, flush)
                 kt = rt["kernel_ms"] / max(rt["kernel_launches"], 1)
-                at = FLOPS_PER_PSTEP[4] * (rt["psteps"] / max(rt["kernel_launches"], 1)) / (kt * 1e-3) / 1e12
+                at = flops_per_pstep(4) * (rt["psteps"] / max(rt["kernel_launches"], 1)) / (kt * 1e-3) / 1e12
                 line["target_1m_x4"] = {"value": rt["psteps"] / (rt["ms"] * 1e-3), "unit": UNIT,
                                         "ms_per_step": rt["ms"] / max(3, args.steps // 4),
-                                        "roofline_frac": at / (peak / 1e12), "achieved_tflops": at,
+                                        "roofline_frac": at / FP64_NOMINAL_TFLOPS, "achieved_tflops": at,
+                                        "frac_of_probe": at / (peak / 1e12),
                                         "workload": WORKLOADS["1m_x4"][0]}
             rate, secs, ps = oracle_rate(w, 16384, 3000)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
