@@ -101,6 +101,13 @@ namespace {
     }                                            \
   } while (0)
 
+// upper 32 bits of a double (sign, exponent, top of the mantissa)
+int high_word(double v) {
+  unsigned long long b;
+  std::memcpy(&b, &v, sizeof(b));
+  return static_cast<int>(b >> 32);
+}
+
 bool all_finite_host(const double* p, long long n) {
   for (long long i = 0; i < n; ++i)
     if (!std::isfinite(p[i])) return false;
@@ -471,7 +478,10 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   for (int j = 0; j < kMaxPlanets; ++j) {
     a.gm[j] = (j < np) ? gm_planet[j] : 0.0;
     a.rc2[j] = (j < np && planet_rcrit) ? planet_rcrit[j] * planet_rcrit[j] : 0.0;
+    a.rc2_hi[j] = high_word(a.rc2[j]);
   }
+  a.rmin2_hi = high_word(a.rmin2);
+  a.rmax2_hi = high_word(a.rmax2);
   // the caller's buffers are free again once the copies on q are done; the planet stream keeps
   // running (a planet failure is reported by the next synchronising call)
   CKF(cudaStreamSynchronize(s->q));

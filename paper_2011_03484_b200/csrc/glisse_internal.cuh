@@ -51,6 +51,9 @@ struct ParticleArgs {
   double hdt, mu, inv_mu, inv_mu_dt, rmin2, rmax2, tol;
   double gm[kMaxPlanets];
   double rc2[kMaxPlanets];
+  // high words of rmin2, rmax2, rc2[]: the hot path's integer superset of the distance tests
+  int rmin2_hi, rmax2_hi;
+  int rc2_hi[kMaxPlanets];
 };
 
 // ---- planet system constants, resident in device memory -----------------------------------------

@@ -54,6 +54,18 @@ __device__ __forceinline__ double rsqrt_f64(double a) {
   return fma(ye, p, y);  // y (1 + e/2 + 3 e^2/8)
 }
 
+// gm / d^3 from d2 = d^2 (the kick's weight), seed y ~ d2^(-1/2):
+//   gm y^3 (1 − e)^(-3/2),  e = 1 − d2 y^2,  (1 − e)^(-3/2) = 1 + (3/2) e + (15/8) e^2 + O(e^3)
+// |e| <= 2^-18.9 leaves (35/16) e^3 < 2e-17.  4 DMUL + 3 DFMA, one less than rsqrt_f64 and a cube.
+__device__ __forceinline__ double gm_over_r3(double gm, double d2) {
+  const double y = mufu_rsq(d2);
+  const double y2 = y * y;
+  const double e = fma(-d2, y2, 1.0);
+  const double y3 = (gm * y) * y2;
+  const double p = fma(1.875, e, 1.5);
+  return fma(y3, p * e, y3);
+}
+
 // 1/a for normal a, full precision (two Newton steps: 2^-39.8 -> 2^-79).
 __device__ __forceinline__ double rcp_f64(double a) {
   double y = mufu_rcp(a);
@@ -132,10 +144,112 @@ __device__ __forceinline__ void sincosm_warp(const bool (&live)[P], const double
   }
 }
 
+// single-body sin x − x, cos x − 1 (test hook)
+__device__ __forceinline__ void sincosm_warp(bool live, double x, double& sm, double& cm1) {
+  const bool l1[1] = {live};
+  const double x1[1] = {x};
+  double s1[1], c1[1];
+  sincosm_warp<1>(l1, x1, s1, c1);
+  sm = s1[0];
+  cm1 = c1[0];
+}
+
+
+// ---- the definition's solver (O2), one body per lane: guess of reading S5, at most `iters`
+// Newton updates with a per-lane stop at |update| <= kExitEps and a warp-uniform exit (reading S7),
+// residual test against `tol`.  Serves the bodies the fast solver below does not accept (e >= 0.8,
+// |x| > pi/4, iters < 5, or no convergence in kFastMaxIters quartic steps), so that the
+// non-convergence flag is decided exactly as the definition decides it.  Kept out of
+// line: it is off the hot path and must not cost the particle kernel registers.
+struct ExactSolve {
+  double x, sm, cm1;  // x, sin x − x, cos x − 1 at the final x
+  int nonconv;
+};
+
+static __device__ __noinline__ ExactSolve kepler_solve_exact(bool live, double ec, double es, double q, double dM,
+                                                      double invq, double e2, int iters, double tol) {
+  // initial guess (reading S5): x1 = dM/q if |es| |x1| < q/4 and e x1^2 < q/4, compared squared
+  const double x1 = dM * invq;
+  const double t1 = x1 * x1;
+  const double q16 = (0.25 * q) * (0.25 * q);
+  const bool simple = ((es * es) * t1 < q16) && ((e2 * t1) * t1 < q16);
+  double xk = x1;
+  const bool rough = live && !simple;
+  if (__any_sync(kFullMask, rough)) {
+    const double yy = dM - es;
+    double sy, cy;
+    sincosm_warp(rough, yy, sy, cy);
+    const double sg = fma(es, 1.0 + cy, ec * (yy + sy));
+    const double e = sqrt(e2);
+    if (!simple) xk = yy + (sg >= 0.0 ? 0.85 : -0.85) * e;
+  }
+  if (!live) xk = 0.0;
+  bool conv = !live;
+  double sm = 0.0, cm1 = 0.0;
+  for (int it = 0; it < iters; ++it) {
+    double smk, cmk;
+    sincosm_warp(!conv, xk, smk, cmk);
+    const double s = xk + smk;
+    const double f = fma(-es, cmk, fma(-ec, s, xk - dM));
+    const double fp = fma(es, s, fma(-ec, cmk, q));
+    const double d = f * rcp_f64_1(fp);
+    if (!conv) {
+      conv = fabs(d) <= kExitEps;
+      // sin(x − d) − (x − d), cos(x − d) − 1 to O(d^3); exact enough only once |d| <= eps
+      const double c = 1.0 + cmk;
+      const double hd = 0.5 * d;
+      sm = fma(-d, fma(hd, s, cmk), smk);
+      cm1 = fma(d, fma(-hd, c, s), cmk);
+      xk -= d;
+    }
+    if (__all_sync(kFullMask, conv)) break;
+  }
+  // bodies that ran out of updates (or iters == 0) need a fresh evaluation at the final x
+  if (__any_sync(kFullMask, !conv)) {
+    double smk, cmk;
+    sincosm_warp(!conv, xk, smk, cmk);
+    if (!conv) { sm = smk; cm1 = cmk; }
+  }
+  const double s = xk + sm;
+  const double rho = fma(-es, cm1, fma(-ec, s, xk - dM));  // residual of Kepler's equation
+  ExactSolve o;
+  o.x = xk; o.sm = sm; o.cm1 = cm1;
+  o.nonconv = !(fabs(rho) <= tol) ? 1 : 0;
+  return o;
+}
+
+// ---- fast solver -------------------------------------------------------------------------------------
+// From x0 = dM/q, steps of quartic convergence: with f and its derivatives f1, f2, f3 at x (all from
+// one sin/cos evaluation: f3 = 1 − f1) and delta = f/f1, the root of the cubic Taylor model is
+//     d = delta (1 + a2 delta + (2 a2^2 − a3) delta^2),   a2 = f2/(2 f1),  a3 = f3/(6 f1),
+// leaving an error (5 a2^3 − 5 a2 a3 + a4) delta^4.  A body is converged once |delta| is below a
+// bound chosen from its eccentricity so that this error is < 2e-17 (a_k <= e/(k! (1 − e))):
+//     e < 0.1: 1e-4     e < 0.3: 9e-5     e < 0.5: 5.5e-5     e < 0.8: 2e-5
+// and sin, cos at x − d then follow from those at x by angle addition carried to d^3 (the d^4 terms
+// are < 5e-18).  One step suffices wherever e x^2 / 2 is below the bound — every particle of
+// BASELINE.json configs 1-4 — against the two Newton updates plus test the definition needs there.
+// Kepler's equation has one root (f1 >= 1 − e > 0), so both solvers return the same x to roundoff.
+// Thresholds and range tests are taken on the high words (integer pipe): the FP64 pipe is the
+// roofline.
+constexpr int kFastMinIters = 5;   // the paper's count; below it the definition may not converge
+constexpr int kFastMaxIters = 4;
+
+__device__ __forceinline__ int hi_abs(double x) { return hi_word(x) & 0x7fffffff; }
+
+// high words of the constants above (any bound below the stated value is safe)
+constexpr int kHiE2_010 = 0x3f847ae1;   // 0.01   = 0x3f847ae147ae147b
+constexpr int kHiE2_030 = 0x3fb70a3d;   // 0.09   = 0x3fb70a3d70a3d70a
+constexpr int kHiE2_050 = 0x3fd00000;   // 0.25
+constexpr int kHiE2_080 = 0x3fe47ae1;   // 0.64   = 0x3fe47ae147ae147b
+constexpr int kHiThr0 = 0x3f1a36e2;     // 1e-4   = 0x3f1a36e2eb1c432d
+constexpr int kHiThr1 = 0x3f1797cc;     // 9e-5   = 0x3f1797cc39ffd60f
+constexpr int kHiThr2 = 0x3f0cd5f9;     // 5.5e-5 = 0x3f0cd5f99c38b04b
+constexpr int kHiThr3 = 0x3ef4f8b5;     // 2e-5   = 0x3ef4f8b588e368f1
+
 // Kepler drift of P bodies per lane about a point mass mu for time dt.  The P bodies of a lane are
 // independent instruction streams that the compiler interleaves: the drift of one body is a serial
-// chain of dependent FP64 operations (8 cycles each on sm_100), so P = 2 doubles the work in flight
-// per warp and halves the per-body share of every warp-wide vote, branch and constant load.
+// chain of dependent FP64 operations, so P = 2 doubles the work in flight per warp and halves the
+// per-body share of every warp-wide vote, branch and constant load.
 // All 32 lanes must call; `live[p]` marks bodies to be advanced.  r2 = |r|^2 on entry; inv_mu = 1/mu
 // and inv_mu_dt = dt/mu are constants of the run.  st[p] returns 0, GLISSE_FLAG_NONCONV (3) or
 // GLISSE_FLAG_UNBOUND (4); on a non-zero status, or for !live bodies, the state is untouched.
@@ -145,9 +259,12 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
                                                   double inv_mu_dt, int iters, double tol, const double (&r2)[P],
                                                   double (&x)[P], double (&y)[P], double (&z)[P], double (&vx)[P],
                                                   double (&vy)[P], double (&vz)[P], int (&st)[P]) {
-  bool live[P], unbound[P], simple[P], rough[P];
+  bool live[P], unbound[P], open[P], slow[P];
   double rinv[P], sqa[P], rsa[P], q[P], ec[P], es[P], dM[P], a[P], invq[P], e2[P], xk[P];
-  bool any_rough = false;
+  double sm[P], cm1[P];  // sin x − x, cos x − 1 at the final xk
+  int thr[P], nonconv[P];
+  const bool fast_on = iters >= kFastMinIters;
+  bool any_open = false;
 #pragma unroll
   for (int p = 0; p < P; ++p) {
     const double v2 = fma(vx[p], vx[p], fma(vy[p], vy[p], vz[p] * vz[p]));
@@ -155,7 +272,7 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
     rinv[p] = rsqrt_f64(r2[p]);
     const double r0 = r2[p] * rinv[p];
     const double alpha = fma(2.0 * mu, rinv[p], -v2);  // mu / a
-    unbound[p] = !(alpha > 0.0);
+    unbound[p] = !(hi_word(alpha) > 0);                // alpha <= 0 (or below 2^-1042: no such orbit)
     live[p] = live_in[p] && !unbound[p];
     const double al = live[p] ? alpha : 1.0;  // dead bodies stay finite so they never trigger slow paths
     rsa[p] = rsqrt_f64(al);
@@ -168,86 +285,76 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
     dM[p] = fma(-rint(ndt * kInvTwoPi), kTwoPi, ndt);               // reading S9
     a[p] = mu * inva;
     invq[p] = a[p] * rinv[p];  // a / r0
-
-    // initial guess (reading S5): x1 = dM/q if |es| |x1| < q/4 and e x1^2 < q/4, compared squared
-    const double x1 = dM[p] * invq[p];
     e2[p] = fma(ec[p], ec[p], es[p] * es[p]);
-    const double t1 = x1 * x1;
-    const double q16 = (0.25 * q[p]) * (0.25 * q[p]);
-    simple[p] = ((es[p] * es[p]) * t1 < q16) && ((e2[p] * t1) * t1 < q16);
-    xk[p] = x1;
-    rough[p] = live[p] && !simple[p];
-    any_rough = any_rough || rough[p];
-  }
-  if (__any_sync(kFullMask, any_rough)) {
-    double yy[P], sy[P], cy[P];
-#pragma unroll
-    for (int p = 0; p < P; ++p) yy[p] = dM[p] - es[p];
-    sincosm_warp<P>(rough, yy, sy, cy);
-#pragma unroll
-    for (int p = 0; p < P; ++p) {
-      const double sg = fma(es[p], 1.0 + cy[p], ec[p] * (yy[p] + sy[p]));
-      const double e = sqrt(e2[p]);
-      if (!simple[p]) xk[p] = yy[p] + (sg >= 0.0 ? 0.85 : -0.85) * e;
-    }
-  }
+    xk[p] = live[p] ? dM[p] * invq[p] : 0.0;
 
-  // Newton updates, warp-uniform exit.  After a body's last update d (|d| <= eps)
-  // its sin/cos at x − d follow from those at x by angle addition instead of a fresh evaluation.
-  bool conv[P], open[P];
-  double sm[P], cm1[P];  // sin x − x, cos x − 1 at the current xk
-#pragma unroll
-  for (int p = 0; p < P; ++p) {
-    if (!live[p]) xk[p] = 0.0;
-    conv[p] = !live[p];
+    const int e2h = hi_word(e2[p]);
+    thr[p] = e2h < kHiE2_010 ? kHiThr0 : (e2h < kHiE2_030 ? kHiThr1 : (e2h < kHiE2_050 ? kHiThr2 : kHiThr3));
+    open[p] = live[p] && fast_on && e2h < kHiE2_080 && is_small_angle(xk[p]);
+    slow[p] = live[p] && !open[p];
+    any_open = any_open || open[p];
     sm[p] = 0.0;
     cm1[p] = 0.0;
+    nonconv[p] = 0;
   }
-  for (int it = 0; it < iters; ++it) {
-    double smk[P], cmk[P];
-#pragma unroll
-    for (int p = 0; p < P; ++p) open[p] = !conv[p];
-    sincosm_warp<P>(open, xk, smk, cmk);
-    bool all_conv = true;
+
+  for (int it = 0; it < kFastMaxIters && __any_sync(kFullMask, any_open); ++it) {
+    any_open = false;
 #pragma unroll
     for (int p = 0; p < P; ++p) {
-      const double s = xk[p] + smk[p];
-      const double f = fma(-es[p], cmk[p], fma(-ec[p], s, xk[p] - dM[p]));
-      const double fp = fma(es[p], s, fma(-ec[p], cmk[p], q[p]));
-      const double d = f * rcp_f64_1(fp);
-      if (!conv[p]) {
-        conv[p] = fabs(d) <= kExitEps;
-        // sin(x − d) − (x − d), cos(x − d) − 1 to O(d^3); exact enough only once |d| <= eps
-        const double c = 1.0 + cmk[p];
-        const double hd = 0.5 * d;
-        sm[p] = fma(-d, fma(hd, s, cmk[p]), smk[p]);
-        cm1[p] = fma(d, fma(-hd, c, s), cmk[p]);
+      double smk, cmk;
+      sincosm_small(xk[p], smk, cmk);
+      const double s = xk[p] + smk;
+      const double c = 1.0 + cmk;
+      const double f = fma(-es[p], cmk, fma(-ec[p], s, xk[p] - dM[p]));
+      const double f1 = fma(es[p], s, fma(-ec[p], cmk, q[p]));
+      const double f2 = fma(ec[p], s, es[p] * c);
+      const double f3 = 1.0 - f1;
+      const double inv = rcp_f64_1(f1);
+      const double dl = f * inv;        // Newton update
+      const double h = dl * inv;
+      const double u2 = f2 * h;         // 2 a2 delta
+      const double v6 = (f3 * h) * dl;  // 6 a3 delta^2
+      const double w = fma(u2, fma(0.5, u2, 0.5), v6 * (-1.0 / 6.0));
+      const double d = fma(dl, w, dl);
+      // sin(x − d) − (x − d) and cos(x − d) − 1 from s, c at x:  sin d = d − d^3/6, cos d = 1 − d^2/2
+      const double hd = 0.5 * d;
+      const double h2 = hd * d;                  // d^2 / 2
+      const double d3 = h2 * (d * (1.0 / 3.0));  // d^3 / 6
+      const double smn = fma(c, d3, fma(-h2, s, fma(-d, cmk, smk)));
+      const double cmn = fma(-s, d3, fma(-h2, c, fma(d, s, cmk)));
+      if (open[p]) {
+        sm[p] = smn;
+        cm1[p] = cmn;
         xk[p] -= d;
+        const bool done = hi_abs(dl) < thr[p];
+        const bool lost = !done && !is_small_angle(xk[p]);  // left the polynomial's range (or NaN)
+        open[p] = !done && !lost;
+        slow[p] = slow[p] || lost;
       }
-      all_conv = all_conv && conv[p];
+      any_open = any_open || open[p];
     }
-    if (__all_sync(kFullMask, all_conv)) break;
   }
-  // bodies that ran out of updates (or iters == 0) need a fresh evaluation at the final x
-  bool any_open = false;
+  bool any_slow = false;
 #pragma unroll
   for (int p = 0; p < P; ++p) {
-    open[p] = !conv[p];
-    any_open = any_open || open[p];
+    slow[p] = slow[p] || open[p];  // no convergence in kFastMaxIters steps
+    any_slow = any_slow || slow[p];
   }
-  if (__any_sync(kFullMask, any_open)) {
-    double smk[P], cmk[P];
-    sincosm_warp<P>(open, xk, smk, cmk);
+  if (__any_sync(kFullMask, any_slow)) {
 #pragma unroll
-    for (int p = 0; p < P; ++p)
-      if (open[p]) { sm[p] = smk[p]; cm1[p] = cmk[p]; }
+    for (int p = 0; p < P; ++p) {
+      if (__any_sync(kFullMask, slow[p])) {
+        const ExactSolve o = kepler_solve_exact(slow[p], ec[p], es[p], q[p], dM[p], invq[p], e2[p], iters, tol);
+        if (slow[p]) {
+          xk[p] = o.x; sm[p] = o.sm; cm1[p] = o.cm1; nonconv[p] = o.nonconv;
+        }
+      }
+    }
   }
 #pragma unroll
   for (int p = 0; p < P; ++p) {
     const double s = xk[p] + sm[p];
-    const double rho = fma(-es[p], cm1[p], fma(-ec[p], s, xk[p] - dM[p]));  // residual of Kepler's equation
-    const bool nonconv = !(fabs(rho) <= tol);
-
     // Gauss f, g (PAPER.md:94 step 4), applied as r += (f−1) r + g v, v += fdot r + (gdot−1) v
     const double pr = fma(es[p], s, fma(-ec[p], cm1[p], q[p]));  // r(t)/a
     const double invp = rcp_f64(pr);
@@ -255,7 +362,7 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
     const double g = (dM[p] + sm[p]) * (a[p] * rsa[p]);  // (dM − x + sin x) / n
     const double fd = -(s * invp) * (sqa[p] * rinv[p]);
     const double gm1 = cm1[p] * invp;
-    if (live[p] && !nonconv) {
+    if (live[p] && !nonconv[p]) {
       const double nx = fma(fm1, x[p], fma(g, vx[p], x[p]));
       const double ny = fma(fm1, y[p], fma(g, vy[p], y[p]));
       const double nz = fma(fm1, z[p], fma(g, vz[p], z[p]));
@@ -264,7 +371,7 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
       vz[p] = fma(fd, z[p], fma(gm1, vz[p], vz[p]));
       x[p] = nx; y[p] = ny; z[p] = nz;
     }
-    st[p] = !live_in[p] ? 0 : (unbound[p] ? GLISSE_FLAG_UNBOUND : (nonconv ? GLISSE_FLAG_NONCONV : 0));
+    st[p] = !live_in[p] ? 0 : (unbound[p] ? GLISSE_FLAG_UNBOUND : (nonconv[p] ? GLISSE_FLAG_NONCONV : 0));
   }
 }
 
@@ -279,16 +386,6 @@ __device__ __forceinline__ int kepler_drift_warp(bool live, double mu, double in
   kepler_drift_warp<1>(l1, mu, inv_mu, inv_mu_dt, iters, tol, r21, x1, y1, z1, vx1, vy1, vz1, st);
   x = x1[0]; y = y1[0]; z = z1[0]; vx = vx1[0]; vy = vy1[0]; vz = vz1[0];
   return st[0];
-}
-
-// single-body sin x − x, cos x − 1 (test hook)
-__device__ __forceinline__ void sincosm_warp(bool live, double x, double& sm, double& cm1) {
-  const bool l1[1] = {live};
-  const double x1[1] = {x};
-  double s1[1], c1[1];
-  sincosm_warp<1>(l1, x1, s1, c1);
-  sm = s1[0];
-  cm1 = c1[0];
 }
 
 }  // namespace glisse

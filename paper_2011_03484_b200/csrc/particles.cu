@@ -131,35 +131,59 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
     for (int kk = 0; kk < recs; ++kk, ++k) {
       const double* rec = stage + kk * stride;
       // ---- a3/a4: force evaluation with the tests (O1/O4/O5) at time t_{step0+k} ----------------
+      // The tests compare squared distances (O5).  On the hot path they are taken on the HIGH WORDS
+      // in the integer pipe, as a superset (d2 < R2 implies hi(d2) <= hi(R2) for non-negative
+      // doubles); the exact fp64 comparisons run only in a warp where some lane passes the superset.
       double r2[P], ax[P], ay[P], az[P];
-      int hit[P];
+      bool maybe[P];
 #pragma unroll
       for (int p = 0; p < P; ++p) {
         r2[p] = fma(x[p], x[p], fma(y[p], y[p], z[p] * z[p]));
         ax[p] = rec[3 * np]; ay[p] = rec[3 * np + 1]; az[p] = rec[3 * np + 2];  // h0
-        hit[p] = 0;
+        const int r2h = __double2hiint(r2[p]);
+        maybe[p] = (r2h >= a.rmax2_hi) || (r2h <= a.rmin2_hi);
       }
 #pragma unroll
-      for (int jj = 0; jj < np; ++jj) {
-        const int j = np - 1 - jj;  // descending, so the lowest index wins (reading S11)
+      for (int j = 0; j < np; ++j) {
         const double qx = rec[3 * j], qy = rec[3 * j + 1], qz = rec[3 * j + 2];
 #pragma unroll
         for (int p = 0; p < P; ++p) {
           const double dx = x[p] - qx, dy = y[p] - qy, dz = z[p] - qz;
           const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
-          hit[p] = (d2 < a.rc2[j]) ? (GLISSE_FLAG_PLANET0 + j) : hit[p];
-          const double ri = rsqrt_f64(d2);
-          const double w = (a.gm[j] * ri) * (ri * ri);
+          maybe[p] = maybe[p] || (__double2hiint(d2) <= a.rc2_hi[j]);
+          const double w = gm_over_r3(a.gm[j], d2);
           ax[p] = fma(-w, dx, ax[p]);
           ay[p] = fma(-w, dy, ay[p]);
           az[p] = fma(-w, dz, az[p]);
         }
       }
+      int hit[P];
+      bool any_maybe = false;
+#pragma unroll
+      for (int p = 0; p < P; ++p) {
+        hit[p] = 0;
+        any_maybe = any_maybe || (maybe[p] && alive[p]);
+      }
+      if (__any_sync(kFullMask, any_maybe)) {  // rare: the exact tests, lowest planet index wins (S11)
+        for (int jj = 0; jj < np; ++jj) {
+          const int j = np - 1 - jj;
+          const double qx = rec[3 * j], qy = rec[3 * j + 1], qz = rec[3 * j + 2];
+#pragma unroll
+          for (int p = 0; p < P; ++p) {
+            const double dx = x[p] - qx, dy = y[p] - qy, dz = z[p] - qz;
+            const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
+            hit[p] = (d2 < a.rc2[j]) ? (GLISSE_FLAG_PLANET0 + j) : hit[p];
+          }
+        }
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+          hit[p] = (r2[p] > a.rmax2) ? GLISSE_FLAG_RMAX : hit[p];
+          hit[p] = (r2[p] < a.rmin2) ? GLISSE_FLAG_RMIN : hit[p];
+        }
+      }
       bool any_alive_k = false;
 #pragma unroll
       for (int p = 0; p < P; ++p) {
-        hit[p] = (r2[p] > a.rmax2) ? GLISSE_FLAG_RMAX : hit[p];
-        hit[p] = (r2[p] < a.rmin2) ? GLISSE_FLAG_RMIN : hit[p];
         if (alive[p] && hit[p] != 0) {
           flag[p] = hit[p];
           rs[p] = a.step0 + k;
