@@ -232,7 +232,7 @@ int run_compaction(glisse_sim* s) {
 int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
   LogBuffer& B = s->buf[b];
   CKS(s, cudaStreamWaitEvent(s->p, B.consumed, 0));
-  CKS(s, launch_planet_kernel(s->d_sys, jin, B.log, B.jlog, s->K, s->dt, s->p));
+  CKS(s, launch_planet_kernel(s->d_sys, s->np, jin, B.log, B.jlog, s->K, s->dt, s->p));
   s->launches += 1;
   CKS(s, cudaEventRecord(B.ready, s->p));
   B.start = start;
@@ -564,7 +564,7 @@ int glisse_planet_log(glisse_sim* s, long long n_steps, double* log) {
   cudaError_t e = dmalloc(&d_jlog, static_cast<size_t>(n_steps + 1) * 6 * np);
   if (e == cudaSuccess) e = cudaStreamWaitEvent(s->q, B.ready, 0);
   if (e == cudaSuccess)
-    e = launch_planet_kernel(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_log, d_jlog,
+    e = launch_planet_kernel(s->d_sys, s->np, B.jlog + static_cast<size_t>(off) * 6 * np, d_log, d_jlog,
                              static_cast<int>(n_steps), s->dt, s->q);
   s->launches += 1;
   if (e == cudaSuccess) e = cudaMemcpyAsync(log, d_log, count * sizeof(double), cudaMemcpyDefault, s->q);

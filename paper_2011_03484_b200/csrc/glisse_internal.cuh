@@ -10,7 +10,7 @@ namespace glisse {
 
 constexpr int kMaxPlanets = GLISSE_MAX_PLANETS;
 #ifndef GL_BLOCK
-#define GL_BLOCK 128
+#define GL_BLOCK 32
 #endif
 #ifndef GL_PPT
 #define GL_PPT 1
@@ -20,7 +20,7 @@ constexpr int kParticlesPerThread = GL_PPT;  // particles per thread (independen
 constexpr int kParticleWarps = kParticleBlock / 32;
 constexpr int kRingSlots = 2;        // planet-log stages resident in shared memory per WARP
 #ifndef GL_MIN_BLOCKS
-#define GL_MIN_BLOCKS 6
+#define GL_MIN_BLOCKS 24
 #endif
 
 // Doubles per planet-log record (include/glisse.h: glisse_log_stride).
@@ -75,8 +75,8 @@ cudaError_t configure_particle_kernels();
 
 // Planet-history kernel (a1): from the Jacobi state `jin` write nsteps+1 log records and nsteps+1
 // Jacobi state records (record 0 = the input state).
-cudaError_t launch_planet_kernel(PlanetSystem* sys, const double* jin, double* log, double* jlog, int nsteps,
-                                 double dt, cudaStream_t s);
+cudaError_t launch_planet_kernel(PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
+                                 int nsteps, double dt, cudaStream_t s);
 // heliocentric (q, qd) [np][3] -> Jacobi state record
 cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const double* qd, double* jstate,
                                cudaStream_t s);

@@ -86,8 +86,13 @@ __device__ __forceinline__ double rcp_f64_1(double a) {
 // The polynomial coefficients live in the constant bank so that every DFMA of the Horner chains takes
 // its coefficient as a c[3][..] operand: as 64-bit immediates they cost two UMOV each per use, which
 // competes with the FP64 pipe for issue slots (profiles/r01: 54 UMOV per particle-step).
+#ifdef GL_SINCOS_IMM
+constexpr double kSinCoef[6] = {GL_S0, GL_S1, GL_S2, GL_S3, GL_S4, GL_S5};
+constexpr double kCosCoef[6] = {GL_C0, GL_C1, GL_C2, GL_C3, GL_C4, GL_C5};
+#else
 static __constant__ double kSinCoef[6] = {GL_S0, GL_S1, GL_S2, GL_S3, GL_S4, GL_S5};
 static __constant__ double kCosCoef[6] = {GL_C0, GL_C1, GL_C2, GL_C3, GL_C4, GL_C5};
+#endif
 
 __device__ __forceinline__ int hi_word(double x) { return __double2hiint(x); }
 

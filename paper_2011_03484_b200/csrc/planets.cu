@@ -25,75 +25,86 @@ struct Lane {
   int np, lane;
   bool live;
   double gm0, gm, eta, eta_prev, wj;  // wj = gm/eta
+  double inv_eta, inv_eta_prev, sc;   // 1/eta_k, 1/eta_{k-1}, eta_k/eta_{k-1}
   double mu, inv_mu;
 };
 
 __device__ __forceinline__ double shfl(double v, int src) { return __shfl_sync(kFullMask, v, src); }
 
+// NP > 0: compile-time planet count, every sum over planets fully unrolled so that the np
+// independent chains (one rsqrt each) overlap: the step is serial in time and latency is all that
+// counts.  NP == 0: run-time count.
+template <int NP>
+__device__ __forceinline__ int count(const Lane& L) { return NP > 0 ? NP : L.np; }
+
 // exclusive prefix sum over lanes i < lane of c_i, added in increasing i
+template <int NP>
 __device__ __forceinline__ void prefix3(const Lane& L, double cx, double cy, double cz, double& sx, double& sy,
                                         double& sz) {
   sx = sy = sz = 0.0;
-  for (int i = 0; i + 1 < L.np; ++i) {
+  const int np = count<NP>(L);
+#pragma unroll
+  for (int i = 0; i + 1 < np; ++i) {
     const double tx = shfl(cx, i), ty = shfl(cy, i), tz = shfl(cz, i);
     if (i < L.lane) { sx += tx; sy += ty; sz += tz; }
   }
 }
 
 // q from r' (Jacobi -> heliocentric); the same linear map serves velocities
+template <int NP>
 __device__ __forceinline__ void jacobi_to_helio(const Lane& L, double rx, double ry, double rz, double& qx,
                                                 double& qy, double& qz) {
   double sx, sy, sz;
-  prefix3(L, L.wj * rx, L.wj * ry, L.wj * rz, sx, sy, sz);
+  prefix3<NP>(L, L.wj * rx, L.wj * ry, L.wj * rz, sx, sy, sz);
   qx = rx + sx; qy = ry + sy; qz = rz + sz;
 }
 
 // r' from q (heliocentric -> Jacobi)
+template <int NP>
 __device__ __forceinline__ void helio_to_jacobi(const Lane& L, double qx, double qy, double qz, double& rx,
                                                 double& ry, double& rz) {
   double sx, sy, sz;
-  prefix3(L, L.gm * qx, L.gm * qy, L.gm * qz, sx, sy, sz);
-  const double ie = 1.0 / L.eta_prev;
-  rx = qx - sx * ie; ry = qy - sy * ie; rz = qz - sz * ie;
+  prefix3<NP>(L, L.gm * qx, L.gm * qy, L.gm * qz, sx, sy, sz);
+  rx = qx - sx * L.inv_eta_prev; ry = qy - sy * L.inv_eta_prev; rz = qz - sz * L.inv_eta_prev;
 }
 
 // Jacobi acceleration of this lane's planet, and h0 (the same on every lane)
+template <int NP>
 __device__ __forceinline__ void kick_accel(const Lane& L, double qx, double qy, double qz, double rx, double ry,
                                            double rz, double& ax, double& ay, double& az, double& hx, double& hy,
                                            double& hz) {
+  const int np = count<NP>(L);
   // star term of A_i and this planet's contribution to h0
   const double q2 = fma(qx, qx, fma(qy, qy, qz * qz));
-  const double qi = rsqrt_f64(q2);
-  const double qi3 = qi * qi * qi;
+  const double qi3 = gm_over_r3(1.0, q2);
   double Ax = -(L.gm0 * qi3) * qx, Ay = -(L.gm0 * qi3) * qy, Az = -(L.gm0 * qi3) * qz;
   const double tx = (L.gm * qi3) * qx, ty = (L.gm * qi3) * qy, tz = (L.gm * qi3) * qz;
+  // the Jacobi two-body term, independent of the sums below
+  const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
+  const double w0 = gm_over_r3(L.gm0, r2);
   hx = hy = hz = 0.0;
-  for (int j = 0; j < L.np; ++j) {
+#pragma unroll
+  for (int j = 0; j < np; ++j) {
     const double gj = shfl(L.gm, j);
     const double qjx = shfl(qx, j), qjy = shfl(qy, j), qjz = shfl(qz, j);
     hx -= shfl(tx, j); hy -= shfl(ty, j); hz -= shfl(tz, j);
     const bool self = (j == L.lane);
     const double dx = qx - qjx, dy = qy - qjy, dz = qz - qjz;
     const double d2 = self ? 1.0 : fma(dx, dx, fma(dy, dy, dz * dz));
-    const double di = rsqrt_f64(d2);
-    const double w = self ? 0.0 : (gj * di) * (di * di);
+    const double w = self ? 0.0 : gm_over_r3(gj, d2);
     Ax = fma(-w, dx, Ax); Ay = fma(-w, dy, Ay); Az = fma(-w, dz, Az);
   }
   // tail_k = sum_{i>k} gm_i A_i, added in increasing i
   const double mx = L.gm * Ax, my = L.gm * Ay, mz = L.gm * Az;
   double Tx = 0.0, Ty = 0.0, Tz = 0.0;
-  for (int i = 1; i < L.np; ++i) {
+#pragma unroll
+  for (int i = 1; i < np; ++i) {
     const double ux = shfl(mx, i), uy = shfl(my, i), uz = shfl(mz, i);
     if (i > L.lane) { Tx += ux; Ty += uy; Tz += uz; }
   }
-  const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
-  const double ri = rsqrt_f64(r2);
-  const double w0 = L.gm0 * (ri * ri * ri);
-  const double ie = 1.0 / L.eta;
-  const double sc = L.eta / L.eta_prev;
-  ax = sc * (fma(w0, rx, Ax) + Tx * ie);
-  ay = sc * (fma(w0, ry, Ay) + Ty * ie);
-  az = sc * (fma(w0, rz, Az) + Tz * ie);
+  ax = L.sc * (fma(w0, rx, Ax) + Tx * L.inv_eta);
+  ay = L.sc * (fma(w0, ry, Ay) + Ty * L.inv_eta);
+  az = L.sc * (fma(w0, rz, Az) + Tz * L.inv_eta);
 }
 
 __device__ __forceinline__ Lane make_lane(const PlanetSystem* sys) {
@@ -106,6 +117,9 @@ __device__ __forceinline__ Lane make_lane(const PlanetSystem* sys) {
   L.eta = L.live ? sys->eta[L.lane] : 1.0;
   L.eta_prev = L.live ? sys->eta_prev[L.lane] : 1.0;
   L.wj = L.gm / L.eta;
+  L.inv_eta = 1.0 / L.eta;
+  L.inv_eta_prev = 1.0 / L.eta_prev;
+  L.sc = L.eta / L.eta_prev;
   L.mu = L.gm0 * L.eta / L.eta_prev;
   L.inv_mu = 1.0 / L.mu;
   return L;
@@ -127,6 +141,7 @@ __device__ __forceinline__ void write_record(const Lane& L, double* log, double*
   }
 }
 
+template <int NP>
 __global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, const double* __restrict__ jin,
                                                              double* __restrict__ log, double* __restrict__ jlog,
                                                              int nsteps, double dt) {
@@ -141,8 +156,8 @@ __global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, c
     vx = jin[3 * L.np + 3 * L.lane]; vy = jin[3 * L.np + 3 * L.lane + 1]; vz = jin[3 * L.np + 3 * L.lane + 2];
   }
   double qx, qy, qz, ax, ay, az, hx, hy, hz;
-  jacobi_to_helio(L, rx, ry, rz, qx, qy, qz);
-  kick_accel(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
+  jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
+  kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
   write_record(L, log, jlog, 0, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
   int bad = 0;
   for (int s = 0; s < nsteps; ++s) {
@@ -152,8 +167,8 @@ __global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, c
                                      rx, ry, rz, vx, vy, vz);
     const unsigned failed = __ballot_sync(kFullMask, st != 0);
     if (failed && !bad) bad = __ffs(failed);
-    jacobi_to_helio(L, rx, ry, rz, qx, qy, qz);
-    kick_accel(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
+    jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
+    kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
     if (L.live) { vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz); }
     write_record(L, log, jlog, s + 1, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
   }
@@ -169,8 +184,8 @@ __global__ void __launch_bounds__(32) planet_init_kernel(const PlanetSystem* sys
     wx = qd[3 * L.lane]; wy = qd[3 * L.lane + 1]; wz = qd[3 * L.lane + 2];
   }
   double rx, ry, rz, vx, vy, vz;
-  helio_to_jacobi(L, qx, qy, qz, rx, ry, rz);
-  helio_to_jacobi(L, wx, wy, wz, vx, vy, vz);
+  helio_to_jacobi<0>(L, qx, qy, qz, rx, ry, rz);
+  helio_to_jacobi<0>(L, wx, wy, wz, vx, vy, vz);
   if (L.live) {
     jstate[3 * L.lane] = rx; jstate[3 * L.lane + 1] = ry; jstate[3 * L.lane + 2] = rz;
     jstate[3 * L.np + 3 * L.lane] = vx; jstate[3 * L.np + 3 * L.lane + 1] = vy;
@@ -188,8 +203,8 @@ __global__ void __launch_bounds__(32) planet_read_kernel(const PlanetSystem* sys
     vz = jstate[3 * L.np + 3 * L.lane + 2];
   }
   double qx, qy, qz, wx, wy, wz;
-  jacobi_to_helio(L, rx, ry, rz, qx, qy, qz);
-  jacobi_to_helio(L, vx, vy, vz, wx, wy, wz);
+  jacobi_to_helio<0>(L, rx, ry, rz, qx, qy, qz);
+  jacobi_to_helio<0>(L, vx, vy, vz, wx, wy, wz);
   if (L.live) {
     if (q) { q[3 * L.lane] = qx; q[3 * L.lane + 1] = qy; q[3 * L.lane + 2] = qz; }
     if (qd) { qd[3 * L.lane] = wx; qd[3 * L.lane + 1] = wy; qd[3 * L.lane + 2] = wz; }
@@ -198,9 +213,13 @@ __global__ void __launch_bounds__(32) planet_read_kernel(const PlanetSystem* sys
 
 }  // namespace
 
-cudaError_t launch_planet_kernel(PlanetSystem* sys, const double* jin, double* log, double* jlog, int nsteps,
-                                 double dt, cudaStream_t s) {
-  planet_history_kernel<<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt);
+cudaError_t launch_planet_kernel(PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
+                                 int nsteps, double dt, cudaStream_t s) {
+  switch (np) {
+    case 4: planet_history_kernel<4><<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt); break;
+    case 8: planet_history_kernel<8><<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt); break;
+    default: planet_history_kernel<0><<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt); break;
+  }
   return cudaGetLastError();
 }
 
