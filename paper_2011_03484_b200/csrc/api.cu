@@ -42,6 +42,7 @@ struct glisse_sim {
   glisse_params prm{};
   int K = 1024;
   int stride = 0;
+  int planet_smem = 0;  // dynamic shared memory the planet-history kernel asks for (one SM to itself)
   int status = GLISSE_OK;  // sticky
 
   PlanetSystem* d_sys = nullptr;
@@ -232,7 +233,7 @@ int run_compaction(glisse_sim* s) {
 int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
   LogBuffer& B = s->buf[b];
   CKS(s, cudaStreamWaitEvent(s->p, B.consumed, 0));
-  CKS(s, launch_planet_kernel(s->d_sys, s->np, jin, B.log, B.jlog, s->K, s->dt, s->p));
+  CKS(s, launch_planet_kernel(s->d_sys, s->np, jin, B.log, B.jlog, s->K, s->dt, s->planet_smem, s->p));
   s->launches += 1;
   CKS(s, cudaEventRecord(B.ready, s->p));
   B.start = start;
@@ -356,6 +357,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   }
   CKF(cudaStreamCreateWithFlags(&s->p, cudaStreamNonBlocking));
   CKF(configure_particle_kernels());
+  CKF(configure_planet_kernels(&s->planet_smem));
 
   // ---- allocations: one device arena, carved at 256-byte boundaries ------------------------------
   {
@@ -497,25 +499,26 @@ int glisse_advance(glisse_sim* s, long long n_steps) {
   CKS(s, cudaSetDevice(s->device));
   const int np = s->np;
   while (n_steps > 0) {
-    long long off = s->step - s->buf[s->cur].start;
-    if (off == s->K) {
-      // this buffer is used up: hand it back to the planet stream, which refills it with the chunk
-      // after the next one while the particles work through the next one
-      const int old = s->cur;
-      CKS(s, cudaEventRecord(s->buf[old].consumed, s->q));
-      s->cur ^= 1;
-      const LogBuffer& nxt = s->buf[s->cur];
-      const int st = fill_log_buffer(s, old, nxt.jlog + static_cast<size_t>(s->K) * 6 * np, nxt.start + s->K);
-      if (st != GLISSE_OK) return st;
-      off = 0;
-    }
     const LogBuffer& B = s->buf[s->cur];
+    const long long off = s->step - B.start;  // 0 <= off < K: an exhausted buffer is handed back at once
     CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
     const int m = static_cast<int>(std::min<long long>(n_steps, s->K - off));
     const int st = launch_particles(s, B.log + static_cast<size_t>(off) * s->stride, m);
     if (st != GLISSE_OK) return st;
     s->step += m;
     n_steps -= m;
+    if (off + m == s->K) {
+      // this buffer is used up: hand it back to the planet stream, which refills it with the chunk
+      // after the next one while the particles work through the next one.  Done BEFORE the compaction
+      // is queued, so that the planet-history block (which takes an SM to itself, planets.cu) is
+      // resident before the next particle kernel fills the device.
+      const int old = s->cur;
+      CKS(s, cudaEventRecord(s->buf[old].consumed, s->q));
+      s->cur ^= 1;
+      const LogBuffer& nxt = s->buf[s->cur];
+      const int sf = fill_log_buffer(s, old, nxt.jlog + static_cast<size_t>(s->K) * 6 * np, nxt.start + s->K);
+      if (sf != GLISSE_OK) return sf;
+    }
     if (s->prm.resync_chunks > 0 && ++s->chunks_since_resync >= s->prm.resync_chunks) {
       const int sc = run_compaction(s);
       if (sc != GLISSE_OK) return sc;
@@ -565,7 +568,7 @@ int glisse_planet_log(glisse_sim* s, long long n_steps, double* log) {
   if (e == cudaSuccess) e = cudaStreamWaitEvent(s->q, B.ready, 0);
   if (e == cudaSuccess)
     e = launch_planet_kernel(s->d_sys, s->np, B.jlog + static_cast<size_t>(off) * 6 * np, d_log, d_jlog,
-                             static_cast<int>(n_steps), s->dt, s->q);
+                             static_cast<int>(n_steps), s->dt, 0, s->q);
   s->launches += 1;
   if (e == cudaSuccess) e = cudaMemcpyAsync(log, d_log, count * sizeof(double), cudaMemcpyDefault, s->q);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->q);

@@ -74,9 +74,12 @@ cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_slots_upper, cud
 cudaError_t configure_particle_kernels();
 
 // Planet-history kernel (a1): from the Jacobi state `jin` write nsteps+1 log records and nsteps+1
-// Jacobi state records (record 0 = the input state).
+// Jacobi state records (record 0 = the input state).  exclusive_sm_bytes > 0: dynamic
+// shared memory to request (unused) so that no other block fits on its SM.
 cudaError_t launch_planet_kernel(PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
-                                 int nsteps, double dt, cudaStream_t s);
+                                 int nsteps, double dt, int exclusive_sm_bytes, cudaStream_t s);
+// allows the planet-history kernel the whole shared memory of an SM; returns that size in bytes
+cudaError_t configure_planet_kernels(int* exclusive_sm_bytes);
 // heliocentric (q, qd) [np][3] -> Jacobi state record
 cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const double* qd, double* jstate,
                                cudaStream_t s);

@@ -214,13 +214,30 @@ __global__ void __launch_bounds__(32) planet_read_kernel(const PlanetSystem* sys
 }  // namespace
 
 cudaError_t launch_planet_kernel(PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
-                                 int nsteps, double dt, cudaStream_t s) {
+                                 int nsteps, double dt, int exclusive_sm_bytes, cudaStream_t s) {
+  // The kernel is one warp whose K steps are serial: all that counts is its latency, and sharing an
+  // SM with ~25 particle warps that saturate the FP64 pipe doubles it.  It therefore asks for the
+  // whole shared memory of an SM (unused), which keeps every other block off that SM: 1/148 of the
+  // device for the ~1.4 ms it runs per chunk.
+  const size_t smem = exclusive_sm_bytes > 0 ? static_cast<size_t>(exclusive_sm_bytes) : 0;
   switch (np) {
-    case 4: planet_history_kernel<4><<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt); break;
-    case 8: planet_history_kernel<8><<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt); break;
-    default: planet_history_kernel<0><<<1, 32, 0, s>>>(sys, jin, log, jlog, nsteps, dt); break;
+    case 4: planet_history_kernel<4><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt); break;
+    case 8: planet_history_kernel<8><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt); break;
+    default: planet_history_kernel<0><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt); break;
   }
   return cudaGetLastError();
+}
+
+cudaError_t configure_planet_kernels(int* exclusive_sm_bytes) {
+  int dev = 0, optin = 0;
+  cudaError_t e;
+  if ((e = cudaGetDevice(&dev))) return e;
+  if ((e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev))) return e;
+  if ((e = cudaFuncSetAttribute(planet_history_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin))) return e;
+  if ((e = cudaFuncSetAttribute(planet_history_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin))) return e;
+  if ((e = cudaFuncSetAttribute(planet_history_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin))) return e;
+  *exclusive_sm_bytes = optin;
+  return cudaSuccess;
 }
 
 cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const double* qd, double* jstate,
