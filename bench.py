@@ -14,8 +14,10 @@ value   = particle-steps actually integrated (sum over steps of the active count
           resident in HBM, device time from CUDA events on the launching stream, max over ranks.
 e2e     = the same metric through the C ABI with HOST buffers: every step does glisse_create (H2D of
           the particle state from pinned memory), glisse_advance(1,024), glisse_read (D2H), destroy.
-roofline= FP64-ALU bound: counted flops per particle-step x particle-steps per launch / mean
-          particle-kernel duration, against the FP64 FMA rate measured by the library's probe.
+roofline= FP64-ALU bound: algorithmic flops per particle-step (410 at N_p = 4) x
+          particle-steps per launch / mean particle-kernel duration, against the nominal FP64 FMA
+          rate (148 SMs x 64 lanes x 2 x 1.965 GHz); the flops the kernel actually executes (ncu
+          counters) and the library's measured DFMA probe are reported beside it.
 --impl reference times the oracle (oracle/, plain single-threaded C++) on a bounded sample.
 """
 from __future__ import annotations
@@ -43,20 +45,23 @@ L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
 # captures under profiles/ (the kernel is ALU-bound; this only shows that state traffic is negligible)
 TRAFFIC_BYTES_PER_LAUNCH = {"c2": 6.7e6, "1m_x4": 5.3e7}
 
-# Counted fp64 flops per particle-step of the particle kernel (DFMA = 2, DADD/DMUL = 1, compares,
-# MUFU seeds and integer work = 0): the ncu instruction counters of the current kernel
-# (profiles/*_particle_kernel_*.md, "Derived per launch") divided by the thread-steps of the launch;
-# DESIGN.md §7 states the derivation.  N_p = 4 is measured; other N_p add 25 flops per planet (the
-# kick's per-planet instruction count).
-FLOPS_PER_PSTEP_NP4 = 328.0
+# ALGORITHMIC fp64 flops per particle-step (DFMA = 2, DADD/DMUL = 1; compares, MUFU seeds and
+# integer work = 0): SURVEY.md §8(d)'s figure for the method as the paper defines it with the two
+# Newton updates its convergence needs on these workloads — ~410 at N_p = 4, +25 per further planet
+# (DESIGN.md §7 restates the count).  The roofline's `achieved` uses this figure.
+ALGO_FLOPS_NP4 = 410.0
+# EXECUTED flops per particle-step of the current particle kernel, from its ncu instruction counters
+# (profiles/*_particle_kernel_*.md, "Derived per launch"): the quartic solver and the merged
+# gm/d^3 do the same step in fewer operations.  Reported beside the algorithmic figure.
+EXEC_FLOPS_NP4 = 282.0
 FLOPS_PER_PLANET = 25.0
 # FP64 peak: ncu reports sm__sass_thread_inst_executed_op_dfma_pred_on.sum.peak_sustained = 64 per SM
 # per cycle; x 148 SMs x 2 flops x 1.965 GHz (clocks.max.sm of B200_PROFILING.md)
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
 
-def flops_per_pstep(n_planets: int) -> float:
-    return FLOPS_PER_PSTEP_NP4 + FLOPS_PER_PLANET * (n_planets - 4)
+def flops_per_pstep(n_planets: int, executed: bool = False) -> float:
+    return (EXEC_FLOPS_NP4 if executed else ALGO_FLOPS_NP4) + FLOPS_PER_PLANET * (n_planets - 4)
 
 WORKLOADS = {
     "c2": ("BASELINE.json configs[1]: 4 giants, 131,072 particles a~U[20,28], dt=180 d, K=1024", lambda n: inputs.config(2, n)),
@@ -313,6 +318,10 @@ def main():
                 "kernel": "particle_kernel", "kernel_ms_per_launch": k_ms,
                 "kernel_share_of_step": res["kernel_ms"] / res["ms"],
                 "flops_per_particle_step": fl,
+                "flops_source": "algorithmic: SURVEY.md 8(d) / DESIGN.md 7 count of the defined step with 2 Newton updates",
+                "executed_flops_per_particle_step": flops_per_pstep(w.n_planets, executed=True),
+                "executed_tflops": achieved * flops_per_pstep(w.n_planets, executed=True) / fl,
+                "executed_frac": achieved * flops_per_pstep(w.n_planets, executed=True) / fl / FP64_NOMINAL_TFLOPS,
                 "peak_source": "nominal FP64 FMA rate: 148 SMs x 64 DFMA lanes (ncu peak_sustained) x 2 x "
                                "1.965 GHz; MEASURED_PEAKS.json has no FP64 figure",
                 "probe_tflops": peak / 1e12, "frac_of_probe": achieved / (peak / 1e12),
@@ -352,6 +361,7 @@ def main():
                 line["target_1m_x4"] = {"value": rt["psteps"] / (rt["ms"] * 1e-3), "unit": UNIT,
                                         "ms_per_step": rt["ms"] / max(3, args.steps // 4),
                                         "roofline_frac": at / FP64_NOMINAL_TFLOPS, "achieved_tflops": at,
+                                        "executed_frac": at * EXEC_FLOPS_NP4 / ALGO_FLOPS_NP4 / FP64_NOMINAL_TFLOPS,
                                         "frac_of_probe": at / (peak / 1e12),
                                         "workload": WORKLOADS["1m_x4"][0]}
             rate, secs, ps = oracle_rate(w, 16384, 3000)
