@@ -50,6 +50,7 @@ struct glisse_sim {
   double* d_ptmp = nullptr;  // [6 Np] scratch: heliocentric planet state in / out
   LogBuffer buf[2];
   int cur = 0;
+  bool ahead = false;  // buf[cur ^ 1] holds (or is being filled with) the chunk after buf[cur]'s
   long long step = 0;
   bool external_log_used = false;
 
@@ -240,9 +241,11 @@ int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
   return GLISSE_OK;
 }
 
+// Waits for everything the caller has asked for.  The planet stream may still be working on a chunk
+// AHEAD of the particles: that is not waited for (every chunk the particles have used is complete,
+// the particle kernel waited for it), and a planet failure in it is reported once it is used.
 int sync_all(glisse_sim* s) {
   CKS(s, cudaStreamSynchronize(s->q));
-  CKS(s, cudaStreamSynchronize(s->p));
   if (s->nslots_pending) {
     s->nslots_upper = *s->h_nslots;
     s->nslots_pending = false;
@@ -421,9 +424,8 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     s->launches += 1;
   }
   CKF(cudaStreamSynchronize(s->p));  // the caller's planet arrays and `hs` are consumed
-  // chunk 0 into buffer 0, chunk 1 into buffer 1 (one chunk ahead from the start)
-  if (fill_log_buffer(s, 0, s->d_j0, 0) != GLISSE_OK ||
-      fill_log_buffer(s, 1, s->buf[0].jlog + static_cast<size_t>(s->K) * 6 * np, s->K) != GLISSE_OK) {
+  // chunk 0 into buffer 0; the chunk after it is started by the first advance (s->ahead)
+  if (fill_log_buffer(s, 0, s->d_j0, 0) != GLISSE_OK) {
     const int st = s->status;
     free_sim(s);
     return st;
@@ -500,24 +502,27 @@ int glisse_advance(glisse_sim* s, long long n_steps) {
   const int np = s->np;
   while (n_steps > 0) {
     const LogBuffer& B = s->buf[s->cur];
-    const long long off = s->step - B.start;  // 0 <= off < K: an exhausted buffer is handed back at once
+    const long long off = s->step - B.start;  // 0 <= off < K: an exhausted buffer is left at once
+    if (!s->ahead) {
+      // the planet stream works one chunk ahead: the other buffer gets the chunk after this one
+      // while the particles work through this one.  Queued BEFORE the particle kernel so that the
+      // planet-history block (which takes an SM to itself, planets.cu) is resident before the
+      // particles fill the device, and only when particles are about to be advanced: a caller that
+      // stops here never pays for a chunk it does not use.
+      const int sf = fill_log_buffer(s, s->cur ^ 1, B.jlog + static_cast<size_t>(s->K) * 6 * np, B.start + s->K);
+      if (sf != GLISSE_OK) return sf;
+      s->ahead = true;
+    }
     CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
     const int m = static_cast<int>(std::min<long long>(n_steps, s->K - off));
     const int st = launch_particles(s, B.log + static_cast<size_t>(off) * s->stride, m);
     if (st != GLISSE_OK) return st;
     s->step += m;
     n_steps -= m;
-    if (off + m == s->K) {
-      // this buffer is used up: hand it back to the planet stream, which refills it with the chunk
-      // after the next one while the particles work through the next one.  Done BEFORE the compaction
-      // is queued, so that the planet-history block (which takes an SM to itself, planets.cu) is
-      // resident before the next particle kernel fills the device.
-      const int old = s->cur;
-      CKS(s, cudaEventRecord(s->buf[old].consumed, s->q));
+    if (off + m == s->K) {  // this buffer is used up: the planet stream may overwrite it
+      CKS(s, cudaEventRecord(s->buf[s->cur].consumed, s->q));
       s->cur ^= 1;
-      const LogBuffer& nxt = s->buf[s->cur];
-      const int sf = fill_log_buffer(s, old, nxt.jlog + static_cast<size_t>(s->K) * 6 * np, nxt.start + s->K);
-      if (sf != GLISSE_OK) return sf;
+      s->ahead = false;
     }
     if (s->prm.resync_chunks > 0 && ++s->chunks_since_resync >= s->prm.resync_chunks) {
       const int sc = run_compaction(s);
