@@ -8,6 +8,7 @@
 #include <cstddef>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -28,6 +29,59 @@ struct LogBuffer {
 struct TimedLaunch {
   cudaEvent_t t0, t1;
 };
+
+// Device memory of a sim comes from one stream-ordered pool per device that keeps up to 1 GiB of
+// freed memory cached: a create/destroy cycle then costs microseconds instead of the ~1 ms of a
+// cudaMalloc/cudaFree pair (which also synchronise the device).
+std::mutex g_mu;
+cudaMemPool_t g_pool[64] = {};
+
+cudaError_t arena_pool(int dev, cudaMemPool_t* out) {
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_mu);
+  if (!g_pool[dev]) {
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaError_t e = cudaMemPoolCreate(&g_pool[dev], &props);
+    if (e != cudaSuccess) return e;
+    unsigned long long keep = 1ull << 30;
+    e = cudaMemPoolSetAttribute(g_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+    if (e != cudaSuccess) return e;
+  }
+  *out = g_pool[dev];
+  return cudaSuccess;
+}
+
+// The pinned word through which a sim's survivor count comes back: handed out from one pinned page
+// per process (cudaMallocHost/cudaFreeHost per sim cost ~0.2 ms).
+constexpr int kPinnedWords = 1024;
+int* g_pinned = nullptr;
+std::vector<int> g_pinned_free;
+
+int* pinned_word() {
+  std::lock_guard<std::mutex> lock(g_mu);
+  if (!g_pinned) {
+    if (cudaMallocHost(reinterpret_cast<void**>(&g_pinned), kPinnedWords * sizeof(int)) != cudaSuccess) {
+      (void)cudaGetLastError();
+      g_pinned = nullptr;
+      return nullptr;
+    }
+    for (int i = kPinnedWords - 1; i >= 0; --i) g_pinned_free.push_back(i);
+  }
+  if (g_pinned_free.empty()) return nullptr;
+  const int i = g_pinned_free.back();
+  g_pinned_free.pop_back();
+  return g_pinned + i;
+}
+
+void release_pinned_word(int* w) {
+  if (!w) return;
+  std::lock_guard<std::mutex> lock(g_mu);
+  g_pinned_free.push_back(static_cast<int>(w - g_pinned));
+}
 
 }  // namespace
 
@@ -116,15 +170,6 @@ bool all_finite_host(const double* p, long long n) {
   return true;
 }
 
-bool is_device_pointer(const void* p) {
-  cudaPointerAttributes at{};
-  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
-    (void)cudaGetLastError();
-    return false;
-  }
-  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
-}
-
 void free_sim(glisse_sim* s) {
   if (!s) return;
   cudaSetDevice(s->device);
@@ -134,8 +179,12 @@ void free_sim(glisse_sim* s) {
     if (s->buf[b].ready) cudaEventDestroy(s->buf[b].ready);
     if (s->buf[b].consumed) cudaEventDestroy(s->buf[b].consumed);
   }
-  cudaFree(s->arena);
-  if (s->h_nslots) cudaFreeHost(s->h_nslots);
+  if (s->arena) {
+    cudaStream_t fs = s->q ? s->q : s->p;
+    if (!fs || cudaFreeAsync(s->arena, fs) != cudaSuccess) cudaFree(s->arena);
+    if (fs) cudaStreamSynchronize(fs);
+  }
+  release_pinned_word(s->h_nslots);
   if (s->nslots_ready) cudaEventDestroy(s->nslots_ready);
   for (auto& t : s->timed_free) { cudaEventDestroy(t.t0); cudaEventDestroy(t.t1); }
   for (auto& t : s->timed_busy) { cudaEventDestroy(t.t0); cudaEventDestroy(t.t1); }
@@ -358,7 +407,14 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     CKF(cudaStreamCreateWithFlags(&s->q, cudaStreamNonBlocking));
     s->own_q = true;
   }
-  CKF(cudaStreamCreateWithFlags(&s->p, cudaStreamNonBlocking));
+  {
+    // the planet stream at the highest priority: when a planet-history block and the blocks of a
+    // particle kernel become runnable together, the planet block (one warp, on the critical path
+    // of the NEXT chunk, and needing an SM to itself) must be placed first
+    int least = 0, greatest = 0;
+    CKF(cudaDeviceGetStreamPriorityRange(&least, &greatest));
+    CKF(cudaStreamCreateWithPriority(&s->p, cudaStreamNonBlocking, greatest));
+  }
   CKF(configure_particle_kernels());
   CKF(configure_planet_kernels(&s->planet_smem));
 
@@ -388,7 +444,16 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     need(&s->d_ptmp, static_cast<size_t>(6 * np));
     size_t total = 0;
     for (auto& r : reqs) total += (r.bytes + 255) & ~static_cast<size_t>(255);
-    CKF(cudaMalloc(&s->arena, total));
+    cudaMemPool_t pool = nullptr;
+    CKF(arena_pool(s->device, &pool));
+    CKF(cudaMallocFromPoolAsync(&s->arena, total, pool, s->q));
+    // stream-ordered memory: the planet stream may touch it only after the allocation on q
+    cudaEvent_t born = nullptr;
+    CKF(cudaEventCreateWithFlags(&born, cudaEventDisableTiming));
+    cudaError_t eb = cudaEventRecord(born, s->q);
+    if (eb == cudaSuccess) eb = cudaStreamWaitEvent(s->p, born, 0);
+    cudaEventDestroy(born);
+    CKF(eb);
     size_t off = 0;
     for (auto& r : reqs) {
       *r.p = static_cast<char*>(s->arena) + off;
@@ -399,7 +464,11 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     CKF(cudaEventCreateWithFlags(&s->buf[b].ready, cudaEventDisableTiming));
     CKF(cudaEventCreateWithFlags(&s->buf[b].consumed, cudaEventDisableTiming));
   }
-  CKF(cudaMallocHost(reinterpret_cast<void**>(&s->h_nslots), sizeof(int)));
+  s->h_nslots = pinned_word();
+  if (!s->h_nslots) {
+    free_sim(s);
+    return GLISSE_ENOMEM;
+  }
   CKF(cudaEventCreateWithFlags(&s->nslots_ready, cudaEventDisableTiming));
 
   // ---- planet system ----------------------------------------------------------------------------
@@ -432,19 +501,14 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   }
 
   // ---- particle state ---------------------------------------------------------------------------
-  const bool dev_in = is_device_pointer(pos[0]);
+  // (finiteness is checked on the device after the upload, for host and device inputs alike: a
+  // host loop over 6 N doubles costs more than the whole upload)
   for (int k = 0; k < 3; ++k) {
-    if (!dev_in) {
-      if (!all_finite_host(pos[k], N) || !all_finite_host(vel[k], N)) {
-        free_sim(s);
-        return GLISSE_EINVAL;
-      }
-    }
     CKF(cudaMemcpyAsync(s->work[0][k], pos[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
     CKF(cudaMemcpyAsync(s->work[0][3 + k], vel[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
   }
   CKF(cudaMemsetAsync(s->d_counters, 0, 2 * sizeof(unsigned long long), s->q));
-  if (dev_in) {
+  {
     for (int k = 0; k < 6; ++k) {
       CKF(launch_count_nonfinite(s->work[0][k], N, s->d_counters + 1, s->q));
       s->launches += 1;
