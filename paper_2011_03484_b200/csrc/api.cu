@@ -22,6 +22,7 @@ struct LogBuffer {
   double* log = nullptr;    // [(K+1) * stride]
   double* jlog = nullptr;   // [(K+1) * 6 Np]   Jacobi state of the planets at every record
   long long start = 0;      // step index of record 0
+  int len = 0;              // steps it holds (records 0..len); K except while ramping up
   cudaEvent_t ready = nullptr;     // planet-history kernel that fills it has finished   (stream P)
   cudaEvent_t consumed = nullptr;  // last particle kernel that reads it has finished    (stream Q)
 };
@@ -279,11 +280,23 @@ int run_compaction(glisse_sim* s) {
   return GLISSE_OK;
 }
 
+// Steps in the log buffer that starts at step `start`.  The first chunk is cut into pieces of 64, 64,
+// 128, 256, ... steps (summing to K): the planet-history kernel is serial in time, so a full first
+// chunk would keep the particles waiting for K x 1.3 us before their first step; after the ramp
+// the planets stay one buffer ahead.  Results do not depend on the cut.
+int buffer_len(const glisse_sim* s, long long start) {
+  const int K = s->K;
+  if (K < 256 || start >= K) return K;
+  if (start == 0) return 64;
+  return static_cast<int>(std::min<long long>(start, K - start));
+}
+
 // planet-history kernel into buffer b, starting from the Jacobi state `jin` at step `start`
 int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
   LogBuffer& B = s->buf[b];
   CKS(s, cudaStreamWaitEvent(s->p, B.consumed, 0));
-  CKS(s, launch_planet_kernel(s->d_sys, s->np, jin, B.log, B.jlog, s->K, s->dt, s->planet_smem, s->p));
+  CKS(s, launch_planet_kernel(s->d_sys, s->np, jin, B.log, B.jlog, buffer_len(s, start), s->dt, s->planet_smem, s->p));
+  B.len = buffer_len(s, start);
   s->launches += 1;
   CKS(s, cudaEventRecord(B.ready, s->p));
   B.start = start;
@@ -566,24 +579,24 @@ int glisse_advance(glisse_sim* s, long long n_steps) {
   const int np = s->np;
   while (n_steps > 0) {
     const LogBuffer& B = s->buf[s->cur];
-    const long long off = s->step - B.start;  // 0 <= off < K: an exhausted buffer is left at once
+    const long long off = s->step - B.start;  // 0 <= off < B.len: an exhausted buffer is left at once
     if (!s->ahead) {
       // the planet stream works one chunk ahead: the other buffer gets the chunk after this one
       // while the particles work through this one.  Queued BEFORE the particle kernel so that the
       // planet-history block (which takes an SM to itself, planets.cu) is resident before the
       // particles fill the device, and only when particles are about to be advanced: a caller that
       // stops here never pays for a chunk it does not use.
-      const int sf = fill_log_buffer(s, s->cur ^ 1, B.jlog + static_cast<size_t>(s->K) * 6 * np, B.start + s->K);
+      const int sf = fill_log_buffer(s, s->cur ^ 1, B.jlog + static_cast<size_t>(B.len) * 6 * np, B.start + B.len);
       if (sf != GLISSE_OK) return sf;
       s->ahead = true;
     }
     CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
-    const int m = static_cast<int>(std::min<long long>(n_steps, s->K - off));
+    const int m = static_cast<int>(std::min<long long>(n_steps, B.len - off));
     const int st = launch_particles(s, B.log + static_cast<size_t>(off) * s->stride, m);
     if (st != GLISSE_OK) return st;
     s->step += m;
     n_steps -= m;
-    if (off + m == s->K) {  // this buffer is used up: the planet stream may overwrite it
+    if (off + m == B.len) {  // this buffer is used up: the planet stream may overwrite it
       CKS(s, cudaEventRecord(s->buf[s->cur].consumed, s->q));
       s->cur ^= 1;
       s->ahead = false;
