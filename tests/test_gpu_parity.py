@@ -310,6 +310,12 @@ def test_bit_exact_under_chunking_splitting_and_compaction(gl):
                       (dict(chunk_steps=7, resync_chunks=3), [700]),
                       (dict(chunk_steps=64, resync_chunks=1), [1, 0, 63, 64, 65, 507]),
                       (dict(chunk_steps=1024, resync_chunks=1), [350, 350]),
+                      # the first chunk is cut into a 64, 64, 128, 256, ... ramp (api.cu buffer_len):
+                      # advance calls that end on, just before and just after the ramp's joints
+                      (dict(chunk_steps=1024, resync_chunks=2), [64, 64, 128, 256, 188]),
+                      (dict(chunk_steps=1024, resync_chunks=1), [63, 2, 62, 130, 443]),
+                      (dict(chunk_steps=256, resync_chunks=1), [700]),
+                      (dict(chunk_steps=300, resync_chunks=0), [1, 299, 301, 99]),
                       (dict(chunk_steps=100, resync_chunks=0), [699, 1])]:
         out, ps, pl = _run_gpu(gl, w, sched, **kw)
         for a, b in zip(out, ref):
