@@ -65,6 +65,8 @@ def lib():
         L.oracle_log_stride.argtypes = [c_int]
         L.oracle_log_stride.restype = c_int
         L.oracle_default_params.argtypes = [POINTER(_Params)]
+        L.oracle_elements.argtypes = [c_double, c_void_p, c_void_p, c_void_p]
+        L.oracle_elements.restype = None
         L.oracle_kepler_drift.argtypes = [c_double, c_void_p, c_void_p, c_double, c_int, c_double]
         L.oracle_kepler_drift.restype = c_int
         L.oracle_planet_kick_accel.argtypes = [c_int, c_double, c_void_p, c_void_p, c_void_p]
@@ -183,6 +185,17 @@ class OracleSim:
 
 
 # ---- single-function entry points for the pins -------------------------------------------------
+
+def elements(mu, pos, vel):
+    """Osculating elements (a, e, i, Omega, omega, M) of each column of pos, vel ([3, N]) -> [6, N]."""
+    L = lib()
+    pos = np.ascontiguousarray(np.asarray(pos, dtype=np.float64).T)
+    vel = np.ascontiguousarray(np.asarray(vel, dtype=np.float64).T)
+    out = np.empty((pos.shape[0], 6))
+    for k in range(pos.shape[0]):
+        L.oracle_elements(c_double(mu), _p(pos[k]), _p(vel[k]), _p(out[k]))
+    return np.ascontiguousarray(out.T)
+
 
 def kepler_drift(mu, r, v, dt, iters=5, tol=1e-14):
     """O2 on one body. Returns (flag, r_new, v_new)."""

@@ -498,4 +498,57 @@ int oracle_particle_accel(int np, const double* gm, const double* q, const doubl
   return particle_accel(np, gm, q, h0, rc2.data(), P, r, a);
 }
 
+/* Osculating heliocentric elements (a, e, i, Omega, omega, M) of a massless body from (r, v): the
+ * quantities the paper logs ("logged orbital elements at a 2048-year interval", PAPER.md:268;
+ * periodic output).  Textbook definition (Murray & Dermott, Solar System Dynamics,
+ * §2.8): h = r x v, a from the vis-viva integral, the eccentricity vector
+ * evec = (v x h)/mu − r/|r|, tan i = |h_xy|/h_z, node vector n = z x h = (−h_y, h_x, 0),
+ * Omega = atan2(n_y, n_x), omega = angle from n to evec measured in the orbital plane about h,
+ * e cos E = 1 − |r|/a, e sin E = r.v / sqrt(mu a), M = E − e sin E.  Conventions where an angle is
+ * undefined: i = 0 (n = 0): Omega = 0 and omega = atan2(evec_y, evec_x); e = 0: omega = 0 and M is
+ * the angle from n (or from x when i = 0) to r; unbound (1/a <= 0): M = NaN.  Angles in [0, 2 pi). */
+void oracle_elements(double mu, const double* r, const double* v, double* out) {
+  const double two_pi = 2.0 * M_PI;
+  const double R = std::sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+  const double V2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+  const double rv = r[0] * v[0] + r[1] * v[1] + r[2] * v[2];
+  const double h[3] = {r[1] * v[2] - r[2] * v[1], r[2] * v[0] - r[0] * v[2], r[0] * v[1] - r[1] * v[0]};
+  const double H = std::sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+  const double inv_a = 2.0 / R - V2 / mu;
+  const double a = 1.0 / inv_a;
+  const double ev[3] = {(v[1] * h[2] - v[2] * h[1]) / mu - r[0] / R, (v[2] * h[0] - v[0] * h[2]) / mu - r[1] / R,
+                        (v[0] * h[1] - v[1] * h[0]) / mu - r[2] / R};
+  const double e = std::sqrt(ev[0] * ev[0] + ev[1] * ev[1] + ev[2] * ev[2]);
+  const double n[2] = {-h[1], h[0]};
+  const double N = std::sqrt(n[0] * n[0] + n[1] * n[1]);
+  const double inc = std::atan2(N, h[2]);  /* tan i = |h_xy| / h_z: acos(h_z/|h|) has no digits left near i = 0 */
+  auto wrap = [&](double x) { x = std::fmod(x, two_pi); return x < 0.0 ? x + two_pi : x; };
+  /* angle of a vector w in the orbital plane, measured from the node (or from x when i = 0) about h:
+   * components along nhat and along hhat x nhat */
+  auto in_plane_angle = [&](const double* w) {
+    if (N == 0.0) return std::atan2(h[2] >= 0.0 ? w[1] : -w[1], w[0]);
+    const double nh[3] = {n[0] / N, n[1] / N, 0.0};
+    const double hh[3] = {h[0] / H, h[1] / H, h[2] / H};
+    const double m[3] = {hh[1] * nh[2] - hh[2] * nh[1], hh[2] * nh[0] - hh[0] * nh[2], hh[0] * nh[1] - hh[1] * nh[0]};
+    return std::atan2(w[0] * m[0] + w[1] * m[1] + w[2] * m[2], w[0] * nh[0] + w[1] * nh[1] + w[2] * nh[2]);
+  };
+  const double Omega = (N == 0.0) ? 0.0 : wrap(std::atan2(n[1], n[0]));
+  double omega, M;
+  if (e == 0.0) {
+    omega = 0.0;
+    M = wrap(in_plane_angle(r));
+  } else {
+    omega = wrap(in_plane_angle(ev));
+    if (inv_a > 0.0) {
+      const double ecosE = 1.0 - R / a;
+      const double esinE = rv / std::sqrt(mu * a);
+      const double E = std::atan2(esinE, ecosE);
+      M = wrap(E - esinE);
+    } else {
+      M = std::numeric_limits<double>::quiet_NaN();
+    }
+  }
+  out[0] = a; out[1] = e; out[2] = inc; out[3] = Omega; out[4] = omega; out[5] = M;
+}
+
 }  // extern "C"

@@ -439,3 +439,73 @@ def test_advance_with_own_log_is_identical(oracle_mod):
         assert np.array_equal(x, y)
     qa, _ = A.read_planets()
     assert np.array_equal(log[200, :12].reshape(4, 3), qa)
+
+
+# ---------------------------------------------------------------------------------------------------
+# T9  osculating elements (snapshot output) against the textbook construction
+# ---------------------------------------------------------------------------------------------------
+def _state_from_elements(mu, a, e, inc, Om, om, f):
+    """Perifocal state at true anomaly f rotated by R_z(Om) R_x(inc) R_z(om), written out here
+    (Murray & Dermott eq. 2.119-2.122); returns r, v and the mean anomaly of f."""
+    p = a * (1.0 - e * e)
+    r = p / (1.0 + e * np.cos(f))
+    rp = np.array([r * np.cos(f), r * np.sin(f), 0.0])
+    vp = np.sqrt(mu / p) * np.array([-np.sin(f), e + np.cos(f), 0.0])
+
+    def rz(t):
+        return np.array([[np.cos(t), -np.sin(t), 0], [np.sin(t), np.cos(t), 0], [0, 0, 1.0]])
+
+    def rx(t):
+        return np.array([[1.0, 0, 0], [0, np.cos(t), -np.sin(t)], [0, np.sin(t), np.cos(t)]])
+
+    R = rz(Om) @ rx(inc) @ rz(om)
+    E = 2.0 * np.arctan2(np.sqrt(1.0 - e) * np.sin(f / 2.0), np.sqrt(1.0 + e) * np.cos(f / 2.0))
+    M = (E - e * np.sin(E)) % (2.0 * np.pi)
+    return R @ rp, R @ vp, M
+
+
+def test_T9_elements_match_textbook_construction(oracle_mod):
+    mu = inputs.G
+    rng = np.random.default_rng(9)
+    worst = 0.0
+    for _ in range(400):
+        a, e = rng.uniform(0.5, 80.0), rng.uniform(0.01, 0.9)
+        inc, Om, om, f = rng.uniform(0.05, 3.0), *rng.uniform(0.0, 2.0 * np.pi, 3)
+        r, v, M = _state_from_elements(mu, a, e, inc, Om, om, f)
+        el = oracle_mod.elements(mu, r[:, None], v[:, None])[:, 0]
+        worst = max(worst, abs(el[0] / a - 1.0), abs(el[1] - e), abs(el[2] - inc),
+                    abs(angle_diff(el[3], Om)) * np.sin(inc), abs(angle_diff(el[4], om)) * e * np.sin(inc),
+                    abs(angle_diff(el[5], M)) * e)
+    assert worst < 5e-13, worst
+
+
+def test_T9_elements_special_cases_and_drift_invariance(oracle_mod):
+    mu = inputs.G
+    a, e = 30.0, 0.25
+    # pericentre on the x axis of an equatorial orbit: (a, e, 0, 0, 0, 0)
+    r = np.array([a * (1 - e), 0.0, 0.0])
+    v = np.array([0.0, np.sqrt(mu * (1 + e) / (a * (1 - e))), 0.0])
+    el = oracle_mod.elements(mu, r[:, None], v[:, None])[:, 0]
+    assert abs(el[0] - a) < 1e-12 and abs(el[1] - e) < 1e-14 and el[2] == 0.0 and el[3] == 0.0
+    assert min(el[4], 2 * np.pi - el[4]) < 1e-14 and min(el[5], 2 * np.pi - el[5]) < 1e-14
+    # circular equatorial orbit a quarter turn on: omega = 0 by convention, M = the longitude
+    r = np.array([0.0, 7.0, 0.0])
+    v = np.array([-np.sqrt(mu / 7.0), 0.0, 0.0])
+    el = oracle_mod.elements(mu, r[:, None], v[:, None])[:, 0]
+    assert abs(el[0] - 7.0) < 1e-12 and el[1] < 1e-15 and el[2] == 0.0 and el[3] == 0.0
+    assert abs(el[4] + el[5] - np.pi / 2) < 1e-12 or abs(el[4] + el[5] - np.pi / 2 - 2 * np.pi) < 1e-12
+    # retrograde: i = pi
+    el = oracle_mod.elements(mu, r[:, None], -v[:, None])[:, 0]
+    assert abs(el[2] - np.pi) < 1e-15
+    # hyperbolic: a < 0, e > 1, M undefined
+    el = oracle_mod.elements(mu, r[:, None], 2.0 * v[:, None])[:, 0]
+    assert el[0] < 0 and el[1] > 1 and np.isnan(el[5])
+    # under the oracle's own two-body drift a, e, i, Omega, omega stay and M advances by n dt
+    r0, v0, M0 = _state_from_elements(mu, 25.0, 0.3, 0.4, 1.0, 2.0, 0.7)
+    fl, r1, v1 = oracle_mod.kepler_drift(mu, r0, v0, 180.0)
+    assert fl == 0
+    e0 = oracle_mod.elements(mu, r0[:, None], v0[:, None])[:, 0]
+    e1 = oracle_mod.elements(mu, r1[:, None], v1[:, None])[:, 0]
+    assert np.allclose(e0[:5], e1[:5], rtol=0, atol=2e-13)
+    n = np.sqrt(mu / 25.0 ** 3)
+    assert abs(angle_diff(e1[5], e0[5] + n * 180.0)) < 1e-12
