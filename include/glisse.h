@@ -137,6 +137,31 @@ int glisse_planet_log(glisse_sim* sim, long long n_steps, double* log);
 int glisse_read(glisse_sim* sim, double* const pos[3], double* const vel[3],
                 int* flag, long long* removal_step);
 
+/*
+ * Snapshot: the periodic output of the particle arrays ("copied back to the CPU after
+ * a user-configurable number of planetary chunk calculations"; "logged orbital
+ * elements").  ASYNCHRONOUS: the call queues a device-side copy of the state
+ * at the current step, in original particle order, and returns; a third stream then copies it to
+ * the caller's buffers while later glisse_advance calls keep the device busy.  The buffers must stay
+ * valid, and must not be read, until glisse_snapshot_wait returns.  One snapshot is in flight at a
+ * time: a second call first waits (on the device) for the first one's copies.
+ *   kind   GLISSE_SNAPSHOT_CARTESIAN  out[0..5] = x, y, z, vx, vy, vz
+ *          GLISSE_SNAPSHOT_ELEMENTS   out[0..5] = a, e, i, Omega, omega, M: osculating heliocentric
+ *          elements about gm_star (Murray & Dermott §2.8: h = r x v, vis-viva, eccentricity vector;
+ *          tan i = |h_xy|/h_z; i = 0: Omega = 0 and omega from x; e = 0: omega = 0, M = angle of r;
+ *          unbound: a < 0, M = NaN; angles in [0, 2 pi))
+ *   out    six pointers to arrays of N doubles (any may be NULL: skipped); flag int[N] and
+ *          removal_step long long[N] as in glisse_read (may be NULL).  Host (pinned, for the copy
+ *          to overlap) or device.
+ * A removed particle reports the state (or elements of the state) frozen at its removal.
+ */
+#define GLISSE_SNAPSHOT_CARTESIAN 0
+#define GLISSE_SNAPSHOT_ELEMENTS  1
+int glisse_snapshot(glisse_sim* sim, int kind, double* const out[6], int* flag, long long* removal_step);
+
+/* Wait until the buffers of the last glisse_snapshot are filled.  Does not wait for the particles. */
+int glisse_snapshot_wait(glisse_sim* sim);
+
 /* Heliocentric planet positions and velocities at the current step, [n_planets][3] each, host
  * or device, either may be NULL.  Synchronises. */
 int glisse_read_planets(glisse_sim* sim, double* pos, double* vel);

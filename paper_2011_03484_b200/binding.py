@@ -24,6 +24,7 @@ FLAG_ACTIVE, FLAG_RMIN, FLAG_RMAX, FLAG_NONCONV, FLAG_UNBOUND, FLAG_PLANET0 = 0,
 EXPORTS = (
     "glisse_default_params", "glisse_create", "glisse_advance", "glisse_advance_with_log",
     "glisse_log_stride", "glisse_planet_log", "glisse_read", "glisse_read_planets",
+    "glisse_snapshot", "glisse_snapshot_wait",
     "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_launch_count", "glisse_sync",
     "glisse_particle_kernel_time", "glisse_fp64_peak_probe", "glisse_test_primitive", "glisse_destroy",
     "glisse_strerror",
@@ -70,6 +71,10 @@ def lib():
         L.glisse_planet_log.restype = c_int
         L.glisse_read.argtypes = [c_void_p, P3, P3, c_void_p, c_void_p]
         L.glisse_read.restype = c_int
+        L.glisse_snapshot.argtypes = [c_void_p, c_int, POINTER(c_void_p), c_void_p, c_void_p]
+        L.glisse_snapshot.restype = c_int
+        L.glisse_snapshot_wait.argtypes = [c_void_p]
+        L.glisse_snapshot_wait.restype = c_int
         L.glisse_read_planets.argtypes = [c_void_p, c_void_p, c_void_p]
         L.glisse_read_planets.restype = c_int
         for name in ("glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_launch_count"):
@@ -201,6 +206,32 @@ class GlisseSim:
                                _ptr(flag), _ptr(rstep))
         _check(st, "glisse_read")
         return pos, vel, flag, rstep
+
+    def snapshot(self, kind="cartesian", out=None):
+        """glisse_snapshot: queue an asynchronous copy of the state at the current step and return
+        at once.  kind: "cartesian" (x, y, z, vx, vy, vz) or "elements" (a, e, i, Omega, omega, M).
+        out = (data[6,N], flag[N] int32, removal_step[N] int64): numpy arrays (pinned, e.g. views of
+        pinned torch tensors, for the copy to overlap) or torch CUDA tensors; allocated (pageable)
+        when omitted.  The arrays are valid after snapshot_wait()."""
+        k = {"cartesian": 0, "elements": 1}[kind]
+        if out is None:
+            data = np.empty((6, self.n), dtype=np.float64)
+            flag = np.empty(self.n, dtype=np.int32)
+            rstep = np.empty(self.n, dtype=np.int64)
+        else:
+            data, flag, rstep = out
+        rows = None
+        if data is not None:
+            rows = (c_void_p * 6)(*[(data[j].data_ptr() if _is_torch(data) else data[j].ctypes.data)
+                                    for j in range(6)])
+        st = lib().glisse_snapshot(self._h, k, rows, _ptr(flag), _ptr(rstep))
+        _check(st, "glisse_snapshot")
+        self._snap_keep = (data, flag, rstep)   # keep the buffers alive until the wait
+        return data, flag, rstep
+
+    def snapshot_wait(self):
+        _check(lib().glisse_snapshot_wait(self._h), "glisse_snapshot_wait")
+        self._snap_keep = None
 
     def read_planets(self):
         pos = np.empty((self.n_planets, 3), dtype=np.float64)

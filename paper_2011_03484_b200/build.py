@@ -15,7 +15,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libglisse.so")
-SOURCES = ["api.cu", "particles.cu", "planets.cu", "compact.cu", "probe.cu"]
+SOURCES = ["api.cu", "particles.cu", "planets.cu", "compact.cu", "snapshot.cu", "probe.cu"]
 HEADERS = ["glisse_internal.cuh", "kepler.cuh", "sincos_coeffs.inc", os.path.join("..", "..", "include", "glisse.h")]
 
 NVCC_FLAGS = [

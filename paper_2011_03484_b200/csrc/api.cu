@@ -126,6 +126,15 @@ struct glisse_sim {
   bool nslots_pending = false;
   int chunks_since_resync = 0;
 
+  // snapshot staging (glisse_snapshot): a copy in original order that stream r ships to the caller
+  double* snap[6] = {};
+  int* snap_flag = nullptr;
+  long long* snap_rstep = nullptr;
+  cudaStream_t r = nullptr;            // snapshot copy stream
+  cudaEvent_t snap_ready = nullptr;    // staging written            (stream Q)
+  cudaEvent_t snap_done = nullptr;     // staging copied to the caller (stream R)
+  bool snap_in_flight = false;
+
   unsigned long long* d_counters = nullptr;  // [0] particle-steps, [1] scratch for counts
   long long launches = 0;
 
@@ -176,6 +185,10 @@ void free_sim(glisse_sim* s) {
   cudaSetDevice(s->device);
   if (s->q) cudaStreamSynchronize(s->q);
   if (s->p) cudaStreamSynchronize(s->p);
+  if (s->r) cudaStreamSynchronize(s->r);
+  if (s->snap_ready) cudaEventDestroy(s->snap_ready);
+  if (s->snap_done) cudaEventDestroy(s->snap_done);
+  if (s->r) cudaStreamDestroy(s->r);
   for (int b = 0; b < 2; ++b) {
     if (s->buf[b].ready) cudaEventDestroy(s->buf[b].ready);
     if (s->buf[b].consumed) cudaEventDestroy(s->buf[b].consumed);
@@ -449,6 +462,9 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     for (int k = 0; k < 6; ++k) need(&s->fin[k], N);
     need(&s->fin_flag, N);
     need(&s->fin_rstep, N);
+    for (int k = 0; k < 6; ++k) need(&s->snap[k], N);
+    need(&s->snap_flag, N);
+    need(&s->snap_rstep, N);
     need(&s->d_nslots, 2);
     need(&s->d_block_counts, static_cast<size_t>((N + 255) / 256 + 1));
     need(&s->d_counters, 2);
@@ -684,6 +700,63 @@ int glisse_read(glisse_sim* s, double* const pos[3], double* const vel[3], int* 
   if (removal_step)
     CKS(s, cudaMemcpyAsync(removal_step, s->fin_rstep, N * sizeof(long long), cudaMemcpyDefault, s->q));
   return sync_all(s);
+}
+
+int glisse_snapshot(glisse_sim* s, int kind, double* const out[6], int* flag, long long* removal_step) {
+  if (!s || (kind != GLISSE_SNAPSHOT_CARTESIAN && kind != GLISSE_SNAPSHOT_ELEMENTS)) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  if (!s->r) {  // first snapshot of this sim: its copy stream and events
+    CKS(s, cudaStreamCreateWithFlags(&s->r, cudaStreamNonBlocking));
+    CKS(s, cudaEventCreateWithFlags(&s->snap_ready, cudaEventDisableTiming));
+    CKS(s, cudaEventCreateWithFlags(&s->snap_done, cudaEventDisableTiming));
+  }
+  // the staging arrays are free once the previous snapshot's copies are done (device-side wait)
+  if (s->snap_in_flight) CKS(s, cudaStreamWaitEvent(s->q, s->snap_done, 0));
+  // working order -> original order (as glisse_read), then -> staging, Cartesian or elements
+  ScatterArgs g{};
+  const int w = s->w;
+  for (int k = 0; k < 6; ++k) {
+    g.st[k] = s->work[w][k];
+    g.fin[k] = s->fin[k];
+  }
+  g.id = s->id[w]; g.flag = s->flag[w]; g.rstep = s->rstep[w];
+  g.n_slots = s->d_nslots + w;
+  g.fin_flag = s->fin_flag; g.fin_rstep = s->fin_rstep;
+  CKS(s, launch_scatter_to_original(g, s->nslots_upper, s->q));
+  SnapshotArgs a{};
+  for (int k = 0; k < 6; ++k) {
+    a.fin[k] = s->fin[k];
+    a.out[k] = s->snap[k];
+  }
+  a.fin_flag = s->fin_flag; a.fin_rstep = s->fin_rstep;
+  a.out_flag = s->snap_flag; a.out_rstep = s->snap_rstep;
+  a.n = s->n;
+  a.mu = s->gm0;
+  a.kind = kind;
+  CKS(s, launch_snapshot(a, s->q));
+  s->launches += 2;
+  CKS(s, cudaEventRecord(s->snap_ready, s->q));
+  // from here on the particle stream is free to go on; stream r ships the staging copy
+  CKS(s, cudaStreamWaitEvent(s->r, s->snap_ready, 0));
+  const size_t N = static_cast<size_t>(s->n);
+  for (int k = 0; k < 6; ++k)
+    if (out && out[k]) CKS(s, cudaMemcpyAsync(out[k], s->snap[k], N * sizeof(double), cudaMemcpyDefault, s->r));
+  if (flag) CKS(s, cudaMemcpyAsync(flag, s->snap_flag, N * sizeof(int), cudaMemcpyDefault, s->r));
+  if (removal_step)
+    CKS(s, cudaMemcpyAsync(removal_step, s->snap_rstep, N * sizeof(long long), cudaMemcpyDefault, s->r));
+  CKS(s, cudaEventRecord(s->snap_done, s->r));
+  s->snap_in_flight = true;
+  return GLISSE_OK;
+}
+
+int glisse_snapshot_wait(glisse_sim* s) {
+  if (!s) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (!s->r) return GLISSE_OK;  // no snapshot was ever taken
+  CKS(s, cudaSetDevice(s->device));
+  CKS(s, cudaStreamSynchronize(s->r));
+  return GLISSE_OK;
 }
 
 int glisse_read_planets(glisse_sim* s, double* pos, double* vel) {

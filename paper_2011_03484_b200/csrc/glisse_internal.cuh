@@ -115,6 +115,18 @@ cudaError_t launch_init_ids(int* id, int* flag, long long* rstep, int* fin_flag,
                             cudaStream_t s);
 cudaError_t launch_count_nonfinite(const double* p, long long n, unsigned long long* out, cudaStream_t s);
 
+// snapshot.cu: original-order arrays -> staging copy, Cartesian or osculating elements
+struct SnapshotArgs {
+  const double* fin[6];
+  const int* fin_flag; const long long* fin_rstep;
+  double* out[6];
+  int* out_flag; long long* out_rstep;
+  long long n;
+  double mu;
+  int kind;
+};
+cudaError_t launch_snapshot(const SnapshotArgs& a, cudaStream_t s);
+
 cudaError_t run_fp64_probe(cudaStream_t s, double millis, double* flops);
 cudaError_t run_primitive(int which, long long n, const double* in, double* out, cudaStream_t s);
 

@@ -557,3 +557,73 @@ def test_full_size_sampled_parity(gl, oracle_mod, name):
     assert (ok & (bound <= TOL)).sum() >= (0.75 if name == "c5" else 0.99) * len(idx)
     if name in ("c2", "1m_x4"):
         assert ok.all() and dev.max() <= TOL
+
+
+# ---------------------------------------------------------------------------------------------------
+# snapshots
+# ---------------------------------------------------------------------------------------------------
+def test_snapshot_cartesian_is_the_state_at_the_call_and_overlaps_advance(gl):
+    """The snapshot is asynchronous: taken at step 300, waited for after the sim has gone on to step
+    900, it must hold the state of step 300 bit for bit (compaction in between included)."""
+    w = inputs.config(5, n_particles=6000)
+    S = gl.GlisseSim.from_workload(w, chunk_steps=100, resync_chunks=1)
+    S.advance(300)
+    data, flag, rstep = S.snapshot("cartesian")
+    S.advance(600)
+    S.snapshot_wait()
+    later = S.read()
+    S.close()
+    ref, _, _ = _run_gpu(gl, w, [300], chunk_steps=100, resync_chunks=1)
+    assert np.array_equal(data[:3], ref[0]) and np.array_equal(data[3:], ref[1])
+    assert np.array_equal(flag, ref[2]) and np.array_equal(rstep, ref[3])
+    assert (flag != 0).sum() > 50 and not np.array_equal(later[0], ref[0])
+
+
+def test_snapshot_elements_match_oracle(gl, oracle_mod):
+    """a, e, i, Omega, omega, M of the state against the oracle's textbook elements of the same
+    state; an angle is compared times the quantity that conditions it (sin i for Omega, e sin i for
+    omega, e for M) and through the well-conditioned sums (longitude of pericentre, mean longitude)."""
+    w = inputs.config(5, n_particles=4096)
+    S = gl.GlisseSim.from_workload(w, chunk_steps=128)
+    S.advance(256)
+    el, flag, rstep = S.snapshot("elements")
+    S.snapshot_wait()
+    pos, vel, f2, r2 = S.read()
+    two = S.snapshot("elements")     # a second snapshot reuses the staging arrays
+    S.snapshot_wait()
+    S.close()
+    assert np.array_equal(flag, f2) and np.array_equal(rstep, r2)
+    assert np.array_equal(two[0], el, equal_nan=True)
+    ref = oracle_mod.elements(w.gm_star, pos, vel)
+    bound = ref[0] > 0
+
+    def ang(a, b):
+        return np.abs((a - b + np.pi) % (2 * np.pi) - np.pi)
+
+    assert np.isnan(el[5][~bound]).all() and np.isnan(ref[5][~bound]).all()
+    assert np.max(np.abs(el[0] / ref[0] - 1)) < 1e-13
+    assert np.max(np.abs(el[1] - ref[1])) < 1e-13 and np.max(np.abs(el[2] - ref[2])) < 1e-13
+    si, e = np.sin(ref[2]), ref[1]
+    assert np.max(ang(el[3], ref[3]) * si) < 1e-12
+    assert np.max(ang(el[4], ref[4]) * e * si) < 1e-12
+    assert np.max((ang(el[5], ref[5]) * e)[bound]) < 1e-12
+    assert np.max(ang(el[3] + el[4], ref[3] + ref[4]) * e) < 1e-11          # longitude of pericentre
+    assert np.max(ang((el[3] + el[4] + el[5])[bound], (ref[3] + ref[4] + ref[5])[bound])) < 1e-11  # mean longitude
+    assert ((el[3:5] >= 0) & (el[3:5] < 2 * np.pi)).all()
+
+
+def test_snapshot_to_device_buffers_and_bad_kind(gl):
+    import torch
+    w = inputs.config(1)
+    S = gl.GlisseSim.from_workload(w)
+    S.advance(10)
+    d = torch.empty((6, w.n_particles), dtype=torch.float64, device="cuda")
+    fl = torch.empty(w.n_particles, dtype=torch.int32, device="cuda")
+    rs = torch.empty(w.n_particles, dtype=torch.int64, device="cuda")
+    S.snapshot("cartesian", out=(d, fl, rs))
+    S.snapshot_wait()
+    pos, vel, f, r = S.read()
+    assert np.array_equal(d[:3].cpu().numpy(), pos) and np.array_equal(d[3:].cpu().numpy(), vel)
+    assert np.array_equal(fl.cpu().numpy(), f) and np.array_equal(rs.cpu().numpy(), r)
+    assert gl.lib().glisse_snapshot(S._h, 7, None, None, None) == gl.EINVAL
+    S.close()
