@@ -37,38 +37,53 @@ __device__ __forceinline__ double shfl(double v, int src) { return __shfl_sync(k
 template <int NP>
 __device__ __forceinline__ int count(const Lane& L) { return NP > 0 ? NP : L.np; }
 
-// exclusive prefix sum over lanes i < lane of c_i, added in increasing i
+// Partner of this lane in round jj = 0 .. np−2 of an all-pairs exchange: lane+1, lane+2, ... wrapping
+// at np.  No lane ever meets itself, so the pair terms need no self test and no branch; partners
+// above the lane come first and in increasing order, then those below it in increasing order, so the
+// one-sided sums of the definition (over i > k, over i < k) are still added in increasing i.
 template <int NP>
-__device__ __forceinline__ void prefix3(const Lane& L, double cx, double cy, double cz, double& sx, double& sy,
-                                        double& sz) {
-  sx = sy = sz = 0.0;
+__device__ __forceinline__ int partner(const Lane& L, int jj) {
   const int np = count<NP>(L);
-#pragma unroll
-  for (int i = 0; i + 1 < np; ++i) {
-    const double tx = shfl(cx, i), ty = shfl(cy, i), tz = shfl(cz, i);
-    if (i < L.lane) { sx += tx; sy += ty; sz += tz; }
-  }
+  const int j = L.lane + 1 + jj;
+  return j >= np ? j - np : j;   // lanes >= np (idle) read some live lane; their results are discarded
 }
 
-// q from r' (Jacobi -> heliocentric); the same linear map serves velocities
+// q from r' (Jacobi -> heliocentric): q_k = r'_k + sum_{i<k} (gm_i/eta_i) r'_i; the same linear map
+// serves velocities
 template <int NP>
 __device__ __forceinline__ void jacobi_to_helio(const Lane& L, double rx, double ry, double rz, double& qx,
                                                 double& qy, double& qz) {
-  double sx, sy, sz;
-  prefix3<NP>(L, L.wj * rx, L.wj * ry, L.wj * rz, sx, sy, sz);
+  const int np = count<NP>(L);
+  const double cx = L.wj * rx, cy = L.wj * ry, cz = L.wj * rz;
+  double sx = 0.0, sy = 0.0, sz = 0.0;
+#pragma unroll
+  for (int jj = 0; jj + 1 < np; ++jj) {
+    const int j = partner<NP>(L, jj);
+    const double tx = shfl(cx, j), ty = shfl(cy, j), tz = shfl(cz, j);
+    const bool below = j < L.lane;
+    sx += below ? tx : 0.0; sy += below ? ty : 0.0; sz += below ? tz : 0.0;
+  }
   qx = rx + sx; qy = ry + sy; qz = rz + sz;
 }
 
-// r' from q (heliocentric -> Jacobi)
+// r' from q (heliocentric -> Jacobi): r'_k = q_k − (sum_{i<k} gm_i q_i)/eta_{k−1}
 template <int NP>
 __device__ __forceinline__ void helio_to_jacobi(const Lane& L, double qx, double qy, double qz, double& rx,
                                                 double& ry, double& rz) {
-  double sx, sy, sz;
-  prefix3<NP>(L, L.gm * qx, L.gm * qy, L.gm * qz, sx, sy, sz);
+  const int np = count<NP>(L);
+  const double cx = L.gm * qx, cy = L.gm * qy, cz = L.gm * qz;
+  double sx = 0.0, sy = 0.0, sz = 0.0;
+#pragma unroll
+  for (int jj = 0; jj + 1 < np; ++jj) {
+    const int j = partner<NP>(L, jj);
+    const double tx = shfl(cx, j), ty = shfl(cy, j), tz = shfl(cz, j);
+    const bool below = j < L.lane;
+    sx += below ? tx : 0.0; sy += below ? ty : 0.0; sz += below ? tz : 0.0;
+  }
   rx = qx - sx * L.inv_eta_prev; ry = qy - sy * L.inv_eta_prev; rz = qz - sz * L.inv_eta_prev;
 }
 
-// Jacobi acceleration of this lane's planet, and h0 (the same on every lane)
+// Jacobi acceleration of this lane's planet, and h0 (valid on lane 0, which writes it)
 template <int NP>
 __device__ __forceinline__ void kick_accel(const Lane& L, double qx, double qy, double qz, double rx, double ry,
                                            double rz, double& ax, double& ay, double& az, double& hx, double& hy,
@@ -82,29 +97,33 @@ __device__ __forceinline__ void kick_accel(const Lane& L, double qx, double qy, 
   // the Jacobi two-body term, independent of the sums below
   const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
   const double w0 = gm_over_r3(L.gm0, r2);
-  hx = hy = hz = 0.0;
+  hx = -tx; hy = -ty; hz = -tz;   // lane 0: t_0, then t_1, t_2, ... in the rounds below
 #pragma unroll
-  for (int j = 0; j < np; ++j) {
+  for (int jj = 0; jj + 1 < np; ++jj) {
+    const int j = partner<NP>(L, jj);
     const double gj = shfl(L.gm, j);
     const double qjx = shfl(qx, j), qjy = shfl(qy, j), qjz = shfl(qz, j);
     hx -= shfl(tx, j); hy -= shfl(ty, j); hz -= shfl(tz, j);
-    const bool self = (j == L.lane);
     const double dx = qx - qjx, dy = qy - qjy, dz = qz - qjz;
-    const double d2 = self ? 1.0 : fma(dx, dx, fma(dy, dy, dz * dz));
-    const double w = self ? 0.0 : gm_over_r3(gj, d2);
+    const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    const double w = gm_over_r3(gj, d2);
     Ax = fma(-w, dx, Ax); Ay = fma(-w, dy, Ay); Az = fma(-w, dz, Az);
   }
   // tail_k = sum_{i>k} gm_i A_i, added in increasing i
   const double mx = L.gm * Ax, my = L.gm * Ay, mz = L.gm * Az;
   double Tx = 0.0, Ty = 0.0, Tz = 0.0;
 #pragma unroll
-  for (int i = 1; i < np; ++i) {
-    const double ux = shfl(mx, i), uy = shfl(my, i), uz = shfl(mz, i);
-    if (i > L.lane) { Tx += ux; Ty += uy; Tz += uz; }
+  for (int jj = 0; jj + 1 < np; ++jj) {
+    const int j = partner<NP>(L, jj);
+    const double ux = shfl(mx, j), uy = shfl(my, j), uz = shfl(mz, j);
+    const bool above = j > L.lane;
+    Tx += above ? ux : 0.0; Ty += above ? uy : 0.0; Tz += above ? uz : 0.0;
   }
-  ax = L.sc * (fma(w0, rx, Ax) + Tx * L.inv_eta);
-  ay = L.sc * (fma(w0, ry, Ay) + Ty * L.inv_eta);
-  az = L.sc * (fma(w0, rz, Az) + Tz * L.inv_eta);
+  // idle lanes get a zero kick: their stand-in orbit stays the circle it started as
+  const double sc = L.live ? L.sc : 0.0;
+  ax = sc * (fma(w0, rx, Ax) + Tx * L.inv_eta);
+  ay = sc * (fma(w0, ry, Ay) + Ty * L.inv_eta);
+  az = sc * (fma(w0, rz, Az) + Tz * L.inv_eta);
 }
 
 __device__ __forceinline__ Lane make_lane(const PlanetSystem* sys) {
@@ -149,8 +168,11 @@ __global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, c
   const int stride = log_stride(L.np);
   const double hdt = 0.5 * dt;
   const double inv_mu_dt = L.inv_mu * dt;
-  // dead lanes carry a harmless circular-orbit state
-  double rx = 1.0 + L.lane, ry = 0.0, rz = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+  // Idle lanes (lane >= np) carry a stand-in: a circular orbit with n dt = 0.01, never kicked, never
+  // written.  It takes the same path through the drift as the planets (one quartic step), so the
+  // warp does not diverge there; a lane that is merely masked off would.
+  const double r_idle = cbrt(L.gm0 * dt * dt * 1e4);
+  double rx = r_idle, ry = 0.0, rz = 0.0, vx = 0.0, vy = sqrt(L.gm0 / r_idle), vz = 0.0;
   if (L.live) {
     rx = jin[3 * L.lane]; ry = jin[3 * L.lane + 1]; rz = jin[3 * L.lane + 2];
     vx = jin[3 * L.np + 3 * L.lane]; vy = jin[3 * L.np + 3 * L.lane + 1]; vz = jin[3 * L.np + 3 * L.lane + 2];
@@ -161,15 +183,15 @@ __global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, c
   write_record(L, log, jlog, 0, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
   int bad = 0;
   for (int s = 0; s < nsteps; ++s) {
-    if (L.live) { vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz); }
+    vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
     const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
-    const int st = kepler_drift_warp(L.live, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2,
+    const int st = kepler_drift_warp(true, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2,
                                      rx, ry, rz, vx, vy, vz);
-    const unsigned failed = __ballot_sync(kFullMask, st != 0);
+    const unsigned failed = __ballot_sync(kFullMask, st != 0 && L.live);
     if (failed && !bad) bad = __ffs(failed);
     jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
     kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
-    if (L.live) { vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz); }
+    vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
     write_record(L, log, jlog, s + 1, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
   }
   if (bad && L.lane == 0 && sys->status == 0) sys->status = bad;
