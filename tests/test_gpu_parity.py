@@ -627,3 +627,28 @@ def test_snapshot_to_device_buffers_and_bad_kind(gl):
     assert np.array_equal(fl.cpu().numpy(), f) and np.array_equal(rs.cpu().numpy(), r)
     assert gl.lib().glisse_snapshot(S._h, 7, None, None, None) == gl.EINVAL
     S.close()
+
+
+def test_several_sims_share_the_device_and_the_pools(gl):
+    """Interleaved lifetimes: the arena pool, the pinned page and the per-device kernel configuration
+    are process-wide; every sim must still reproduce the stand-alone result bit for bit."""
+    w1, w2 = inputs.config(1), inputs.config(5, n_particles=3000)
+    ref1, _, _ = _run_gpu(gl, w1, [300], chunk_steps=64)
+    ref2, _, _ = _run_gpu(gl, w2, [300], chunk_steps=128)
+    A = gl.GlisseSim.from_workload(w1, chunk_steps=64)
+    B = gl.GlisseSim.from_workload(w2, chunk_steps=128)
+    A.advance(100)
+    C = gl.GlisseSim.from_workload(w1, chunk_steps=64)
+    B.advance(300)
+    A.advance(200)
+    C.advance(300)
+    outs = [A.read(), B.read(), C.read()]
+    B.close()
+    D = gl.GlisseSim.from_workload(w2, chunk_steps=128)   # reuses what B gave back
+    D.advance(300)
+    outs.append(D.read())
+    for S in (A, C, D):
+        S.close()
+    for out, ref in zip(outs, (ref1, ref2, ref1, ref2)):
+        for a, b in zip(out, ref):
+            assert np.array_equal(a, b)
