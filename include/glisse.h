@@ -162,6 +162,30 @@ int glisse_snapshot(glisse_sim* sim, int kind, double* const out[6], int* flag, 
 /* Wait until the buffers of the last glisse_snapshot are filled.  Does not wait for the particles. */
 int glisse_snapshot_wait(glisse_sim* sim);
 
+/*
+ * Resonant-argument reduction on the device.  For the p:q
+ * mean-motion resonance with planet `planet` the argument is
+ *     phi = p lambda − q lambda_planet − (p − q) varpi,   lambda = Omega + omega + M,  varpi = Omega + omega
+ * (phi_31 = 3 lambda − lambda_N − 2 varpi, phi_52 = 5 lambda − 2 lambda_N − 3 varpi in the paper), from
+ * the osculating heliocentric elements of glisse_snapshot; the planet's about gm_star + gm_planet.
+ * "Librating particles [are] those with a resonant argument that never comes within 10 deg of 0 deg or
+ * never within 10 deg of 180 deg": the library keeps, per particle, whether phi has been within
+ * `window` (radians) of 0 and of pi at any sample.
+ *   glisse_resonance_begin   choose the resonance and clear the record.  p > q >= 1.
+ *   glisse_resonance_sample  evaluate phi at the current step for every ACTIVE particle and update the
+ *                            record; asynchronous on the particle stream (call it between advances,
+ *                            at the cadence of the paper's element log).
+ *   glisse_resonance_read    seen0[N], seen180[N] (bytes, 0/1), phi_last[N] (the last sample's phi in
+ *                            [0, 2 pi); NaN-free only for particles sampled at least once), original
+ *                            particle order, host or device, any may be NULL; *n_samples = samples
+ *                            taken since begin.  Synchronises.
+ * GLISSE_EINVAL without a preceding begin, for planet outside [0, n_planets), or p <= q or q < 1.
+ */
+int glisse_resonance_begin(glisse_sim* sim, int planet, int p, int q, double window);
+int glisse_resonance_sample(glisse_sim* sim);
+int glisse_resonance_read(glisse_sim* sim, unsigned char* seen0, unsigned char* seen180, double* phi_last,
+                          long long* n_samples);
+
 /* Heliocentric planet positions and velocities at the current step, [n_planets][3] each, host
  * or device, either may be NULL.  Synchronises. */
 int glisse_read_planets(glisse_sim* sim, double* pos, double* vel);

@@ -67,6 +67,9 @@ def lib():
         L.oracle_default_params.argtypes = [POINTER(_Params)]
         L.oracle_elements.argtypes = [c_double, c_void_p, c_void_p, c_void_p]
         L.oracle_elements.restype = None
+        L.oracle_resonant_argument.argtypes = [c_double, c_void_p, c_void_p, c_double, c_void_p, c_void_p,
+                                               c_int, c_int]
+        L.oracle_resonant_argument.restype = c_double
         L.oracle_kepler_drift.argtypes = [c_double, c_void_p, c_void_p, c_double, c_int, c_double]
         L.oracle_kepler_drift.restype = c_int
         L.oracle_planet_kick_accel.argtypes = [c_int, c_double, c_void_p, c_void_p, c_void_p]
@@ -195,6 +198,16 @@ def elements(mu, pos, vel):
     for k in range(pos.shape[0]):
         L.oracle_elements(c_double(mu), _p(pos[k]), _p(vel[k]), _p(out[k]))
     return np.ascontiguousarray(out.T)
+
+
+def resonant_argument(mu, pos, vel, mu_pl, rp, vp, p, q):
+    """phi = p lambda − q lambda_pl − (p − q) varpi of each column of pos, vel ([3, N]) -> [N]."""
+    L = lib()
+    pos = np.ascontiguousarray(np.asarray(pos, dtype=np.float64).T)
+    vel = np.ascontiguousarray(np.asarray(vel, dtype=np.float64).T)
+    rp, vp = _f64(rp), _f64(vp)
+    return np.array([L.oracle_resonant_argument(c_double(mu), _p(pos[k]), _p(vel[k]), c_double(mu_pl), _p(rp),
+                                                _p(vp), int(p), int(q)) for k in range(pos.shape[0])])
 
 
 def kepler_drift(mu, r, v, dt, iters=5, tol=1e-14):

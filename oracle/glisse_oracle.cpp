@@ -551,4 +551,21 @@ void oracle_elements(double mu, const double* r, const double* v, double* out) {
   out[0] = a; out[1] = e; out[2] = inc; out[3] = Omega; out[4] = omega; out[5] = M;
 }
 
+/* Resonant argument of the p:q mean-motion resonance with a planet:
+ * phi = p lambda − q lambda_pl − (p − q) varpi, lambda = Omega + omega + M, varpi = Omega + omega, from
+ * the osculating elements above (the particle's about mu, the planet's about mu_pl = G(m0 + m_pl));
+ * returned in [0, 2 pi). */
+double oracle_resonant_argument(double mu, const double* r, const double* v, double mu_pl, const double* rp,
+                                const double* vp, int p, int q) {
+  double el[6], pl[6];
+  oracle_elements(mu, r, v, el);
+  oracle_elements(mu_pl, rp, vp, pl);
+  const double varpi = el[3] + el[4];
+  const double lambda = varpi + el[5];
+  const double lambda_pl = pl[3] + pl[4] + pl[5];
+  double phi = std::fmod(p * lambda - q * lambda_pl - (p - q) * varpi, 2.0 * M_PI);
+  if (phi < 0.0) phi += 2.0 * M_PI;
+  return phi;
+}
+
 }  // extern "C"

@@ -25,6 +25,7 @@ EXPORTS = (
     "glisse_default_params", "glisse_create", "glisse_advance", "glisse_advance_with_log",
     "glisse_log_stride", "glisse_planet_log", "glisse_read", "glisse_read_planets",
     "glisse_snapshot", "glisse_snapshot_wait",
+    "glisse_resonance_begin", "glisse_resonance_sample", "glisse_resonance_read",
     "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_launch_count", "glisse_sync",
     "glisse_particle_kernel_time", "glisse_fp64_peak_probe", "glisse_test_primitive", "glisse_destroy",
     "glisse_strerror",
@@ -75,6 +76,12 @@ def lib():
         L.glisse_snapshot.restype = c_int
         L.glisse_snapshot_wait.argtypes = [c_void_p]
         L.glisse_snapshot_wait.restype = c_int
+        L.glisse_resonance_begin.argtypes = [c_void_p, c_int, c_int, c_int, c_double]
+        L.glisse_resonance_begin.restype = c_int
+        L.glisse_resonance_sample.argtypes = [c_void_p]
+        L.glisse_resonance_sample.restype = c_int
+        L.glisse_resonance_read.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_longlong)]
+        L.glisse_resonance_read.restype = c_int
         L.glisse_read_planets.argtypes = [c_void_p, c_void_p, c_void_p]
         L.glisse_read_planets.restype = c_int
         for name in ("glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_launch_count"):
@@ -232,6 +239,23 @@ class GlisseSim:
     def snapshot_wait(self):
         _check(lib().glisse_snapshot_wait(self._h), "glisse_snapshot_wait")
         self._snap_keep = None
+
+    def resonance_begin(self, planet, p, q, window):
+        _check(lib().glisse_resonance_begin(self._h, int(planet), int(p), int(q), float(window)),
+               "glisse_resonance_begin")
+
+    def resonance_sample(self):
+        _check(lib().glisse_resonance_sample(self._h), "glisse_resonance_sample")
+
+    def resonance_read(self):
+        """(seen0[N] uint8, seen180[N] uint8, phi_last[N], n_samples)"""
+        s0 = np.empty(self.n, dtype=np.uint8)
+        s180 = np.empty(self.n, dtype=np.uint8)
+        phi = np.empty(self.n, dtype=np.float64)
+        ns = c_longlong(0)
+        _check(lib().glisse_resonance_read(self._h, _ptr(s0), _ptr(s180), _ptr(phi), byref(ns)),
+               "glisse_resonance_read")
+        return s0, s180, phi, int(ns.value)
 
     def read_planets(self):
         pos = np.empty((self.n_planets, 3), dtype=np.float64)

@@ -135,6 +135,15 @@ struct glisse_sim {
   cudaEvent_t snap_done = nullptr;     // staging copied to the caller (stream R)
   bool snap_in_flight = false;
 
+  // resonant-argument record (glisse_resonance_*), original order
+  double* res_phi = nullptr;
+  unsigned char* res_seen0 = nullptr;
+  unsigned char* res_seen180 = nullptr;
+  int res_planet = -1, res_p = 0, res_q = 0;
+  double res_window = 0.0;
+  long long res_samples = 0;
+  std::vector<double> gm_planet_host;
+
   unsigned long long* d_counters = nullptr;  // [0] particle-steps, [1] scratch for counts
   long long launches = 0;
 
@@ -462,6 +471,9 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     for (int k = 0; k < 6; ++k) need(&s->fin[k], N);
     need(&s->fin_flag, N);
     need(&s->fin_rstep, N);
+    need(&s->res_phi, N);
+    need(&s->res_seen0, N);
+    need(&s->res_seen180, N);
     for (int k = 0; k < 6; ++k) need(&s->snap[k], N);
     need(&s->snap_flag, N);
     need(&s->snap_rstep, N);
@@ -512,6 +524,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     hs.eta[j] = eta;
   }
   hs.status = 0;
+  s->gm_planet_host.assign(gm_planet, gm_planet + np);
   CKF(cudaMemcpyAsync(s->d_sys, &hs, sizeof(hs), cudaMemcpyHostToDevice, s->p));
   if (np > 0) {
     double* d_q = s->d_ptmp;
@@ -757,6 +770,73 @@ int glisse_snapshot_wait(glisse_sim* s) {
   CKS(s, cudaSetDevice(s->device));
   CKS(s, cudaStreamSynchronize(s->r));
   return GLISSE_OK;
+}
+
+int glisse_resonance_begin(glisse_sim* s, int planet, int p, int q, double window) {
+  if (!s || planet < 0 || planet >= s->np || q < 1 || p <= q || !(window > 0.0)) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  const size_t N = static_cast<size_t>(s->n);
+  CKS(s, cudaMemsetAsync(s->res_seen0, 0, N, s->q));
+  CKS(s, cudaMemsetAsync(s->res_seen180, 0, N, s->q));
+  CKS(s, cudaMemsetAsync(s->res_phi, 0, N * sizeof(double), s->q));
+  s->res_planet = planet; s->res_p = p; s->res_q = q;
+  s->res_window = window;
+  s->res_samples = 0;
+  return GLISSE_OK;
+}
+
+int glisse_resonance_sample(glisse_sim* s) {
+  if (!s || s->res_planet < 0) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (s->external_log_used) return GLISSE_EINVAL;  // the internal planet clock is stale
+  CKS(s, cudaSetDevice(s->device));
+  const int np = s->np;
+  // particles: working order -> original order (as glisse_read)
+  ScatterArgs g{};
+  const int w = s->w;
+  for (int k = 0; k < 6; ++k) {
+    g.st[k] = s->work[w][k];
+    g.fin[k] = s->fin[k];
+  }
+  g.id = s->id[w]; g.flag = s->flag[w]; g.rstep = s->rstep[w];
+  g.n_slots = s->d_nslots + w;
+  g.fin_flag = s->fin_flag; g.fin_rstep = s->fin_rstep;
+  CKS(s, launch_scatter_to_original(g, s->nslots_upper, s->q));
+  // planets at the current step: heliocentric q, qd from the Jacobi state of this record
+  const LogBuffer& B = s->buf[s->cur];
+  const long long off = s->step - B.start;
+  double* d_out = s->d_ptmp;
+  CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+  CKS(s, launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q));
+  ResonanceArgs a{};
+  for (int k = 0; k < 6; ++k) a.fin[k] = s->fin[k];
+  a.fin_flag = s->fin_flag;
+  a.planet_q = d_out + 3 * s->res_planet;
+  a.planet_qd = d_out + 3 * np + 3 * s->res_planet;
+  a.phi = s->res_phi; a.seen0 = s->res_seen0; a.seen180 = s->res_seen180;
+  a.n = s->n;
+  a.mu = s->gm0;
+  a.mu_planet = s->gm0 + s->gm_planet_host[s->res_planet];
+  a.window = s->res_window;
+  a.p = s->res_p; a.q = s->res_q;
+  CKS(s, launch_resonance(a, s->q));
+  s->launches += 3;
+  s->res_samples += 1;
+  return GLISSE_OK;
+}
+
+int glisse_resonance_read(glisse_sim* s, unsigned char* seen0, unsigned char* seen180, double* phi_last,
+                          long long* n_samples) {
+  if (!s || s->res_planet < 0) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  const size_t N = static_cast<size_t>(s->n);
+  if (seen0) CKS(s, cudaMemcpyAsync(seen0, s->res_seen0, N, cudaMemcpyDefault, s->q));
+  if (seen180) CKS(s, cudaMemcpyAsync(seen180, s->res_seen180, N, cudaMemcpyDefault, s->q));
+  if (phi_last) CKS(s, cudaMemcpyAsync(phi_last, s->res_phi, N * sizeof(double), cudaMemcpyDefault, s->q));
+  if (n_samples) *n_samples = s->res_samples;
+  return sync_all(s);
 }
 
 int glisse_read_planets(glisse_sim* s, double* pos, double* vel) {

@@ -127,6 +127,21 @@ struct SnapshotArgs {
 };
 cudaError_t launch_snapshot(const SnapshotArgs& a, cudaStream_t s);
 
+// snapshot.cu: resonant-argument reduction over the original-order arrays
+struct ResonanceArgs {
+  const double* fin[6];
+  const int* fin_flag;
+  const double* planet_q;   // [3] heliocentric position of the planet at the current step (device)
+  const double* planet_qd;  // [3] velocity
+  double* phi;              // [n] last value of the argument, [0, 2 pi)
+  unsigned char* seen0;     // [n] phi has been within `window` of 0
+  unsigned char* seen180;   // [n] phi has been within `window` of pi
+  long long n;
+  double mu, mu_planet, window;
+  int p, q;
+};
+cudaError_t launch_resonance(const ResonanceArgs& a, cudaStream_t s);
+
 cudaError_t run_fp64_probe(cudaStream_t s, double millis, double* flops);
 cudaError_t run_primitive(int which, long long n, const double* in, double* out, cudaStream_t s);
 

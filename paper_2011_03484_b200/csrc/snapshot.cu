@@ -36,19 +36,8 @@ __device__ __forceinline__ double in_plane_angle(const double (&w)[3], const dou
   return atan2(w[0] * mx + w[1] * my + w[2] * mz, w[0] * ax + w[1] * ay);
 }
 
-__global__ void __launch_bounds__(256) snapshot_kernel(SnapshotArgs a) {
-  const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
-  if (i >= a.n) return;
-  const double r[3] = {a.fin[0][i], a.fin[1][i], a.fin[2][i]};
-  const double v[3] = {a.fin[3][i], a.fin[4][i], a.fin[5][i]};
-  a.out_flag[i] = a.fin_flag[i];
-  a.out_rstep[i] = a.fin_rstep[i];
-  if (a.kind == GLISSE_SNAPSHOT_CARTESIAN) {
-    a.out[0][i] = r[0]; a.out[1][i] = r[1]; a.out[2][i] = r[2];
-    a.out[3][i] = v[0]; a.out[4][i] = v[1]; a.out[5][i] = v[2];
-    return;
-  }
-  const double mu = a.mu;
+// osculating elements of (r, v) about mu -> el[0..5] = a, e, i, Omega, omega, M
+__device__ __forceinline__ void elements_of(double mu, const double (&r)[3], const double (&v)[3], double (&el)[6]) {
   const double R = sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
   const double V2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
   const double rv = r[0] * v[0] + r[1] * v[1] + r[2] * v[2];
@@ -77,8 +66,51 @@ __global__ void __launch_bounds__(256) snapshot_kernel(SnapshotArgs a) {
       M = __longlong_as_double(0x7ff8000000000000LL);
     }
   }
-  a.out[0][i] = sma; a.out[1][i] = e; a.out[2][i] = inc;
-  a.out[3][i] = Omega; a.out[4][i] = omega; a.out[5][i] = M;
+  el[0] = sma; el[1] = e; el[2] = inc; el[3] = Omega; el[4] = omega; el[5] = M;
+}
+
+__global__ void __launch_bounds__(256) snapshot_kernel(SnapshotArgs a) {
+  const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= a.n) return;
+  const double r[3] = {a.fin[0][i], a.fin[1][i], a.fin[2][i]};
+  const double v[3] = {a.fin[3][i], a.fin[4][i], a.fin[5][i]};
+  a.out_flag[i] = a.fin_flag[i];
+  a.out_rstep[i] = a.fin_rstep[i];
+  if (a.kind == GLISSE_SNAPSHOT_CARTESIAN) {
+    a.out[0][i] = r[0]; a.out[1][i] = r[1]; a.out[2][i] = r[2];
+    a.out[3][i] = v[0]; a.out[4][i] = v[1]; a.out[5][i] = v[2];
+    return;
+  }
+  double el[6];
+  elements_of(a.mu, r, v, el);
+#pragma unroll
+  for (int k = 0; k < 6; ++k) a.out[k][i] = el[k];
+}
+
+// Resonant-argument reduction: phi = p lambda − q lambda_pl − (p − q) varpi with
+// lambda = Omega + omega + M, varpi = Omega + omega, for every ACTIVE particle at the current step;
+// seen0 / seen180 record whether phi has ever come within `window` of 0 or of pi ("librating
+// particles [are] those with a resonant argument that never comes within 10 deg of 0 deg or never
+// within 10 deg of 180 deg").  The planet's elements are about gm_star + gm_planet.
+__global__ void __launch_bounds__(256) resonance_kernel(ResonanceArgs a) {
+  const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= a.n || a.fin_flag[i] != 0) return;
+  const double rp[3] = {a.planet_q[0], a.planet_q[1], a.planet_q[2]};
+  const double vp[3] = {a.planet_qd[0], a.planet_qd[1], a.planet_qd[2]};
+  double pl[6], el[6];
+  elements_of(a.mu_planet, rp, vp, pl);
+  const double r[3] = {a.fin[0][i], a.fin[1][i], a.fin[2][i]};
+  const double v[3] = {a.fin[3][i], a.fin[4][i], a.fin[5][i]};
+  elements_of(a.mu, r, v, el);
+  const double varpi = el[3] + el[4];
+  const double lambda = varpi + el[5];
+  const double lambda_pl = pl[3] + pl[4] + pl[5];
+  const double phi = wrap_2pi(a.p * lambda - a.q * lambda_pl - (a.p - a.q) * varpi);
+  a.phi[i] = phi;
+  const double d0 = fmin(phi, kTwoPiS - phi);          // angular distance to 0
+  const double d180 = fabs(phi - 0.5 * kTwoPiS);       // angular distance to pi
+  if (d0 < a.window) a.seen0[i] = 1;
+  if (d180 < a.window) a.seen180[i] = 1;
 }
 
 }  // namespace
@@ -86,6 +118,12 @@ __global__ void __launch_bounds__(256) snapshot_kernel(SnapshotArgs a) {
 cudaError_t launch_snapshot(const SnapshotArgs& a, cudaStream_t s) {
   const int blocks = static_cast<int>((a.n + 255) / 256);
   snapshot_kernel<<<blocks, 256, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_resonance(const ResonanceArgs& a, cudaStream_t s) {
+  const int blocks = static_cast<int>((a.n + 255) / 256);
+  resonance_kernel<<<blocks, 256, 0, s>>>(a);
   return cudaGetLastError();
 }
 

@@ -652,3 +652,49 @@ def test_several_sims_share_the_device_and_the_pools(gl):
     for out, ref in zip(outs, (ref1, ref2, ref1, ref2)):
         for a, b in zip(out, ref):
             assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------------------------------------------
+# resonant-argument reduction
+# ---------------------------------------------------------------------------------------------------
+def test_resonance_reduction_matches_oracle(gl, oracle_mod):
+    """phi_31 with Neptune on config 3's particles (a in 53-65 AU spans the 3:1 at 62.6 AU): at every
+    sample the device's phi must equal the oracle's phi of the SAME state (read back), and the
+    seen-near-0 / seen-near-180 record must be the OR over the samples of the oracle's window tests
+    (particles sitting within 1e-9 rad of a window edge at some sample are excluded)."""
+    w = inputs.config(3, n_particles=3000)
+    window = np.deg2rad(10.0)
+    nep = 3
+    mu_pl = w.gm_star + w.gm_planet[nep]
+    S = gl.GlisseSim.from_workload(w, chunk_steps=100)
+    assert gl.lib().glisse_resonance_sample(S._h) == gl.EINVAL          # no begin yet
+    assert gl.lib().glisse_resonance_begin(S._h, 4, 3, 1, window) == gl.EINVAL
+    assert gl.lib().glisse_resonance_begin(S._h, nep, 1, 1, window) == gl.EINVAL
+    S.resonance_begin(nep, 3, 1, window)
+    seen0 = np.zeros(w.n_particles, bool)
+    seen180 = np.zeros(w.n_particles, bool)
+    edge = np.zeros(w.n_particles, bool)
+    worst = 0.0
+    for k in range(12):
+        S.advance(170)
+        S.resonance_sample()
+        _, _, phi, ns = S.resonance_read()
+        pos, vel, flag, _ = S.read()
+        qp, qv = S.read_planets()
+        ref = oracle_mod.resonant_argument(w.gm_star, pos, vel, mu_pl, qp[nep], qv[nep], 3, 1)
+        act = flag == 0
+        el = oracle_mod.elements(w.gm_star, pos, vel)
+        d = np.abs((phi - ref + np.pi) % (2 * np.pi) - np.pi)
+        worst = max(worst, np.max((d * el[1])[act]))      # M and omega are conditioned by e
+        d0 = np.minimum(ref, 2 * np.pi - ref)
+        d180 = np.abs(ref - np.pi)
+        seen0 |= act & (d0 < window)
+        seen180 |= act & (d180 < window)
+        edge |= (np.abs(d0 - window) < 1e-9) | (np.abs(d180 - window) < 1e-9)
+        assert ns == k + 1
+    s0, s180, _, _ = S.resonance_read()
+    S.close()
+    assert worst < 1e-11, worst
+    ok = ~edge
+    assert np.array_equal(s0.astype(bool)[ok], seen0[ok]) and np.array_equal(s180.astype(bool)[ok], seen180[ok])
+    assert seen0.any() and seen180.any() and (~seen0).any()

@@ -509,3 +509,33 @@ def test_T9_elements_special_cases_and_drift_invariance(oracle_mod):
     assert np.allclose(e0[:5], e1[:5], rtol=0, atol=2e-13)
     n = np.sqrt(mu / 25.0 ** 3)
     assert abs(angle_diff(e1[5], e0[5] + n * 180.0)) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------------
+# T10  resonant argument against its formula on constructed states, and constant
+#      at exact commensurability
+# ---------------------------------------------------------------------------------------------------
+def test_T10_resonant_argument(oracle_mod):
+    mu, mu_pl = inputs.G, inputs.G * (1.0 + 5.1514e-5)
+    rng = np.random.default_rng(10)
+    for p, q in ((3, 1), (5, 2), (3, 2)):
+        for _ in range(100):
+            e, inc, Om, om, f = rng.uniform(0.05, 0.6), rng.uniform(0.1, 1.0), *rng.uniform(0, 2 * np.pi, 3)
+            r, v, M = _state_from_elements(mu, 62.6, e, inc, Om, om, f)
+            ep, ip, Op, wp, fp = 0.01, 0.03, *rng.uniform(0, 2 * np.pi, 3)
+            rp, vp, Mp = _state_from_elements(mu_pl, 30.1, ep, ip, Op, wp, fp)
+            phi = oracle_mod.resonant_argument(mu, r[:, None], v[:, None], mu_pl, rp, vp, p, q)[0]
+            want = (p * (Om + om + M) - q * (Op + wp + Mp) - (p - q) * (Om + om)) % (2 * np.pi)
+            assert angle_diff(phi, want) < 1e-10 / ep, (p, q)
+    # exact 3:1 commensurability, no interaction: phi-dot = 3 n − n_pl = 0, so phi stays put while both
+    # bodies run round their Kepler orbits under the oracle's drift
+    a_pl = 30.1
+    a = a_pl * (3.0 ** 2 * mu / mu_pl) ** (1.0 / 3.0)      # 3 sqrt(mu/a^3) = sqrt(mu_pl/a_pl^3)
+    r, v, _ = _state_from_elements(mu, a, 0.3, 0.2, 1.0, 2.0, 0.5)
+    rp, vp, _ = _state_from_elements(mu_pl, a_pl, 0.01, 0.03, 0.3, 0.7, 4.0)
+    phi0 = oracle_mod.resonant_argument(mu, r[:, None], v[:, None], mu_pl, rp, vp, 3, 1)[0]
+    for _ in range(200):
+        _, r, v = oracle_mod.kepler_drift(mu, r, v, 180.0)
+        _, rp, vp = oracle_mod.kepler_drift(mu_pl, rp, vp, 180.0)
+    phi1 = oracle_mod.resonant_argument(mu, r[:, None], v[:, None], mu_pl, rp, vp, 3, 1)[0]
+    assert angle_diff(phi1, phi0) < 1e-9
