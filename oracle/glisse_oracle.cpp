@@ -15,7 +15,9 @@
  * Kepler orbit (T2), finite-difference gradient of H_int vs the planet kick (T3), CR3BP Jacobi
  * constant bounded and O(dt^2) (T4), time reversal (T5), order-2 convergence to a brute-force
  * high-order direct integration (T6), the paper's 5-iteration / 1e-14 claim (T7),
- * removal logic on crafted inputs (T8).  Parity unpinned: none of the functions below; the
+ * removal logic on crafted inputs (T8), osculating elements against the textbook perifocal
+ * construction (T9), resonant argument against its formula and constant at exact commensurability
+ * (T10).  Parity unpinned: none of the functions below; the
  * paper's application-level numbers (10.8 % librators …) are unpinned because the authors'
  * initial conditions are not available.
  *
