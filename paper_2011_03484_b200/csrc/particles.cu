@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   double x[P], y[P], z[P], vx[P], vy[P], vz[P];
   int flag[P];
   bool was_alive[P], alive[P];
-  long long rs[P];
+  int rs[P];   // record index (within this launch) at which the particle was flagged, −1 = not yet
   bool any_alive_t = false;
 #pragma unroll
   for (int p = 0; p < P; ++p) {
@@ -97,7 +97,6 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
     rs[p] = -1;
   }
   if (!__any_sync(kFullMask, any_alive_t)) return;  // nothing to do in this warp: leave before any copy
-  unsigned drifts = 0;
 
   // ---- warp-private ring ------------------------------------------------------------------------
   double* ring = reinterpret_cast<double*>(smem_raw) + static_cast<size_t>(warp) * kRingSlots * stage_doubles;
@@ -186,7 +185,7 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
       for (int p = 0; p < P; ++p) {
         if (alive[p] && hit[p] != 0) {
           flag[p] = hit[p];
-          rs[p] = a.step0 + k;
+          rs[p] = k;
           alive[p] = false;
         }
         if (alive[p]) {
@@ -199,14 +198,12 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
       // ---- a5/a6: drift (O2) --------------------------------------------------------------------
       if (k < nsteps) {
         int st_d[P];
-#pragma unroll
-        for (int p = 0; p < P; ++p) drifts += alive[p] ? 1u : 0u;
         kepler_drift_warp<P>(alive, a.mu, a.inv_mu, a.inv_mu_dt, a.iters, a.tol, r2, x, y, z, vx, vy, vz, st_d);
 #pragma unroll
         for (int p = 0; p < P; ++p) {
           if (st_d[p] != 0) {
             flag[p] = st_d[p];
-            rs[p] = a.step0 + k;
+            rs[p] = k;
             alive[p] = false;
           }
         }
@@ -242,9 +239,19 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
       a.st[3][i] = vx[p]; a.st[4][i] = vy[p]; a.st[5][i] = vz[p];
       if (flag[p] != 0) {
         a.flag[i] = flag[p];
-        a.rstep[i] = rs[p];
+        a.rstep[i] = a.step0 + rs[p];
       }
     }
+  }
+  // drifts started by this thread's particles: all nsteps for a survivor; for a particle flagged at
+  // record k, k if a force-evaluation test caught it and k + 1 if its drift did (flags 3 and 4)
+  unsigned drifts = 0;
+#pragma unroll
+  for (int p = 0; p < P; ++p) {
+    if (was_alive[p])
+      drifts += flag[p] == 0 ? static_cast<unsigned>(nsteps)
+                             : static_cast<unsigned>(rs[p]) +
+                                   ((flag[p] == GLISSE_FLAG_NONCONV || flag[p] == GLISSE_FLAG_UNBOUND) ? 1u : 0u);
   }
   unsigned tot = __reduce_add_sync(kFullMask, drifts);
   if (lane == 0 && tot) atomicAdd(a.pstep_counter, static_cast<unsigned long long>(tot));
