@@ -43,7 +43,7 @@ UNIT = "particle-steps/s"
 L2_FLUSH_BYTES = 256 << 20       # > 126 MB L2
 # dram__bytes_read.sum + dram__bytes_write.sum per particle-kernel launch, from the ncu --set full
 # captures under profiles/ (the kernel is ALU-bound; this only shows that state traffic is negligible)
-TRAFFIC_BYTES_PER_LAUNCH = {"c2": 6.7e6, "1m_x4": 5.4e7, "c4": 5.8e7}
+TRAFFIC_BYTES_PER_LAUNCH = {"c2": 6.9e6, "1m_x4": 5.6e7, "c4": 5.7e7}
 
 # ALGORITHMIC fp64 flops per particle-step (DFMA = 2, DADD/DMUL = 1; compares, MUFU seeds and
 # integer work = 0): SURVEY.md §8(d)'s figure for the method as the paper defines it with the two
