@@ -17,11 +17,17 @@
  *    library never throws, aborts or prints.
  *  - Units: the library is unit-agnostic; G is folded into the masses (gm = G·m).  The
  *    benchmark configurations use AU, days, solar masses with G = k² (Gaussian constant).
- *  - Pointers marked "host or device" are classified with cudaPointerGetAttributes; anything
- *    that is not device/managed memory is treated as pageable or pinned host memory.
+ *  - Pointers marked "host or device" are handed to cudaMemcpyAsync with cudaMemcpyDefault: the
+ *    driver's unified addressing tells host from device, the library never classifies them itself.
+ *    Host buffers should be pinned for the copies to overlap; pageable ones work and serialise.
  *  - Ownership: inputs are copied during glisse_create (the caller keeps its buffers); outputs
  *    are caller-allocated.  The library owns its internal device state until glisse_destroy.
- *  - Threading: one glisse_sim per host thread; no global mutable state.
+ *  - Threading: a glisse_sim must be used by one host thread at a time; different sims may be used
+ *    from different threads.  Process-wide state is limited to two caches behind one mutex: a
+ *    stream-ordered memory pool per device (a sim's arena comes from it and goes back to it) and
+ *    one pinned page of mailbox words for survivor counts.
+ *  - Measurement and test hooks (launch counter, kernel timer, FP64 probe, primitive evaluator,
+ *    solver statistics) are NOT part of this interface: include/glisse_test.h.
  */
 #ifndef GLISSE_H_
 #define GLISSE_H_
@@ -52,7 +58,8 @@ extern "C" {
 typedef struct glisse_sim glisse_sim; /* opaque */
 
 /* User-configurable quantities the paper names: Kepler iteration count (fn 5 at
- * 135), planetary chunk size, resync interval.                   */
+ * 135), planetary chunk size, resync interval, output interval
+ * (PAPER.md:121), and the iteration-count sort the paper proposes.             */
 typedef struct {
   double r_min;         /* heliocentric inner removal radius; <= 0 disables the test           */
   double r_max;         /* heliocentric outer removal radius; +inf (or <= 0) disables the test */
@@ -66,6 +73,24 @@ typedef struct {
   int    device;        /* CUDA device ordinal, default 0                                      */
   void*  stream;        /* cudaStream_t on which the particle work is enqueued, or NULL for a
                            stream owned by the library                                         */
+  int    snapshot_chunks;  /* M_s: inside glisse_advance, after every M_s-th completed chunk (a
+                           chunk completes when the step count reaches a multiple of K) write a
+                           snapshot into the ring attached with glisse_snapshot_ring; 0 = off
+                           (default).  PAPER.md:121 "copied back to the CPU after a
+                           user-configurable number of planetary chunk calculations"           */
+  int    resonance_chunks; /* M_r: likewise take a glisse_resonance_sample after every M_r-th
+                           completed chunk once glisse_resonance_begin has been called; 0 = off */
+  int    bin_iterations;   /* 1: at every resync (and once at create) survivors are ordered by the
+                           number of Kepler-solver iterations their orbit can need, hardest group
+                           first, particle-ID order within a group ("sort the
+                           particles by the expected number of iterations ... the most eccentric
+                           group would be launched first"); 0 (default): particle-ID order
+                           (PAPER.md:127).  Performance only: results are bit-identical.       */
+  int    segment_steps;    /* a chunk is issued as back-to-back launches of this many steps whose
+                           warps hand particles on through per-group completion flags, so the
+                           tail of one launch is filled by the next; default 256,
+                           0 = one launch per chunk.  Performance only, results do not depend
+                           on it                                                               */
 } glisse_params;
 
 /* Fill *p with the defaults listed above.  p == NULL is ignored. */
@@ -107,14 +132,26 @@ int glisse_create(glisse_sim** out,
 int glisse_advance(glisse_sim* sim, long long n_steps);
 
 /*
- * Test hook / external planet history ("these planetary positions could be supplied
- * using any method"): advance the PARTICLES by n_steps using a caller-supplied planet log
- * instead of the planet-history kernel.  log holds n_steps+1 records (times t_s … t_{s+n}),
- * host or device, each glisse_log_stride(n_planets) doubles:
- *   [ q_0x q_0y q_0z  q_1x … q_{Np-1}z   h0x h0y h0z   (zero padding to an even count) ]
- * with h0 = −Σ_j gm_j q_j/|q_j|³.  The internal planet state is NOT advanced.
+ * External planet history ("these planetary positions could be supplied using any
+ * method, such as interpolation from a history file"): advance the PARTICLES by n_steps using a
+ * caller-supplied planet log instead of the planet-history kernel.  log holds n_steps+1 records
+ * (times t_s ... t_{s+n}), each glisse_log_stride(n_planets) doubles:
+ *   [ q_0x q_0y q_0z  q_1x ... q_{Np-1}z   h0x h0y h0z   (zero padding to an even count) ]
+ * with h0 = -sum_j gm_j q_j/|q_j|^3, host (pinned, for the upload to overlap) or
+ * device.  ASYNCHRONOUS like glisse_advance: the log is streamed chunk by chunk through the
+ * library's two log buffers on the planet stream while the particle kernel works on the previous
+ * chunk — the paper's own double-buffered upload ("always two sets of planetary
+ * data at a time on the GPU") — with no allocation and no host synchronisation; the caller's log
+ * must stay valid until the next synchronising call (glisse_sync, glisse_read ...).
+ * The internal planet state is NOT advanced: afterwards glisse_advance, glisse_read_planets,
+ * glisse_planet_log and glisse_resonance_sample return GLISSE_EINVAL until glisse_set_planets
+ * re-seeds the planets (glisse_advance_with_log itself can be called again at once).
  */
 int glisse_advance_with_log(glisse_sim* sim, long long n_steps, const double* log);
+
+/* Re-seed the internal planet integration at the CURRENT step: heliocentric positions and
+ * velocities [n_planets][3] each, HOST.  The next glisse_advance continues from them. */
+int glisse_set_planets(glisse_sim* sim, const double* planet_pos, const double* planet_vel);
 
 /* Doubles per planet-log record: 3·(n_planets+1) rounded up to a multiple of 2 (16-byte rows
  * for bulk copies).  Returns 0 if n_planets is out of range. */
@@ -159,8 +196,28 @@ int glisse_read(glisse_sim* sim, double* const pos[3], double* const vel[3],
 #define GLISSE_SNAPSHOT_ELEMENTS  1
 int glisse_snapshot(glisse_sim* sim, int kind, double* const out[6], int* flag, long long* removal_step);
 
-/* Wait until the buffers of the last glisse_snapshot are filled.  Does not wait for the particles. */
+/* Wait until the buffers of the last glisse_snapshot — and every ring slot written so far — are
+ * filled.  Does not wait for the particles. */
 int glisse_snapshot_wait(glisse_sim* sim);
+
+/*
+ * Output ring for the periodic snapshots a long glisse_advance emits on its own (params
+ * snapshot_chunks): the k-th emitted snapshot (k = 0, 1, ...) goes to slot
+ * k mod n_slots,
+ *   data         [n_slots][6][N] doubles (kind as in glisse_snapshot), may not be NULL
+ *   flag         [n_slots][N] ints, or NULL
+ *   removal_step [n_slots][N] long longs, or NULL
+ *   slot_step    [n_slots] long longs, or NULL: the step count at which the slot's snapshot was
+ *                taken, written AFTER the slot's data (same stream), so a host that polls a
+ *                pinned slot_step[] sees complete slots without synchronising the sim
+ * all host (pinned) or device.  No host round trip: glisse_advance only enqueues.  The library
+ * never waits for the caller to consume a slot: size the ring for the snapshots of one
+ * glisse_advance call, or consume between calls.  n_slots = 0 detaches the ring.
+ * glisse_snapshots_emitted returns k (host counter).
+ */
+int glisse_snapshot_ring(glisse_sim* sim, int kind, int n_slots, double* data, int* flag, long long* removal_step,
+                         long long* slot_step);
+long long glisse_snapshots_emitted(glisse_sim* sim);
 
 /*
  * Resonant-argument reduction on the device.  For the p:q
@@ -179,12 +236,29 @@ int glisse_snapshot_wait(glisse_sim* sim);
  *                            [0, 2 pi); NaN-free only for particles sampled at least once), original
  *                            particle order, host or device, any may be NULL; *n_samples = samples
  *                            taken since begin.  Synchronises.
+ * With params.resonance_chunks = M_r > 0 the samples are taken inside glisse_advance after every
+ * M_r-th chunk, fused with the snapshot of the same chunk boundary if there is one (the elements
+ * are computed once for both).
  * GLISSE_EINVAL without a preceding begin, for planet outside [0, n_planets), or p <= q or q < 1.
+ *
+ * Libration amplitude ("a running window that diagnosed successive maxima and minima of
+ * the resonant angle and measured the difference between them"): with phi taken in [0, 2 pi) — i.e.
+ * unwrapped about pi, where the symmetric librators sit and which the asymmetric ones never leave —
+ * every sample updates, per particle, the running minimum and maximum of phi and a turning-point
+ * detector: sample k-1 is a maximum (minimum) if phi rose (fell) into it and falls (rises) out of it,
+ * equal neighbours continuing the trend; each turning point after the first yields one amplitude
+ * sample |phi_ext - phi_previous_ext| / 2.
+ *   glisse_libration_read    phi_min[N], phi_max[N] (running extrema over all samples; +inf / -inf if
+ *                            never sampled), amp_mean[N] (mean of the amplitude samples, NaN if
+ *                            none), amp_max[N] (largest, 0 if none), n_amp[N] (their number), original
+ *                            order, host or device, any may be NULL.  Synchronises.
  */
 int glisse_resonance_begin(glisse_sim* sim, int planet, int p, int q, double window);
 int glisse_resonance_sample(glisse_sim* sim);
 int glisse_resonance_read(glisse_sim* sim, unsigned char* seen0, unsigned char* seen180, double* phi_last,
                           long long* n_samples);
+int glisse_libration_read(glisse_sim* sim, double* phi_min, double* phi_max, double* amp_mean, double* amp_max,
+                          int* n_amp);
 
 /* Heliocentric planet positions and velocities at the current step, [n_planets][3] each, host
  * or device, either may be NULL.  Synchronises. */
@@ -200,33 +274,8 @@ long long glisse_step(glisse_sim* sim);
  * still active when the step began (the "useful work" of BASELINE.json's metric). Synchronises. */
 long long glisse_particle_steps(glisse_sim* sim);
 
-/* Number of kernels the library has launched for this sim so far (bench.py's gpu_launches). */
-long long glisse_launch_count(glisse_sim* sim);
-
 /* Block until all enqueued work of this sim has finished; returns its sticky status. */
 int glisse_sync(glisse_sim* sim);
-
-/* Device time in milliseconds spent in particle kernels since the last call (or since create),
- * measured with CUDA events recorded on the sim's own stream around every particle-kernel
- * launch, and the number of such launches.  Synchronises.  Used by bench.py's roofline. */
-int glisse_particle_kernel_time(glisse_sim* sim, double* ms, long long* launches);
-
-/*
- * Measure this GPU's plain FP64 FMA rate with a register-resident DFMA loop (no memory
- * traffic): returns the achieved FLOP/s (2 per DFMA) in *flops over a kernel of roughly
- * `millis` milliseconds on `device`, `stream` may be NULL.  This is the roofline denominator
- * of the ALU-bound particle kernel (MEASURED_PEAKS.json has no FP64 figure).
- */
-int glisse_fp64_peak_probe(int device, void* stream, double millis, double* flops);
-
-/*
- * Test hook: evaluate one device primitive of the CUDA path on an array, on device 0.
- * in/out are HOST or device arrays.  which = 0 rsqrt (in[n] -> out[n]), 1 reciprocal, 2 reciprocal
- * to 2^-39 (Newton updates only), 3 sin x - x and cos x - 1 (in[n] -> out[2n], interleaved),
- * 4 one Kepler drift (step a5) per body: in[10n] = {mu, dt, kepler_iters, kepler_tol, x, y, z, vx,
- * vy, vz}, out[7n] = {flag, x, y, z, vx, vy, vz}.  Synchronises.
- */
-int glisse_test_primitive(int which, long long n, const double* in, double* out);
 
 void glisse_destroy(glisse_sim* sim);
 

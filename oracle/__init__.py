@@ -70,6 +70,8 @@ def lib():
         L.oracle_resonant_argument.argtypes = [c_double, c_void_p, c_void_p, c_double, c_void_p, c_void_p,
                                                c_int, c_int]
         L.oracle_resonant_argument.restype = c_double
+        L.oracle_libration_summary.argtypes = [c_void_p, c_longlong, c_double, c_void_p]
+        L.oracle_libration_summary.restype = None
         L.oracle_kepler_drift.argtypes = [c_double, c_void_p, c_void_p, c_double, c_int, c_double]
         L.oracle_kepler_drift.restype = c_int
         L.oracle_planet_kick_accel.argtypes = [c_int, c_double, c_void_p, c_void_p, c_void_p]
@@ -208,6 +210,21 @@ def resonant_argument(mu, pos, vel, mu_pl, rp, vp, p, q):
     rp, vp = _f64(rp), _f64(vp)
     return np.array([L.oracle_resonant_argument(c_double(mu), _p(pos[k]), _p(vel[k]), c_double(mu_pl), _p(rp),
                                                 _p(vp), int(p), int(q)) for k in range(pos.shape[0])])
+
+
+def libration_summary(phi, window):
+    """Libration summary of sampled resonant arguments.  phi: [n_samples] or [n_samples, N] (time along
+    axis 0) -> dict of seen0, seen180 (bool), phi_min, phi_max, amp_mean, amp_max, n_amp per particle."""
+    L = lib()
+    phi = np.asarray(phi, dtype=np.float64)
+    one = phi.ndim == 1
+    series = np.ascontiguousarray(phi.reshape(phi.shape[0], -1).T)     # [N, n_samples]
+    out = np.empty((series.shape[0], 7))
+    for k in range(series.shape[0]):
+        L.oracle_libration_summary(_p(series[k]), series.shape[1], c_double(window), _p(out[k]))
+    d = dict(seen0=out[:, 0] != 0, seen180=out[:, 1] != 0, phi_min=out[:, 2], phi_max=out[:, 3],
+             amp_mean=out[:, 4], amp_max=out[:, 5], n_amp=out[:, 6].astype(np.int64))
+    return {k: v[0] for k, v in d.items()} if one else d
 
 
 def kepler_drift(mu, r, v, dt, iters=5, tol=1e-14):

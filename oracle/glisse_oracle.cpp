@@ -17,7 +17,8 @@
  * high-order direct integration (T6), the paper's 5-iteration / 1e-14 claim (T7),
  * removal logic on crafted inputs (T8), osculating elements against the textbook perifocal
  * construction (T9), resonant argument against its formula and constant at exact commensurability
- * (T10).  Parity unpinned: none of the functions below; the
+ * (T10), libration summary against constructed librators and hand-worked series (T11).
+ * Parity unpinned: none of the functions below; the
  * paper's application-level numbers (10.8 % librators …) are unpinned because the authors'
  * initial conditions are not available.
  *
@@ -25,6 +26,7 @@
  * PAPER.md:87); q_j, qd_j heliocentric planet position / velocity; r, v heliocentric particle
  * position / velocity; dt the fixed step.
  */
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -568,6 +570,57 @@ double oracle_resonant_argument(double mu, const double* r, const double* v, dou
   double phi = std::fmod(p * lambda - q * lambda_pl - (p - q) * varpi, 2.0 * M_PI);
   if (phi < 0.0) phi += 2.0 * M_PI;
   return phi;
+}
+
+/* Libration summary of one particle's sampled resonant argument.
+ * phi[0..n) are the samples in [0, 2 pi), in time order.
+ *   - window test ("never comes within 10 deg of 0 deg or never within 10 deg of 180 deg"):
+ *     seen0 = some sample lies within `window` of 0 (or 2 pi), seen180 = within `window` of pi;
+ *   - running extrema: the smallest and largest sample;
+ *   - amplitude ("a running window that diagnosed successive maxima and minima of the
+ *     resonant angle and measured the difference between them"): sample k (0 < k < n-1) is a turning
+ *     point if the series rose into it and falls out of it (a maximum) or fell into it and rises out of
+ *     it (a minimum), where "rose / fell into it" looks back past equal neighbours to the last change;
+ *     every turning point after the first gives one amplitude sample, half its distance to the turning
+ *     point before it.  out = { seen0, seen180, phi_min, phi_max, amp_mean (NaN if none), amp_max (0 if
+ *     none), number of amplitude samples }. */
+void oracle_libration_summary(const double* phi, long long n, double window, double* out) {
+  const double two_pi = 2.0 * M_PI;
+  double seen0 = 0.0, seen180 = 0.0;
+  double lo = std::numeric_limits<double>::infinity(), hi = -std::numeric_limits<double>::infinity();
+  for (long long k = 0; k < n; ++k) {
+    const double to_zero = std::min(phi[k], two_pi - phi[k]);
+    const double to_pi = std::fabs(phi[k] - M_PI);
+    if (to_zero < window) seen0 = 1.0;
+    if (to_pi < window) seen180 = 1.0;
+    lo = std::min(lo, phi[k]);
+    hi = std::max(hi, phi[k]);
+  }
+  std::vector<double> turning; /* values of the turning points, in time order */
+  for (long long k = 1; k + 1 < n; ++k) {
+    /* direction of the last change before sample k (0 if the series has been flat so far) */
+    int into = 0;
+    for (long long j = k; j >= 1 && into == 0; --j) {
+      if (phi[j] > phi[j - 1]) into = 1;
+      if (phi[j] < phi[j - 1]) into = -1;
+    }
+    int out_of = 0;
+    if (phi[k + 1] > phi[k]) out_of = 1;
+    if (phi[k + 1] < phi[k]) out_of = -1;
+    if (into != 0 && out_of == -into) turning.push_back(phi[k]);
+  }
+  double sum = 0.0, largest = 0.0;
+  long long count = 0;
+  for (size_t t = 1; t < turning.size(); ++t) {
+    const double amp = 0.5 * std::fabs(turning[t] - turning[t - 1]);
+    sum += amp;
+    largest = std::max(largest, amp);
+    count += 1;
+  }
+  out[0] = seen0; out[1] = seen180; out[2] = lo; out[3] = hi;
+  out[4] = count > 0 ? sum / static_cast<double>(count) : std::numeric_limits<double>::quiet_NaN();
+  out[5] = largest;
+  out[6] = static_cast<double>(count);
 }
 
 }  // extern "C"

@@ -20,21 +20,27 @@ from . import build as _build
 OK, EINVAL, ECUDA, ENOMEM, EPLANET = 0, -1, -2, -3, -4
 FLAG_ACTIVE, FLAG_RMIN, FLAG_RMAX, FLAG_NONCONV, FLAG_UNBOUND, FLAG_PLANET0 = 0, 1, 2, 3, 4, 16
 
-#: every symbol include/glisse.h declares (tests check that the library exports each one)
+#: every symbol include/glisse.h declares (tests check that the library exports each one) ...
 EXPORTS = (
-    "glisse_default_params", "glisse_create", "glisse_advance", "glisse_advance_with_log",
+    "glisse_default_params", "glisse_create", "glisse_advance", "glisse_advance_with_log", "glisse_set_planets",
     "glisse_log_stride", "glisse_planet_log", "glisse_read", "glisse_read_planets",
-    "glisse_snapshot", "glisse_snapshot_wait",
-    "glisse_resonance_begin", "glisse_resonance_sample", "glisse_resonance_read",
-    "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_launch_count", "glisse_sync",
-    "glisse_particle_kernel_time", "glisse_fp64_peak_probe", "glisse_test_primitive", "glisse_destroy",
+    "glisse_snapshot", "glisse_snapshot_wait", "glisse_snapshot_ring", "glisse_snapshots_emitted",
+    "glisse_resonance_begin", "glisse_resonance_sample", "glisse_resonance_read", "glisse_libration_read",
+    "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_sync", "glisse_destroy",
     "glisse_strerror",
+)
+#: ... and the measurement / test hooks of include/glisse_test.h
+TEST_EXPORTS = (
+    "glisse_launch_count", "glisse_particle_kernel_time", "glisse_fp64_peak_probe", "glisse_test_primitive",
+    "glisse_solver_stats_enable", "glisse_solver_stats",
 )
 
 
 class GlisseParams(ctypes.Structure):
     _fields_ = [("r_min", c_double), ("r_max", c_double), ("kepler_iters", c_int), ("kepler_tol", c_double),
-                ("chunk_steps", c_int), ("resync_chunks", c_int), ("device", c_int), ("stream", c_void_p)]
+                ("chunk_steps", c_int), ("resync_chunks", c_int), ("device", c_int), ("stream", c_void_p),
+                ("snapshot_chunks", c_int), ("resonance_chunks", c_int), ("bin_iterations", c_int),
+                ("segment_steps", c_int)]
 
 
 class GlisseError(RuntimeError):
@@ -66,6 +72,18 @@ def lib():
         L.glisse_advance.restype = c_int
         L.glisse_advance_with_log.argtypes = [c_void_p, c_longlong, c_void_p]
         L.glisse_advance_with_log.restype = c_int
+        L.glisse_set_planets.argtypes = [c_void_p, c_void_p, c_void_p]
+        L.glisse_set_planets.restype = c_int
+        L.glisse_snapshot_ring.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.glisse_snapshot_ring.restype = c_int
+        L.glisse_snapshots_emitted.argtypes = [c_void_p]
+        L.glisse_snapshots_emitted.restype = c_longlong
+        L.glisse_libration_read.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.glisse_libration_read.restype = c_int
+        L.glisse_solver_stats_enable.argtypes = [c_void_p, c_int]
+        L.glisse_solver_stats_enable.restype = c_int
+        L.glisse_solver_stats.argtypes = [c_void_p, POINTER(c_longlong), POINTER(c_longlong), POINTER(c_longlong)]
+        L.glisse_solver_stats.restype = c_int
         L.glisse_log_stride.argtypes = [c_int]
         L.glisse_log_stride.restype = c_int
         L.glisse_planet_log.argtypes = [c_void_p, c_longlong, c_void_p]
@@ -150,7 +168,8 @@ class GlisseSim:
 
     def __init__(self, gm_star, gm_planet, planet_pos, planet_vel, planet_rcrit, pos, vel, dt, *, r_min=0.0,
                  r_max=float("inf"), kepler_iters=5, kepler_tol=1e-14, chunk_steps=1024, resync_chunks=1,
-                 device=0, stream=None):
+                 device=0, stream=None, snapshot_chunks=0, resonance_chunks=0, bin_iterations=0,
+                 segment_steps=None):
         L = lib()
         gm_planet = np.ascontiguousarray(gm_planet, dtype=np.float64).reshape(-1)
         self.n_planets = int(gm_planet.shape[0])
@@ -169,6 +188,10 @@ class GlisseSim:
         prm.chunk_steps, prm.resync_chunks = int(chunk_steps), int(resync_chunks)
         prm.device = self.device
         prm.stream = None if stream is None else c_void_p(int(stream))
+        prm.snapshot_chunks, prm.resonance_chunks = int(snapshot_chunks), int(resonance_chunks)
+        prm.bin_iterations = int(bin_iterations)
+        if segment_steps is not None:
+            prm.segment_steps = int(segment_steps)
         h = c_void_p()
         st = L.glisse_create(byref(h), float(gm_star), self.n_planets, _ptr(gm_planet), _ptr(planet_pos),
                              _ptr(planet_vel), _ptr(rcrit), self.n, _p3(prow), _p3(vrow), float(dt), byref(prm))
@@ -191,6 +214,11 @@ class GlisseSim:
             log = np.ascontiguousarray(log, dtype=np.float64)
         assert log.shape[0] >= n_steps + 1
         _check(lib().glisse_advance_with_log(self._h, int(n_steps), _ptr(log)), "glisse_advance_with_log")
+
+    def set_planets(self, planet_pos, planet_vel):
+        pp = np.ascontiguousarray(planet_pos, dtype=np.float64).reshape(self.n_planets, 3)
+        pv = np.ascontiguousarray(planet_vel, dtype=np.float64).reshape(self.n_planets, 3)
+        _check(lib().glisse_set_planets(self._h, _ptr(pp), _ptr(pv)), "glisse_set_planets")
 
     def planet_log(self, n_steps):
         out = np.zeros((int(n_steps) + 1, log_stride(self.n_planets)), dtype=np.float64)
@@ -239,6 +267,45 @@ class GlisseSim:
     def snapshot_wait(self):
         _check(lib().glisse_snapshot_wait(self._h), "glisse_snapshot_wait")
         self._snap_keep = None
+
+    def snapshot_ring(self, kind, n_slots, data=None, flag=None, removal_step=None, slot_step=None):
+        """glisse_snapshot_ring: attach the output ring of the periodic snapshots (params
+        snapshot_chunks).  data [n_slots, 6, N] float64 (+ optional flag [n_slots, N] int32, removal_step
+        [n_slots, N] int64, slot_step [n_slots] int64): numpy (pinned) or torch CUDA; allocated
+        (pageable numpy) when data is None.  Returns the arrays; they are kept alive by the sim."""
+        k = {"cartesian": 0, "elements": 1}[kind]
+        if data is None and n_slots > 0:
+            data = np.empty((n_slots, 6, self.n), dtype=np.float64)
+            flag = np.empty((n_slots, self.n), dtype=np.int32)
+            removal_step = np.empty((n_slots, self.n), dtype=np.int64)
+            slot_step = np.full(n_slots, -1, dtype=np.int64)
+        _check(lib().glisse_snapshot_ring(self._h, k, int(n_slots), _ptr(data), _ptr(flag), _ptr(removal_step),
+                                          _ptr(slot_step)), "glisse_snapshot_ring")
+        self._ring_keep = (data, flag, removal_step, slot_step)
+        return data, flag, removal_step, slot_step
+
+    def snapshots_emitted(self):
+        return self._count(lib().glisse_snapshots_emitted, "glisse_snapshots_emitted")
+
+    def libration_read(self):
+        """(phi_min[N], phi_max[N], amp_mean[N], amp_max[N], n_amp[N] int32)"""
+        lo = np.empty(self.n, dtype=np.float64)
+        hi = np.empty(self.n, dtype=np.float64)
+        mean = np.empty(self.n, dtype=np.float64)
+        amax = np.empty(self.n, dtype=np.float64)
+        cnt = np.empty(self.n, dtype=np.int32)
+        _check(lib().glisse_libration_read(self._h, _ptr(lo), _ptr(hi), _ptr(mean), _ptr(amax), _ptr(cnt)),
+               "glisse_libration_read")
+        return lo, hi, mean, amax, cnt
+
+    def solver_stats_enable(self, on=True):
+        _check(lib().glisse_solver_stats_enable(self._h, 1 if on else 0), "glisse_solver_stats_enable")
+
+    def solver_stats(self):
+        """(warp drift calls, fast-solver iterations summed over them, calls that entered the slow path)"""
+        a, b, c = c_longlong(), c_longlong(), c_longlong()
+        _check(lib().glisse_solver_stats(self._h, byref(a), byref(b), byref(c)), "glisse_solver_stats")
+        return a.value, b.value, c.value
 
     def resonance_begin(self, planet, p, q, window):
         _check(lib().glisse_resonance_begin(self._h, int(planet), int(p), int(q), float(window)),

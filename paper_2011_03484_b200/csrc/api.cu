@@ -12,6 +12,7 @@
 #include <new>
 #include <vector>
 
+#include "../../include/glisse_test.h"
 #include "glisse_internal.cuh"
 
 using namespace glisse;
@@ -59,6 +60,7 @@ cudaError_t arena_pool(int dev, cudaMemPool_t* out) {
 // The pinned word through which a sim's survivor count comes back: handed out from one pinned page
 // per process (cudaMallocHost/cudaFreeHost per sim cost ~0.2 ms).
 constexpr int kPinnedWords = 1024;
+constexpr int kRingStepWords = 64;   // slot_step copies that may be in flight at once
 int* g_pinned = nullptr;
 std::vector<int> g_pinned_free;
 
@@ -101,13 +103,15 @@ struct glisse_sim {
   int status = GLISSE_OK;  // sticky
 
   PlanetSystem* d_sys = nullptr;
-  double* d_j0 = nullptr;  // Jacobi state at create
+  double* d_j0 = nullptr;    // Jacobi state the planet clock was (re-)seeded with
   double* d_ptmp = nullptr;  // [6 Np] scratch: heliocentric planet state in / out
+  long long* d_fail = nullptr;  // [2] first failed planet step: [0] the sim's clock, [1] scratch of glisse_planet_log
   LogBuffer buf[2];
   int cur = 0;
   bool ahead = false;  // buf[cur ^ 1] holds (or is being filled with) the chunk after buf[cur]'s
   long long step = 0;
-  bool external_log_used = false;
+  long long origin = 0;        // step at which the planet clock was (re-)seeded: chunks are counted from it
+  bool planets_stale = false;  // an external log moved the particles past the internal planet clock
 
   // particle state: two working sets (ping-pong for compaction) + original-order assembly arrays
   double* work[2][6] = {};
@@ -119,12 +123,21 @@ struct glisse_sim {
   long long* fin_rstep = nullptr;
   int* d_nslots = nullptr;  // [2], indexed like the working sets
   int* d_block_counts = nullptr;
+  unsigned char* d_bin = nullptr;
   int w = 0;                // working set in use
   int nslots_upper = 0;     // host upper bound of d_nslots[w]
   int* h_nslots = nullptr;  // pinned
   cudaEvent_t nslots_ready = nullptr;
   bool nslots_pending = false;
-  int chunks_since_resync = 0;
+
+  // launch chain of the particle kernel (particles.cu): completion lists and tickets, by launch parity
+  int* d_list[2] = {};
+  unsigned* d_ticket = nullptr;   // [2]
+  int* d_error = nullptr;
+  int chain_len = 0;              // launches in the open chain (0 = the next launch starts one)
+  int chain_groups = 0;
+  bool stats_on = false;
+  unsigned long long* d_stats = nullptr;  // [3]
 
   // snapshot staging (glisse_snapshot): a copy in original order that stream r ships to the caller
   double* snap[6] = {};
@@ -134,11 +147,19 @@ struct glisse_sim {
   cudaEvent_t snap_ready = nullptr;    // staging written            (stream Q)
   cudaEvent_t snap_done = nullptr;     // staging copied to the caller (stream R)
   bool snap_in_flight = false;
+  // output ring (glisse_snapshot_ring)
+  int ring_kind = 0, ring_slots = 0;
+  double* ring_data = nullptr;
+  int* ring_flag = nullptr;
+  long long* ring_rstep = nullptr;
+  long long* ring_step = nullptr;
+  long long ring_emitted = 0;
+  long long* h_ring_steps = nullptr;   // pinned [kRingStepWords]: sources of the slot_step copies
+  int ring_step_next = 0;
 
   // resonant-argument record (glisse_resonance_*), original order
-  double* res_phi = nullptr;
-  unsigned char* res_seen0 = nullptr;
-  unsigned char* res_seen180 = nullptr;
+  LibrationRecord lib{};
+  double* d_amp_mean = nullptr;
   int res_planet = -1, res_p = 0, res_q = 0;
   double res_window = 0.0;
   long long res_samples = 0;
@@ -198,6 +219,7 @@ void free_sim(glisse_sim* s) {
   if (s->snap_ready) cudaEventDestroy(s->snap_ready);
   if (s->snap_done) cudaEventDestroy(s->snap_done);
   if (s->r) cudaStreamDestroy(s->r);
+  if (s->h_ring_steps) cudaFreeHost(s->h_ring_steps);
   for (int b = 0; b < 2; ++b) {
     if (s->buf[b].ready) cudaEventDestroy(s->buf[b].ready);
     if (s->buf[b].consumed) cudaEventDestroy(s->buf[b].consumed);
@@ -238,6 +260,15 @@ void harvest_timings(glisse_sim* s, bool block) {
   s->timed_busy.resize(kept);
 }
 
+// Anything other than a particle-kernel launch that is enqueued on stream q ends the open launch chain:
+// the next particle launch is an ordinary one (full stream order) and starts a new chain.
+void break_chain(glisse_sim* s) { s->chain_len = 0; }
+
+// Advance every slot of the working set by `nsteps` steps with the planet log at `log` (record 0 = the
+// current step).  Issued as back-to-back launches of prm.segment_steps steps; all but the first of a
+// chain ask for programmatic stream serialisation and take their particle groups from the completion
+// list of the launch before (particles.cu), so the device stays full while a launch drains.  The whole
+// run is bracketed by one pair of timing events (the launches overlap by design).
 int launch_particles(glisse_sim* s, const double* log, int nsteps) {
   ParticleArgs& a = s->pa;
   const int w = s->w;
@@ -245,15 +276,16 @@ int launch_particles(glisse_sim* s, const double* log, int nsteps) {
   a.flag = s->flag[w];
   a.rstep = s->rstep[w];
   a.n_slots = s->d_nslots + w;
-  a.log = log;
-  a.step0 = s->step;
-  a.nsteps = nsteps;
   // a newer survivor count may have arrived from the last compaction: shrink the grid (never blocks)
   if (s->nslots_pending && cudaEventQuery(s->nslots_ready) == cudaSuccess) {
     s->nslots_upper = *s->h_nslots;
     s->nslots_pending = false;
   }
   (void)cudaGetLastError();
+  const int per_group = particles_per_group();
+  const int groups = std::max(1, (s->nslots_upper + per_group - 1) / per_group);
+  if (groups != s->chain_groups) break_chain(s);
+
   TimedLaunch t{};
   bool timed = false;
   if (s->timed_free.empty() && s->timed_busy.size() >= 256) harvest_timings(s, false);
@@ -264,17 +296,42 @@ int launch_particles(glisse_sim* s, const double* log, int nsteps) {
   } else if (s->timed_busy.size() < 256) {
     if (cudaEventCreate(&t.t0) == cudaSuccess && cudaEventCreate(&t.t1) == cudaSuccess) timed = true;
   }
-  if (timed) cudaEventRecord(t.t0, s->q);
-  CKS(s, launch_particle_kernel(a, s->nslots_upper, s->q));
-  s->launches += 1;
+  if (timed) {
+    cudaEventRecord(t.t0, s->q);
+    break_chain(s);   // an event record sits between this run and the launch before it
+  }
+  const int seg = s->prm.segment_steps > 0 ? s->prm.segment_steps : nsteps;
+  for (int off = 0; off < nsteps; off += seg) {
+    const int m = std::min(seg, nsteps - off);
+    const bool first = s->chain_len == 0;
+    if (first) {  // a new chain: clear both completion lists and tickets
+      CKS(s, cudaMemsetAsync(s->d_list[0], 0, sizeof(int) * groups, s->q));
+      CKS(s, cudaMemsetAsync(s->d_list[1], 0, sizeof(int) * groups, s->q));
+      CKS(s, cudaMemsetAsync(s->d_ticket, 0, 2 * sizeof(unsigned), s->q));
+      s->chain_groups = groups;
+    }
+    const int par = s->chain_len & 1;
+    a.wait_list = first ? nullptr : s->d_list[par ^ 1];
+    a.done_list = s->d_list[par];
+    a.done_ticket = s->d_ticket + par;
+    a.ticket_base = static_cast<unsigned>(s->chain_len >> 1) * static_cast<unsigned>(groups);
+    a.log = log + static_cast<size_t>(off) * s->stride;
+    a.step0 = s->step + off;
+    a.nsteps = m;
+    CKS(s, launch_particle_kernel(a, groups, !first, s->stats_on, s->q));
+    s->launches += 1;
+    s->chain_len += 1;
+  }
   if (timed) {
     cudaEventRecord(t.t1, s->q);
+    break_chain(s);
     s->timed_busy.push_back(t);
   }
   return GLISSE_OK;
 }
 
 int run_compaction(glisse_sim* s) {
+  break_chain(s);
   const int w = s->w, o = w ^ 1;
   CompactArgs c{};
   for (int k = 0; k < 6; ++k) {
@@ -289,35 +346,39 @@ int run_compaction(glisse_sim* s) {
   c.n_in = s->d_nslots + w;
   c.n_out = s->d_nslots + o;
   c.block_counts = s->d_block_counts;
+  c.bin = s->d_bin;
+  c.bins = s->prm.bin_iterations ? kCompactBins : 1;
+  c.mu = s->gm0;
+  c.dt = s->dt;
   CKS(s, launch_compaction(c, s->nslots_upper, s->q, &s->launches));
   s->w = o;
-  // survivor count to the host without blocking; the next launches use it once it has arrived
-  if (s->nslots_pending) {
-    // an older copy may still be in flight into the same pinned word: order behind it on stream q
-  }
+  // survivor count to the host without blocking (stream order keeps an older copy into the same pinned
+  // word ahead of this one); the next launches use it once it has arrived
   CKS(s, cudaMemcpyAsync(s->h_nslots, s->d_nslots + o, sizeof(int), cudaMemcpyDeviceToHost, s->q));
   CKS(s, cudaEventRecord(s->nslots_ready, s->q));
   s->nslots_pending = true;
-  s->chunks_since_resync = 0;
   return GLISSE_OK;
 }
 
-// Steps in the log buffer that starts at step `start`.  The first chunk is cut into pieces of 64, 64,
-// 128, 256, ... steps (summing to K): the planet-history kernel is serial in time, so a full first
-// chunk would keep the particles waiting for K x 1.3 us before their first step; after the ramp
-// the planets stay one buffer ahead.  Results do not depend on the cut.
+// Steps in the log buffer that starts at step `start`.  The first chunk after the planet clock is
+// (re-)seeded is cut into pieces of 64, 64, 128, 256, ... steps (summing to K): the planet-history
+// kernel is serial in time, so a full first chunk would keep the particles waiting for K x 1 us before
+// their first step; after the ramp the planets stay one buffer ahead.  Results do not depend on the
+// cut.
 int buffer_len(const glisse_sim* s, long long start) {
   const int K = s->K;
-  if (K < 256 || start >= K) return K;
-  if (start == 0) return 64;
-  return static_cast<int>(std::min<long long>(start, K - start));
+  const long long rel = start - s->origin;
+  if (K < 256 || rel >= K) return K;
+  if (rel == 0) return 64;
+  return static_cast<int>(std::min<long long>(rel, K - rel));
 }
 
 // planet-history kernel into buffer b, starting from the Jacobi state `jin` at step `start`
 int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
   LogBuffer& B = s->buf[b];
   CKS(s, cudaStreamWaitEvent(s->p, B.consumed, 0));
-  CKS(s, launch_planet_kernel(s->d_sys, s->np, jin, B.log, B.jlog, buffer_len(s, start), s->dt, s->planet_smem, s->p));
+  CKS(s, launch_planet_kernel(s->d_sys, s->np, jin, B.log, B.jlog, buffer_len(s, start), s->dt, start, s->d_fail,
+                              s->planet_smem, s->p));
   B.len = buffer_len(s, start);
   s->launches += 1;
   CKS(s, cudaEventRecord(B.ready, s->p));
@@ -327,7 +388,8 @@ int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
 
 // Waits for everything the caller has asked for.  The planet stream may still be working on a chunk
 // AHEAD of the particles: that is not waited for (every chunk the particles have used is complete,
-// the particle kernel waited for it), and a planet failure in it is reported once it is used.
+// the particle kernel waited for it), and a planet failure in it concerns the caller only once the
+// particles have gone past the failed step (glisse_internal.cuh: kNoPlanetFailure).
 int sync_all(glisse_sim* s) {
   CKS(s, cudaStreamSynchronize(s->q));
   if (s->nslots_pending) {
@@ -336,10 +398,12 @@ int sync_all(glisse_sim* s) {
   }
   harvest_timings(s, true);
   if (s->status == GLISSE_OK) {
-    int pst = 0;
-    CKS(s, cudaMemcpy(&pst, reinterpret_cast<char*>(s->d_sys) + offsetof(PlanetSystem, status), sizeof(int),
-                      cudaMemcpyDeviceToHost));
-    if (pst != 0) s->status = GLISSE_EPLANET;
+    long long fail = kNoPlanetFailure;
+    int err = 0;
+    CKS(s, cudaMemcpy(&fail, s->d_fail, sizeof(fail), cudaMemcpyDeviceToHost));
+    CKS(s, cudaMemcpy(&err, s->d_error, sizeof(err), cudaMemcpyDeviceToHost));
+    if (err != 0) s->status = GLISSE_ECUDA;              // a chained warp gave up waiting (particles.cu)
+    else if (!s->planets_stale && fail < s->step) s->status = GLISSE_EPLANET;
   }
   return s->status;
 }
@@ -347,6 +411,120 @@ int sync_all(glisse_sim* s) {
 template <class T>
 cudaError_t dmalloc(T** p, size_t count) {
   return cudaMalloc(reinterpret_cast<void**>(p), (count ? count : 1) * sizeof(T));
+}
+
+ScatterArgs scatter_args(const glisse_sim* s) {
+  ScatterArgs g{};
+  const int w = s->w;
+  for (int k = 0; k < 6; ++k) {
+    g.st[k] = s->work[w][k];
+    g.fin[k] = s->fin[k];
+  }
+  g.id = s->id[w]; g.flag = s->flag[w]; g.rstep = s->rstep[w];
+  g.n_slots = s->d_nslots + w;
+  g.fin_flag = s->fin_flag; g.fin_rstep = s->fin_rstep;
+  return g;
+}
+
+int ensure_snapshot_stream(glisse_sim* s) {
+  if (!s->r) {  // first snapshot of this sim: its copy stream and events
+    CKS(s, cudaStreamCreateWithFlags(&s->r, cudaStreamNonBlocking));
+    CKS(s, cudaEventCreateWithFlags(&s->snap_ready, cudaEventDisableTiming));
+    CKS(s, cudaEventCreateWithFlags(&s->snap_done, cudaEventDisableTiming));
+  }
+  return GLISSE_OK;
+}
+
+// One sample of the state at the current step, on stream q: working order -> original order, then ONE
+// pass that writes the snapshot staging copy (if out != null) and / or updates the resonance record
+// (if resonance): the elements are computed once for both.  The staging copy is shipped to the caller's
+// buffers by stream r; `slot_step` (may be null) receives the step count after the data.
+int enqueue_sample(glisse_sim* s, bool snapshot, int kind, double* const out[6], int* flag, long long* removal_step,
+                   long long* slot_step, bool resonance) {
+  break_chain(s);
+  if (snapshot) {
+    const int st = ensure_snapshot_stream(s);
+    if (st != GLISSE_OK) return st;
+    // the staging arrays are free once the previous snapshot's copies are done (device-side wait)
+    if (s->snap_in_flight) CKS(s, cudaStreamWaitEvent(s->q, s->snap_done, 0));
+  }
+  CKS(s, launch_scatter_to_original(scatter_args(s), s->nslots_upper, s->q));
+  s->launches += 1;
+  SampleArgs a{};
+  for (int k = 0; k < 6; ++k) {
+    a.fin[k] = s->fin[k];
+    a.out[k] = s->snap[k];
+  }
+  a.fin_flag = s->fin_flag; a.fin_rstep = s->fin_rstep;
+  a.out_flag = s->snap_flag; a.out_rstep = s->snap_rstep;
+  a.n = s->n;
+  a.mu = s->gm0;
+  a.do_snapshot = snapshot ? 1 : 0;
+  a.kind = kind;
+  a.do_resonance = resonance ? 1 : 0;
+  if (resonance) {
+    // planets at the current step: heliocentric q, qd from the Jacobi state of this record
+    const int np = s->np;
+    const LogBuffer& B = s->buf[s->cur];
+    const long long off = s->step - B.start;
+    double* d_out = s->d_ptmp;
+    CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+    CKS(s, launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q));
+    s->launches += 1;
+    a.planet_q = d_out + 3 * s->res_planet;
+    a.planet_qd = d_out + 3 * np + 3 * s->res_planet;
+    a.mu_planet = s->gm0 + s->gm_planet_host[s->res_planet];
+    a.window = s->res_window;
+    a.p = s->res_p; a.q = s->res_q;
+    a.lib = s->lib;
+    s->res_samples += 1;
+  }
+  CKS(s, launch_sample(a, s->q));
+  s->launches += 1;
+  if (!snapshot) return GLISSE_OK;
+  CKS(s, cudaEventRecord(s->snap_ready, s->q));
+  // from here on the particle stream is free to go on; stream r ships the staging copy
+  CKS(s, cudaStreamWaitEvent(s->r, s->snap_ready, 0));
+  const size_t N = static_cast<size_t>(s->n);
+  for (int k = 0; k < 6; ++k)
+    if (out && out[k]) CKS(s, cudaMemcpyAsync(out[k], s->snap[k], N * sizeof(double), cudaMemcpyDefault, s->r));
+  if (flag) CKS(s, cudaMemcpyAsync(flag, s->snap_flag, N * sizeof(int), cudaMemcpyDefault, s->r));
+  if (removal_step)
+    CKS(s, cudaMemcpyAsync(removal_step, s->snap_rstep, N * sizeof(long long), cudaMemcpyDefault, s->r));
+  if (slot_step) {  // after the data, same stream: a host polling a pinned slot_step sees complete slots
+    long long* src = s->h_ring_steps + (s->ring_step_next++ % kRingStepWords);
+    *src = s->step;
+    CKS(s, cudaMemcpyAsync(slot_step, src, sizeof(long long), cudaMemcpyDefault, s->r));
+  }
+  CKS(s, cudaEventRecord(s->snap_done, s->r));
+  s->snap_in_flight = true;
+  return GLISSE_OK;
+}
+
+// What happens when the step count reaches a multiple of K (counted from the planet clock's origin): the
+// periodic outputs and the resync, each at its own interval in chunks.
+int chunk_boundary(glisse_sim* s) {
+  const long long chunk = (s->step - s->origin) / s->K;   // chunks completed
+  const glisse_params& P = s->prm;
+  const bool snap = P.snapshot_chunks > 0 && s->ring_slots > 0 && chunk % P.snapshot_chunks == 0;
+  const bool res = P.resonance_chunks > 0 && s->res_planet >= 0 && !s->planets_stale && chunk % P.resonance_chunks == 0;
+  if (snap || res) {
+    double* out[6] = {};
+    int* fl = nullptr;
+    long long *rs = nullptr, *ss = nullptr;
+    if (snap) {
+      const size_t slot = static_cast<size_t>(s->ring_emitted % s->ring_slots), N = static_cast<size_t>(s->n);
+      for (int k = 0; k < 6; ++k) out[k] = s->ring_data + (slot * 6 + k) * N;
+      if (s->ring_flag) fl = s->ring_flag + slot * N;
+      if (s->ring_rstep) rs = s->ring_rstep + slot * N;
+      if (s->ring_step) ss = s->ring_step + slot;
+    }
+    const int st = enqueue_sample(s, snap, s->ring_kind, out, fl, rs, ss, res);
+    if (st != GLISSE_OK) return st;
+    if (snap) s->ring_emitted += 1;
+  }
+  if (P.resync_chunks > 0 && chunk % P.resync_chunks == 0) return run_compaction(s);
+  return GLISSE_OK;
 }
 
 }  // namespace
@@ -363,6 +541,10 @@ void glisse_default_params(glisse_params* p) {
   p->resync_chunks = 1;
   p->device = 0;
   p->stream = nullptr;
+  p->snapshot_chunks = 0;
+  p->resonance_chunks = 0;
+  p->bin_iterations = 0;
+  p->segment_steps = 256;
 }
 
 int glisse_log_stride(int n_planets) {
@@ -403,7 +585,8 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   glisse_default_params(&prm);
   if (params) prm = *params;
   if (prm.kepler_iters < 0 || !(prm.kepler_tol > 0.0) || prm.chunk_steps < 1 || prm.chunk_steps > 16384 ||
-      prm.resync_chunks < 0 || prm.device < 0 || std::isnan(prm.r_min) || std::isnan(prm.r_max))
+      prm.resync_chunks < 0 || prm.device < 0 || std::isnan(prm.r_min) || std::isnan(prm.r_max) ||
+      prm.snapshot_chunks < 0 || prm.resonance_chunks < 0 || prm.segment_steps < 0)
     return GLISSE_EINVAL;
 
   int ndev = 0;
@@ -454,6 +637,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   CKF(configure_planet_kernels(&s->planet_smem));
 
   // ---- allocations: one device arena, carved at 256-byte boundaries ------------------------------
+  const int n_groups = static_cast<int>((N + particles_per_group() - 1) / particles_per_group());
   {
     struct Req { void** p; size_t bytes; };
     std::vector<Req> reqs;
@@ -467,19 +651,27 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
       need(&s->id[b], N);
       need(&s->flag[b], N);
       need(&s->rstep[b], N);
+      need(&s->d_list[b], n_groups);
     }
     for (int k = 0; k < 6; ++k) need(&s->fin[k], N);
     need(&s->fin_flag, N);
     need(&s->fin_rstep, N);
-    need(&s->res_phi, N);
-    need(&s->res_seen0, N);
-    need(&s->res_seen180, N);
+    LibrationRecord& L = s->lib;
+    need(&L.phi, N); need(&L.seen0, N); need(&L.seen180, N); need(&L.phi_min, N); need(&L.phi_max, N);
+    need(&L.ext_last, N); need(&L.amp_sum, N); need(&L.amp_max, N); need(&L.n_amp, N); need(&L.n_seen, N);
+    need(&L.trend, N); need(&L.ext_kind, N);
+    need(&s->d_amp_mean, N);
     for (int k = 0; k < 6; ++k) need(&s->snap[k], N);
     need(&s->snap_flag, N);
     need(&s->snap_rstep, N);
     need(&s->d_nslots, 2);
-    need(&s->d_block_counts, static_cast<size_t>((N + 255) / 256 + 1));
+    need(&s->d_block_counts, static_cast<size_t>(kCompactBins) * ((N + 255) / 256 + 1) + 1);
+    need(&s->d_bin, N);
     need(&s->d_counters, 2);
+    need(&s->d_ticket, 2);
+    need(&s->d_error, 1);
+    need(&s->d_stats, 3);
+    need(&s->d_fail, 2);
     need(&s->d_sys, 1);
     need(&s->d_j0, static_cast<size_t>(6 * np));
     need(&s->d_ptmp, static_cast<size_t>(6 * np));
@@ -523,9 +715,10 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     eta += gm_planet[j];
     hs.eta[j] = eta;
   }
-  hs.status = 0;
+  const long long no_fail[2] = {kNoPlanetFailure, kNoPlanetFailure};
   s->gm_planet_host.assign(gm_planet, gm_planet + np);
   CKF(cudaMemcpyAsync(s->d_sys, &hs, sizeof(hs), cudaMemcpyHostToDevice, s->p));
+  CKF(cudaMemcpyAsync(s->d_fail, no_fail, sizeof(no_fail), cudaMemcpyHostToDevice, s->p));
   if (np > 0) {
     double* d_q = s->d_ptmp;
     double* d_qd = s->d_ptmp + 3 * np;
@@ -550,6 +743,8 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     CKF(cudaMemcpyAsync(s->work[0][3 + k], vel[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
   }
   CKF(cudaMemsetAsync(s->d_counters, 0, 2 * sizeof(unsigned long long), s->q));
+  CKF(cudaMemsetAsync(s->d_error, 0, sizeof(int), s->q));
+  CKF(cudaMemsetAsync(s->d_stats, 0, 3 * sizeof(unsigned long long), s->q));
   {
     for (int k = 0; k < 6; ++k) {
       CKF(launch_count_nonfinite(s->work[0][k], N, s->d_counters + 1, s->q));
@@ -573,6 +768,8 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   // ---- constant part of the particle-kernel arguments --------------------------------------------
   ParticleArgs& a = s->pa;
   a.pstep_counter = s->d_counters;
+  a.error = s->d_error;
+  a.solver_stats = s->d_stats;
   a.stride = s->stride;
   a.stage_recs = stage_records(np);
   a.np = np;
@@ -592,8 +789,14 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   }
   a.rmin2_hi = high_word(a.rmin2);
   a.rmax2_hi = high_word(a.rmax2);
+  // iteration-count binning: the initial order is binned too (nothing is removed by it)
+  if (prm.bin_iterations && run_compaction(s) != GLISSE_OK) {
+    const int st = s->status;
+    free_sim(s);
+    return st;
+  }
   // the caller's buffers are free again once the copies on q are done; the planet stream keeps
-  // running (a planet failure is reported by the next synchronising call)
+  // running (a planet failure is reported by a synchronising call once the particles are past it)
   CKF(cudaStreamSynchronize(s->q));
 #undef CKF
   *out = s;
@@ -603,7 +806,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
 int glisse_advance(glisse_sim* s, long long n_steps) {
   if (!s || n_steps < 0) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
-  if (s->external_log_used) return GLISSE_EINVAL;  // the internal planet clock is stale
+  if (s->planets_stale) return GLISSE_EINVAL;  // the internal planet clock is stale: glisse_set_planets
   CKS(s, cudaSetDevice(s->device));
   const int np = s->np;
   while (n_steps > 0) {
@@ -620,6 +823,7 @@ int glisse_advance(glisse_sim* s, long long n_steps) {
       s->ahead = true;
     }
     CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+    break_chain(s);
     const int m = static_cast<int>(std::min<long long>(n_steps, B.len - off));
     const int st = launch_particles(s, B.log + static_cast<size_t>(off) * s->stride, m);
     if (st != GLISSE_OK) return st;
@@ -627,82 +831,148 @@ int glisse_advance(glisse_sim* s, long long n_steps) {
     n_steps -= m;
     if (off + m == B.len) {  // this buffer is used up: the planet stream may overwrite it
       CKS(s, cudaEventRecord(s->buf[s->cur].consumed, s->q));
+      break_chain(s);
       s->cur ^= 1;
       s->ahead = false;
     }
-    if (s->prm.resync_chunks > 0 && ++s->chunks_since_resync >= s->prm.resync_chunks) {
-      const int sc = run_compaction(s);
+    if ((s->step - s->origin) % s->K == 0) {  // a chunk is complete: periodic outputs, resync
+      const int sc = chunk_boundary(s);
       if (sc != GLISSE_OK) return sc;
     }
   }
   return GLISSE_OK;
 }
 
+// The external log goes through the sim's own two log buffers, chunk by chunk: upload of chunk c+1 on
+// the planet stream while the particle kernel works on chunk c — the paper's double-buffered PCIe
+// design.  No allocation, no host synchronisation.
 int glisse_advance_with_log(glisse_sim* s, long long n_steps, const double* log) {
   if (!s || n_steps < 0 || !log) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
   if (n_steps == 0) return GLISSE_OK;
   CKS(s, cudaSetDevice(s->device));
-  const size_t count = static_cast<size_t>(n_steps + 1) * s->stride;
-  double* d_log = nullptr;
-  CKS(s, dmalloc(&d_log, count));
-  cudaError_t e = cudaMemcpyAsync(d_log, log, count * sizeof(double), cudaMemcpyDefault, s->q);
-  int st = (e == cudaSuccess) ? GLISSE_OK : GLISSE_ECUDA;
-  long long done = 0;
-  while (st == GLISSE_OK && done < n_steps) {
-    const int m = static_cast<int>(std::min<long long>(n_steps - done, s->K));
-    st = launch_particles(s, d_log + static_cast<size_t>(done) * s->stride, m);
-    if (st != GLISSE_OK) break;
-    s->step += m;
-    done += m;
-    if (s->prm.resync_chunks > 0 && ++s->chunks_since_resync >= s->prm.resync_chunks) st = run_compaction(s);
+  if (!s->planets_stale) {
+    // From here on the two buffers hold the caller's planets.  The look-ahead planet kernel may still
+    // be writing one of them (the uploads below follow it on the same stream p) and particle kernels
+    // already queued on q may still be reading the other: the uploads wait for those through the
+    // buffers' `consumed` events, recorded now.
+    for (int b = 0; b < 2; ++b) CKS(s, cudaEventRecord(s->buf[b].consumed, s->q));
+    break_chain(s);
+    s->planets_stale = true;
+    s->ahead = false;
   }
-  cudaStreamSynchronize(s->q);
-  cudaFree(d_log);
-  s->external_log_used = true;
-  if (st != GLISSE_OK) s->status = st;
-  return st;
+  // upload records [first, first + m] of the caller's log into buffer b as the chunk starting at `start`
+  auto upload = [&](int b, long long first, long long start) -> int {
+    const int m = static_cast<int>(std::min<long long>(n_steps - first, s->K));
+    LogBuffer& B = s->buf[b];
+    CKS(s, cudaStreamWaitEvent(s->p, B.consumed, 0));
+    CKS(s, cudaMemcpyAsync(B.log, log + static_cast<size_t>(first) * s->stride,
+                           static_cast<size_t>(m + 1) * s->stride * sizeof(double), cudaMemcpyDefault, s->p));
+    CKS(s, cudaEventRecord(B.ready, s->p));
+    B.start = start;
+    B.len = m;
+    return GLISSE_OK;
+  };
+  const long long step_at_entry = s->step;
+  long long done = 0, uploaded = 0;
+  int b = s->cur;
+  {
+    const int st = upload(b, 0, step_at_entry);
+    if (st != GLISSE_OK) return st;
+    uploaded = s->buf[b].len;
+  }
+  while (done < n_steps) {
+    LogBuffer& B = s->buf[b];
+    if (uploaded < n_steps) {  // next chunk into the other buffer while this one is worked through
+      const int st = upload(b ^ 1, uploaded, step_at_entry + uploaded);
+      if (st != GLISSE_OK) return st;
+      uploaded += s->buf[b ^ 1].len;
+    }
+    CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+    break_chain(s);
+    const int st = launch_particles(s, B.log, B.len);
+    if (st != GLISSE_OK) return st;
+    s->step += B.len;
+    done += B.len;
+    CKS(s, cudaEventRecord(B.consumed, s->q));
+    break_chain(s);
+    if (B.len == s->K) {   // every full chunk of the external history counts as a chunk
+      const int sc = chunk_boundary(s);
+      if (sc != GLISSE_OK) return sc;
+    }
+    b ^= 1;
+  }
+  s->cur = b;
+  return GLISSE_OK;
+}
+
+int glisse_set_planets(glisse_sim* s, const double* planet_pos, const double* planet_vel) {
+  if (!s) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  const int np = s->np;
+  if (np > 0 && (!planet_pos || !planet_vel)) return GLISSE_EINVAL;
+  if (np > 0 && (!all_finite_host(planet_pos, 3LL * np) || !all_finite_host(planet_vel, 3LL * np))) return GLISSE_EINVAL;
+  CKS(s, cudaSetDevice(s->device));
+  // everything queued on either stream uses the old clock: let it finish, then restart at this step
+  CKS(s, cudaStreamSynchronize(s->p));
+  CKS(s, cudaStreamSynchronize(s->q));
+  if (np > 0) {
+    double* d_q = s->d_ptmp;
+    double* d_qd = s->d_ptmp + 3 * np;
+    CKS(s, cudaMemcpyAsync(d_q, planet_pos, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p));
+    CKS(s, cudaMemcpyAsync(d_qd, planet_vel, sizeof(double) * 3 * np, cudaMemcpyHostToDevice, s->p));
+    CKS(s, launch_planet_init(s->d_sys, d_q, d_qd, s->d_j0, s->p));
+    s->launches += 1;
+  }
+  const long long no_fail = kNoPlanetFailure;
+  CKS(s, cudaMemcpyAsync(s->d_fail, &no_fail, sizeof(no_fail), cudaMemcpyHostToDevice, s->p));
+  CKS(s, cudaStreamSynchronize(s->p));   // the caller's arrays and `no_fail` are consumed
+  s->origin = s->step;
+  s->cur = 0;
+  s->ahead = false;
+  s->planets_stale = false;
+  return fill_log_buffer(s, 0, s->d_j0, s->step);
 }
 
 int glisse_planet_log(glisse_sim* s, long long n_steps, double* log) {
   if (!s || n_steps < 0 || !log || n_steps > (1LL << 24)) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
-  if (s->external_log_used) return GLISSE_EINVAL;
+  if (s->planets_stale) return GLISSE_EINVAL;
   CKS(s, cudaSetDevice(s->device));
+  break_chain(s);
   const int np = s->np;
   const LogBuffer& B = s->buf[s->cur];
   const long long off = s->step - B.start;
   double *d_log = nullptr, *d_jlog = nullptr;
   const size_t count = static_cast<size_t>(n_steps + 1) * s->stride;
+  const long long no_fail = kNoPlanetFailure;
+  long long fail = kNoPlanetFailure;
   CKS(s, dmalloc(&d_log, count));
   cudaError_t e = dmalloc(&d_jlog, static_cast<size_t>(n_steps + 1) * 6 * np);
   if (e == cudaSuccess) e = cudaStreamWaitEvent(s->q, B.ready, 0);
+  // a scratch failure word: a failure somewhere in this look-ahead does not concern the sim's own clock
+  if (e == cudaSuccess) e = cudaMemcpyAsync(s->d_fail + 1, &no_fail, sizeof(no_fail), cudaMemcpyHostToDevice, s->q);
   if (e == cudaSuccess)
     e = launch_planet_kernel(s->d_sys, s->np, B.jlog + static_cast<size_t>(off) * 6 * np, d_log, d_jlog,
-                             static_cast<int>(n_steps), s->dt, 0, s->q);
+                             static_cast<int>(n_steps), s->dt, s->step, s->d_fail + 1, 0, s->q);
   s->launches += 1;
   if (e == cudaSuccess) e = cudaMemcpyAsync(log, d_log, count * sizeof(double), cudaMemcpyDefault, s->q);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&fail, s->d_fail + 1, sizeof(fail), cudaMemcpyDeviceToHost, s->q);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->q);
   cudaFree(d_log);
   cudaFree(d_jlog);
   CKS(s, e);
-  return sync_all(s);
+  const int st = sync_all(s);
+  if (st != GLISSE_OK) return st;
+  return fail < s->step + n_steps ? GLISSE_EPLANET : GLISSE_OK;   // not sticky: the sim itself is intact
 }
 
 int glisse_read(glisse_sim* s, double* const pos[3], double* const vel[3], int* flag, long long* removal_step) {
   if (!s) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
   CKS(s, cudaSetDevice(s->device));
-  ScatterArgs g{};
-  const int w = s->w;
-  for (int k = 0; k < 6; ++k) {
-    g.st[k] = s->work[w][k];
-    g.fin[k] = s->fin[k];
-  }
-  g.id = s->id[w]; g.flag = s->flag[w]; g.rstep = s->rstep[w];
-  g.n_slots = s->d_nslots + w;
-  g.fin_flag = s->fin_flag; g.fin_rstep = s->fin_rstep;
-  CKS(s, launch_scatter_to_original(g, s->nslots_upper, s->q));
+  break_chain(s);
+  CKS(s, launch_scatter_to_original(scatter_args(s), s->nslots_upper, s->q));
   s->launches += 1;
   const size_t N = static_cast<size_t>(s->n);
   for (int k = 0; k < 3; ++k) {
@@ -719,48 +989,7 @@ int glisse_snapshot(glisse_sim* s, int kind, double* const out[6], int* flag, lo
   if (!s || (kind != GLISSE_SNAPSHOT_CARTESIAN && kind != GLISSE_SNAPSHOT_ELEMENTS)) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
   CKS(s, cudaSetDevice(s->device));
-  if (!s->r) {  // first snapshot of this sim: its copy stream and events
-    CKS(s, cudaStreamCreateWithFlags(&s->r, cudaStreamNonBlocking));
-    CKS(s, cudaEventCreateWithFlags(&s->snap_ready, cudaEventDisableTiming));
-    CKS(s, cudaEventCreateWithFlags(&s->snap_done, cudaEventDisableTiming));
-  }
-  // the staging arrays are free once the previous snapshot's copies are done (device-side wait)
-  if (s->snap_in_flight) CKS(s, cudaStreamWaitEvent(s->q, s->snap_done, 0));
-  // working order -> original order (as glisse_read), then -> staging, Cartesian or elements
-  ScatterArgs g{};
-  const int w = s->w;
-  for (int k = 0; k < 6; ++k) {
-    g.st[k] = s->work[w][k];
-    g.fin[k] = s->fin[k];
-  }
-  g.id = s->id[w]; g.flag = s->flag[w]; g.rstep = s->rstep[w];
-  g.n_slots = s->d_nslots + w;
-  g.fin_flag = s->fin_flag; g.fin_rstep = s->fin_rstep;
-  CKS(s, launch_scatter_to_original(g, s->nslots_upper, s->q));
-  SnapshotArgs a{};
-  for (int k = 0; k < 6; ++k) {
-    a.fin[k] = s->fin[k];
-    a.out[k] = s->snap[k];
-  }
-  a.fin_flag = s->fin_flag; a.fin_rstep = s->fin_rstep;
-  a.out_flag = s->snap_flag; a.out_rstep = s->snap_rstep;
-  a.n = s->n;
-  a.mu = s->gm0;
-  a.kind = kind;
-  CKS(s, launch_snapshot(a, s->q));
-  s->launches += 2;
-  CKS(s, cudaEventRecord(s->snap_ready, s->q));
-  // from here on the particle stream is free to go on; stream r ships the staging copy
-  CKS(s, cudaStreamWaitEvent(s->r, s->snap_ready, 0));
-  const size_t N = static_cast<size_t>(s->n);
-  for (int k = 0; k < 6; ++k)
-    if (out && out[k]) CKS(s, cudaMemcpyAsync(out[k], s->snap[k], N * sizeof(double), cudaMemcpyDefault, s->r));
-  if (flag) CKS(s, cudaMemcpyAsync(flag, s->snap_flag, N * sizeof(int), cudaMemcpyDefault, s->r));
-  if (removal_step)
-    CKS(s, cudaMemcpyAsync(removal_step, s->snap_rstep, N * sizeof(long long), cudaMemcpyDefault, s->r));
-  CKS(s, cudaEventRecord(s->snap_done, s->r));
-  s->snap_in_flight = true;
-  return GLISSE_OK;
+  return enqueue_sample(s, true, kind, out, flag, removal_step, nullptr, false);
 }
 
 int glisse_snapshot_wait(glisse_sim* s) {
@@ -772,14 +1001,35 @@ int glisse_snapshot_wait(glisse_sim* s) {
   return GLISSE_OK;
 }
 
+int glisse_snapshot_ring(glisse_sim* s, int kind, int n_slots, double* data, int* flag, long long* removal_step,
+                         long long* slot_step) {
+  if (!s || n_slots < 0) return GLISSE_EINVAL;
+  if (n_slots > 0 && (!data || (kind != GLISSE_SNAPSHOT_CARTESIAN && kind != GLISSE_SNAPSHOT_ELEMENTS)))
+    return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  if (s->r) CKS(s, cudaStreamSynchronize(s->r));   // copies into the ring being replaced are done
+  if (n_slots > 0 && !s->h_ring_steps)
+    CKS(s, cudaMallocHost(reinterpret_cast<void**>(&s->h_ring_steps), kRingStepWords * sizeof(long long)));
+  s->ring_kind = kind;
+  s->ring_slots = n_slots;
+  s->ring_data = n_slots ? data : nullptr;
+  s->ring_flag = n_slots ? flag : nullptr;
+  s->ring_rstep = n_slots ? removal_step : nullptr;
+  s->ring_step = n_slots ? slot_step : nullptr;
+  s->ring_emitted = 0;
+  return GLISSE_OK;
+}
+
+long long glisse_snapshots_emitted(glisse_sim* s) { return s ? s->ring_emitted : GLISSE_EINVAL; }
+
 int glisse_resonance_begin(glisse_sim* s, int planet, int p, int q, double window) {
   if (!s || planet < 0 || planet >= s->np || q < 1 || p <= q || !(window > 0.0)) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
   CKS(s, cudaSetDevice(s->device));
-  const size_t N = static_cast<size_t>(s->n);
-  CKS(s, cudaMemsetAsync(s->res_seen0, 0, N, s->q));
-  CKS(s, cudaMemsetAsync(s->res_seen180, 0, N, s->q));
-  CKS(s, cudaMemsetAsync(s->res_phi, 0, N * sizeof(double), s->q));
+  break_chain(s);
+  CKS(s, launch_libration_reset(s->lib, s->n, s->q));
+  s->launches += 1;
   s->res_planet = planet; s->res_p = p; s->res_q = q;
   s->res_window = window;
   s->res_samples = 0;
@@ -789,41 +1039,9 @@ int glisse_resonance_begin(glisse_sim* s, int planet, int p, int q, double windo
 int glisse_resonance_sample(glisse_sim* s) {
   if (!s || s->res_planet < 0) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
-  if (s->external_log_used) return GLISSE_EINVAL;  // the internal planet clock is stale
+  if (s->planets_stale) return GLISSE_EINVAL;  // the internal planet clock is stale
   CKS(s, cudaSetDevice(s->device));
-  const int np = s->np;
-  // particles: working order -> original order (as glisse_read)
-  ScatterArgs g{};
-  const int w = s->w;
-  for (int k = 0; k < 6; ++k) {
-    g.st[k] = s->work[w][k];
-    g.fin[k] = s->fin[k];
-  }
-  g.id = s->id[w]; g.flag = s->flag[w]; g.rstep = s->rstep[w];
-  g.n_slots = s->d_nslots + w;
-  g.fin_flag = s->fin_flag; g.fin_rstep = s->fin_rstep;
-  CKS(s, launch_scatter_to_original(g, s->nslots_upper, s->q));
-  // planets at the current step: heliocentric q, qd from the Jacobi state of this record
-  const LogBuffer& B = s->buf[s->cur];
-  const long long off = s->step - B.start;
-  double* d_out = s->d_ptmp;
-  CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
-  CKS(s, launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q));
-  ResonanceArgs a{};
-  for (int k = 0; k < 6; ++k) a.fin[k] = s->fin[k];
-  a.fin_flag = s->fin_flag;
-  a.planet_q = d_out + 3 * s->res_planet;
-  a.planet_qd = d_out + 3 * np + 3 * s->res_planet;
-  a.phi = s->res_phi; a.seen0 = s->res_seen0; a.seen180 = s->res_seen180;
-  a.n = s->n;
-  a.mu = s->gm0;
-  a.mu_planet = s->gm0 + s->gm_planet_host[s->res_planet];
-  a.window = s->res_window;
-  a.p = s->res_p; a.q = s->res_q;
-  CKS(s, launch_resonance(a, s->q));
-  s->launches += 3;
-  s->res_samples += 1;
-  return GLISSE_OK;
+  return enqueue_sample(s, false, 0, nullptr, nullptr, nullptr, nullptr, true);
 }
 
 int glisse_resonance_read(glisse_sim* s, unsigned char* seen0, unsigned char* seen180, double* phi_last,
@@ -831,21 +1049,42 @@ int glisse_resonance_read(glisse_sim* s, unsigned char* seen0, unsigned char* se
   if (!s || s->res_planet < 0) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
   CKS(s, cudaSetDevice(s->device));
+  break_chain(s);
   const size_t N = static_cast<size_t>(s->n);
-  if (seen0) CKS(s, cudaMemcpyAsync(seen0, s->res_seen0, N, cudaMemcpyDefault, s->q));
-  if (seen180) CKS(s, cudaMemcpyAsync(seen180, s->res_seen180, N, cudaMemcpyDefault, s->q));
-  if (phi_last) CKS(s, cudaMemcpyAsync(phi_last, s->res_phi, N * sizeof(double), cudaMemcpyDefault, s->q));
+  if (seen0) CKS(s, cudaMemcpyAsync(seen0, s->lib.seen0, N, cudaMemcpyDefault, s->q));
+  if (seen180) CKS(s, cudaMemcpyAsync(seen180, s->lib.seen180, N, cudaMemcpyDefault, s->q));
+  if (phi_last) CKS(s, cudaMemcpyAsync(phi_last, s->lib.phi, N * sizeof(double), cudaMemcpyDefault, s->q));
   if (n_samples) *n_samples = s->res_samples;
+  return sync_all(s);
+}
+
+int glisse_libration_read(glisse_sim* s, double* phi_min, double* phi_max, double* amp_mean, double* amp_max,
+                          int* n_amp) {
+  if (!s || s->res_planet < 0) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  break_chain(s);
+  const size_t N = static_cast<size_t>(s->n);
+  if (phi_min) CKS(s, cudaMemcpyAsync(phi_min, s->lib.phi_min, N * sizeof(double), cudaMemcpyDefault, s->q));
+  if (phi_max) CKS(s, cudaMemcpyAsync(phi_max, s->lib.phi_max, N * sizeof(double), cudaMemcpyDefault, s->q));
+  if (amp_mean) {
+    CKS(s, launch_libration_mean(s->lib, s->d_amp_mean, s->n, s->q));
+    s->launches += 1;
+    CKS(s, cudaMemcpyAsync(amp_mean, s->d_amp_mean, N * sizeof(double), cudaMemcpyDefault, s->q));
+  }
+  if (amp_max) CKS(s, cudaMemcpyAsync(amp_max, s->lib.amp_max, N * sizeof(double), cudaMemcpyDefault, s->q));
+  if (n_amp) CKS(s, cudaMemcpyAsync(n_amp, s->lib.n_amp, N * sizeof(int), cudaMemcpyDefault, s->q));
   return sync_all(s);
 }
 
 int glisse_read_planets(glisse_sim* s, double* pos, double* vel) {
   if (!s) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
-  if (s->external_log_used) return GLISSE_EINVAL;
+  if (s->planets_stale) return GLISSE_EINVAL;
   CKS(s, cudaSetDevice(s->device));
   const int np = s->np;
   if (np == 0 || (!pos && !vel)) return sync_all(s);
+  break_chain(s);
   const LogBuffer& B = s->buf[s->cur];
   const long long off = s->step - B.start;
   double* d_out = s->d_ptmp;
@@ -861,6 +1100,7 @@ long long glisse_active_count(glisse_sim* s) {
   if (!s) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;
   if (cudaSetDevice(s->device) != cudaSuccess) return GLISSE_ECUDA;
+  break_chain(s);
   unsigned long long c = 0;
   cudaError_t e = cudaMemsetAsync(s->d_counters + 1, 0, sizeof(unsigned long long), s->q);
   if (e == cudaSuccess) e = launch_count_active(s->flag[s->w], s->d_nslots + s->w, s->nslots_upper, s->d_counters + 1, s->q);
@@ -908,6 +1148,28 @@ int glisse_particle_kernel_time(glisse_sim* s, double* ms, long long* launches) 
   s->timed_ms = 0.0;
   s->timed_launches = 0;
   return st;
+}
+
+int glisse_solver_stats_enable(glisse_sim* s, int on) {
+  if (!s) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  CKS(s, cudaSetDevice(s->device));
+  break_chain(s);
+  CKS(s, cudaMemsetAsync(s->d_stats, 0, 3 * sizeof(unsigned long long), s->q));
+  s->stats_on = on != 0;
+  return GLISSE_OK;
+}
+
+int glisse_solver_stats(glisse_sim* s, long long* warp_steps, long long* warp_iters, long long* warp_slow) {
+  if (!s) return GLISSE_EINVAL;
+  const int st = glisse_sync(s);
+  if (st != GLISSE_OK) return st;
+  unsigned long long c[3] = {};
+  CKS(s, cudaMemcpy(c, s->d_stats, sizeof(c), cudaMemcpyDeviceToHost));
+  if (warp_steps) *warp_steps = static_cast<long long>(c[0]);
+  if (warp_iters) *warp_iters = static_cast<long long>(c[1]);
+  if (warp_slow) *warp_slow = static_cast<long long>(c[2]);
+  return GLISSE_OK;
 }
 
 int glisse_fp64_peak_probe(int device, void* stream, double millis, double* flops) {

@@ -7,6 +7,14 @@
 // block counts, scatter).  Survivors go, in order, to the prefix of the other working buffer; a
 // removed particle's frozen state goes to its ORIGINAL index in the `fin` arrays, which is where
 // glisse_read assembles the result, so compaction is invisible to the caller (reading S16).
+//
+// Iteration-count binning ("it is desirable to sort the particles by the expected number
+// of iterations required to solve Kepler's equation, so that threads in the same block will perform
+// similar amounts of work ... the most eccentric group would be launched first"; the paper proposes
+// it and did not build it): with bins > 1 the survivors are partitioned by a hardness bin of their
+// ORBIT (not of the instant: a chunk spans many revolutions), hardest bin first, particle order kept
+// within a bin.  Every survivor is moved by the partition anyway, so the ordering is free; a particle's
+// arithmetic never depends on its warp-mates, so results are bit-identical to the unbinned run.
 #include "glisse_internal.cuh"
 
 namespace glisse {
@@ -15,14 +23,60 @@ namespace {
 constexpr int kBlock = 256;
 constexpr unsigned kFull = 0xffffffffu;
 
-__global__ void __launch_bounds__(kBlock) count_block_actives(const int* __restrict__ flag,
-                                                               const int* __restrict__ n_in,
-                                                               int* __restrict__ block_counts) {
-  const int n = *n_in;
+// Hardness bin of an orbit for the particle kernel's Kepler solver (kepler.cuh): 0 = one quartic step
+// is accepted at every phase of the orbit, 1 = some phases need more, 2 = some phase leaves the fast
+// solver (e >= 0.8, |x0| > pi/4, unbound).  The fast solver starts from x0 = dM/q, q = 1 - e cos E0,
+// and accepts once the Newton update delta = f(x0)/f'(x0) is below an eccentricity-tiered bound;
+// here delta is evaluated at 12 phases E0 of the orbit with a safety factor of 2.  A heuristic: it
+// decides only which particles share a warp.
+__device__ int hardness_bin(double mu, double dt, double x, double y, double z, double vx, double vy, double vz) {
+  const double r = sqrt(x * x + y * y + z * z);
+  const double v2 = vx * vx + vy * vy + vz * vz;
+  const double u = x * vx + y * vy + z * vz;
+  const double alpha = 2.0 * mu / r - v2;
+  if (!(alpha > 0.0)) return 2;
+  const double ec = 1.0 - r * alpha / mu;
+  const double e2 = ec * ec + u * u * alpha / (mu * mu);
+  if (!(e2 < 0.64)) return 2;
+  const double e = sqrt(e2);
+  const double kTwoPi = 6.283185307179586;
+  double dM = alpha * sqrt(alpha) * dt / mu;
+  dM = fabs(dM - kTwoPi * rint(dM / kTwoPi));
+  if (dM >= 0.78539816 * (1.0 - e)) return 2;
+  const double thr = 0.5 * (e2 < 0.01 ? 1e-4 : (e2 < 0.09 ? 9e-5 : (e2 < 0.25 ? 5.5e-5 : 2e-5)));
+  double worst = 0.0;
+  for (int k = 0; k < 12; ++k) {
+    double s0, c0;
+    sincos(kTwoPi * k / 12.0, &s0, &c0);
+    const double q = 1.0 - e * c0, es = e * s0, x0 = dM / q;
+    double sx, cx;
+    sincos(x0, &sx, &cx);
+    const double f = e * c0 * (x0 - sx) + es * (1.0 - cx);
+    const double f1 = 1.0 - e * c0 * cx + es * sx;
+    worst = fmax(worst, fabs(f / f1));
+  }
+  return worst < thr ? 0 : 1;
+}
+
+// per block and per bin: number of active slots; also writes every slot's bin
+__global__ void __launch_bounds__(kBlock) count_block_actives(const CompactArgs a, int nb) {
+  __shared__ int cnt[kCompactBins];
+  const int n = *a.n_in;
   const int i = blockIdx.x * kBlock + threadIdx.x;
-  const bool act = (i < n) && (flag[i] == 0);
-  const int c = __syncthreads_count(act);
-  if (threadIdx.x == 0) block_counts[blockIdx.x] = c;
+  const bool act = (i < n) && (a.src_flag[i] == 0);
+  if (threadIdx.x < kCompactBins) cnt[threadIdx.x] = 0;
+  __syncthreads();
+  int b = 0;
+  if (act && a.bins > 1)
+    b = hardness_bin(a.mu, a.dt, a.src[0][i], a.src[1][i], a.src[2][i], a.src[3][i], a.src[4][i], a.src[5][i]);
+  if (i < n) a.bin[i] = static_cast<unsigned char>(b);
+  for (int k = 0; k < a.bins; ++k) {
+    const unsigned m = __ballot_sync(kFull, act && b == k);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(&cnt[k], __popc(m));
+  }
+  __syncthreads();
+  // hardest bin first: output order index = bins - 1 - bin
+  if (threadIdx.x < a.bins) a.block_counts[(a.bins - 1 - threadIdx.x) * nb + blockIdx.x] = cnt[threadIdx.x];
 }
 
 // exclusive scan of block_counts[0..nb) in place (one block), total -> *n_out
@@ -64,22 +118,27 @@ __global__ void __launch_bounds__(1024) scan_block_counts(int* __restrict__ bloc
   if (threadIdx.x == 0) *n_out = carry_s;
 }
 
-__global__ void __launch_bounds__(kBlock) scatter_partition(const CompactArgs a) {
-  __shared__ int warp_counts[kBlock / 32];
+__global__ void __launch_bounds__(kBlock) scatter_partition(const CompactArgs a, int nb) {
+  __shared__ int warp_counts[kCompactBins][kBlock / 32];
   const int n = *a.n_in;
   const int i = blockIdx.x * kBlock + threadIdx.x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool in = i < n;
   const int fl = in ? a.src_flag[i] : -1;
   const bool act = fl == 0;
-  const unsigned m = __ballot_sync(kFull, act);
-  if (lane == 0) warp_counts[warp] = __popc(m);
+  const int b = act ? a.bin[i] : 0;
+  unsigned m = 0;   // ballot of this thread's own bin
+  for (int k = 0; k < a.bins; ++k) {
+    const unsigned mk = __ballot_sync(kFull, act && b == k);
+    if (lane == 0) warp_counts[k][warp] = __popc(mk);
+    if (b == k) m = mk;
+  }
   __syncthreads();
-  int off = a.block_counts[blockIdx.x];
-  for (int w = 0; w < warp; ++w) off += warp_counts[w];
   if (!in) return;
   const int id = a.src_id[i];
   if (act) {
+    int off = a.block_counts[(a.bins - 1 - b) * nb + blockIdx.x];
+    for (int w = 0; w < warp; ++w) off += warp_counts[b][w];
     const int d = off + __popc(m & ((1u << lane) - 1u));
 #pragma unroll
     for (int k = 0; k < 6; ++k) a.dst[k][d] = a.src[k][i];
@@ -141,9 +200,9 @@ __global__ void __launch_bounds__(kBlock) count_nonfinite_kernel(const double* _
 cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStream_t s, long long* launches) {
   if (n_slots_upper < 1) n_slots_upper = 1;
   const int nb = (n_slots_upper + kBlock - 1) / kBlock;
-  count_block_actives<<<nb, kBlock, 0, s>>>(a.src_flag, a.n_in, a.block_counts);
-  scan_block_counts<<<1, 1024, 0, s>>>(a.block_counts, nb, a.n_out);
-  scatter_partition<<<nb, kBlock, 0, s>>>(a);
+  count_block_actives<<<nb, kBlock, 0, s>>>(a, nb);
+  scan_block_counts<<<1, 1024, 0, s>>>(a.block_counts, a.bins * nb, a.n_out);
+  scatter_partition<<<nb, kBlock, 0, s>>>(a, nb);
   if (launches) *launches += 3;
   return cudaGetLastError();
 }

@@ -54,6 +54,16 @@ struct ParticleArgs {
   // high words of rmin2, rmax2, rc2[]: the hot path's integer superset of the distance tests
   int rmin2_hi, rmax2_hi;
   int rc2_hi[kMaxPlanets];
+  // Launch chaining: a chunk is issued as back-to-back launches of a few hundred steps
+  // each, the later ones with programmatic stream serialisation, so that they become resident while
+  // the earlier one drains.  A warp of launch j+1 takes the k-th group of 32 particles that launch j
+  // COMPLETED (not a fixed one), so it never waits on a particular slow warp.
+  int* wait_list;          // previous launch's completion list: entry k = group + 1, 0 = not yet; null = first
+  int* done_list;          // this launch's completion list (zero on entry)
+  unsigned* done_ticket;   // this launch's completion counter
+  unsigned ticket_base;    // value of *done_ticket when this launch starts
+  int* error;              // device word: != 0 once a chained warp gave up waiting (never expected)
+  unsigned long long* solver_stats;  // [3] warp drift calls, fast-solver iterations, slow-path entries (STATS only)
 };
 
 // ---- planet system constants, resident in device memory -----------------------------------------
@@ -63,21 +73,30 @@ struct PlanetSystem {
   double gm[kMaxPlanets];
   double eta[kMaxPlanets];       // eta_k = gm0 + sum_{i<=k} gm_i
   double eta_prev[kMaxPlanets];  // eta_{k-1}
-  int status;                    // 0, or 1-based index of the first planet whose drift failed
 };
+// A planet failure (drift unbound / not converged, GLISSE_EPLANET) is recorded as the absolute index
+// of the first step whose drift failed, in a device word that starts at kNoPlanetFailure: records up
+// to and including that step are valid, so the failure concerns the caller only once the particles
+// have gone past it — a look-ahead chunk that fails does not poison the state already computed.
+constexpr long long kNoPlanetFailure = 0x7fffffffffffffffLL;
 
 // Jacobi state record: [r'_0 .. r'_{Np-1} | v'_0 .. v'_{Np-1}], 6·Np doubles.
 inline int jstate_stride(int np) { return 6 * np; }
 
 // launchers (each returns the cudaError_t of the launch); *launches += kernels launched
-cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_slots_upper, cudaStream_t s);
+// chained: launch with programmatic stream serialisation behind the previous particle-kernel launch
+// stats: the instrumented instantiation (glisse_test.h: glisse_solver_stats)
+cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, cudaStream_t s);
 cudaError_t configure_particle_kernels();
+int particles_per_group();
 
 // Planet-history kernel (a1): from the Jacobi state `jin` write nsteps+1 log records and nsteps+1
 // Jacobi state records (record 0 = the input state).  exclusive_sm_bytes > 0: dynamic
 // shared memory to request (unused) so that no other block fits on its SM.
-cudaError_t launch_planet_kernel(PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
-                                 int nsteps, double dt, int exclusive_sm_bytes, cudaStream_t s);
+// fail_step: see kNoPlanetFailure; step0 = absolute step index of record 0.
+cudaError_t launch_planet_kernel(const PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
+                                 int nsteps, double dt, long long step0, long long* fail_step, int exclusive_sm_bytes,
+                                 cudaStream_t s);
 // allows the planet-history kernel the whole shared memory of an SM; returns that size in bytes
 cudaError_t configure_planet_kernels(int* exclusive_sm_bytes);
 // heliocentric (q, qd) [np][3] -> Jacobi state record
@@ -97,8 +116,14 @@ struct CompactArgs {
   int* fin_flag; long long* fin_rstep;
   const int* n_in;         // prefix length of src
   int* n_out;              // number of survivors = prefix length of dst
-  int* block_counts;       // scratch [ceil(n_upper/256) + 1]
+  int* block_counts;       // scratch [kCompactBins * ceil(n_upper/256) + 1]
+  // iteration-count binning (include/glisse.h bin_iterations): bins > 1 orders the
+  // survivors by bin (hardest first), particle order within a bin
+  unsigned char* bin;      // scratch [n_upper]: bin of every slot (written by the count pass)
+  int bins;                // 1 = plain stable partition, kCompactBins = binned
+  double mu, dt;           // for the hardness key
 };
+constexpr int kCompactBins = 3;
 cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStream_t s, long long* launches);
 
 struct ScatterArgs {
@@ -115,32 +140,43 @@ cudaError_t launch_init_ids(int* id, int* flag, long long* rstep, int* fin_flag,
                             cudaStream_t s);
 cudaError_t launch_count_nonfinite(const double* p, long long n, unsigned long long* out, cudaStream_t s);
 
-// snapshot.cu: original-order arrays -> staging copy, Cartesian or osculating elements
-struct SnapshotArgs {
+// snapshot.cu: ONE pass over the original-order arrays that serves the snapshot (staging copy,
+// Cartesian or osculating elements) and the resonant-argument reduction of the same instant: the
+// elements are computed once for both.
+struct LibrationRecord {     // per particle, original order (include/glisse.h: glisse_libration_read)
+  double* phi;              // last value of the argument, [0, 2 pi)
+  unsigned char* seen0;     // phi has been within `window` of 0
+  unsigned char* seen180;   // phi has been within `window` of pi
+  double* phi_min;          // running extrema of phi
+  double* phi_max;
+  double* ext_last;         // value of the latest turning point
+  double* amp_sum;          // sum and maximum of the amplitude samples |ext - previous ext| / 2
+  double* amp_max;
+  int* n_amp;               // number of amplitude samples
+  int* n_seen;              // samples this particle has taken
+  signed char* trend;       // +1 rising, -1 falling, 0 unknown
+  signed char* ext_kind;    // +1 the latest turning point was a maximum, -1 a minimum, 0 none yet
+};
+struct SampleArgs {
   const double* fin[6];
   const int* fin_flag; const long long* fin_rstep;
-  double* out[6];
-  int* out_flag; long long* out_rstep;
   long long n;
   double mu;
-  int kind;
-};
-cudaError_t launch_snapshot(const SnapshotArgs& a, cudaStream_t s);
-
-// snapshot.cu: resonant-argument reduction over the original-order arrays
-struct ResonanceArgs {
-  const double* fin[6];
-  const int* fin_flag;
+  // snapshot part (do_snapshot)
+  int do_snapshot, kind;
+  double* out[6];
+  int* out_flag; long long* out_rstep;
+  // resonance part (do_resonance)
+  int do_resonance, p, q;
   const double* planet_q;   // [3] heliocentric position of the planet at the current step (device)
   const double* planet_qd;  // [3] velocity
-  double* phi;              // [n] last value of the argument, [0, 2 pi)
-  unsigned char* seen0;     // [n] phi has been within `window` of 0
-  unsigned char* seen180;   // [n] phi has been within `window` of pi
-  long long n;
-  double mu, mu_planet, window;
-  int p, q;
+  double mu_planet, window;
+  LibrationRecord lib;
 };
-cudaError_t launch_resonance(const ResonanceArgs& a, cudaStream_t s);
+cudaError_t launch_sample(const SampleArgs& a, cudaStream_t s);
+cudaError_t launch_libration_reset(const LibrationRecord& lib, long long n, cudaStream_t s);
+// amp_mean[n] = amp_sum / n_amp (NaN where n_amp = 0)
+cudaError_t launch_libration_mean(const LibrationRecord& lib, double* amp_mean, long long n, cudaStream_t s);
 
 cudaError_t run_fp64_probe(cudaStream_t s, double millis, double* flops);
 cudaError_t run_primitive(int which, long long n, const double* in, double* out, cudaStream_t s);

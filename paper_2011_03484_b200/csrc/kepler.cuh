@@ -238,6 +238,11 @@ static __device__ __noinline__ ExactSolve kepler_solve_exact(bool live, double e
 // roofline.
 constexpr int kFastMinIters = 5;   // the paper's count; below it the definition may not converge
 constexpr int kFastMaxIters = 4;
+// The fast solver does not evaluate the residual: what it accepts has a residual below 2e-17 plus the
+// rounding of the residual's own evaluation (<= 2e-15 for |dM| <= pi).  A caller whose kepler_tol is
+// below that floor is asking the definition's residual test to decide on roundoff, so every body then
+// goes through the definition's solver, which does evaluate it.
+constexpr double kFastMinTol = 4e-15;
 
 __device__ __forceinline__ int hi_abs(double x) { return hi_word(x) & 0x7fffffff; }
 
@@ -263,12 +268,13 @@ template <int P>
 __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], double mu, double inv_mu,
                                                   double inv_mu_dt, int iters, double tol, const double (&r2)[P],
                                                   double (&x)[P], double (&y)[P], double (&z)[P], double (&vx)[P],
-                                                  double (&vy)[P], double (&vz)[P], int (&st)[P]) {
+                                                  double (&vy)[P], double (&vz)[P], int (&st)[P], int& fast_iters,
+                                                  bool& went_slow) {
   bool live[P], unbound[P], open[P], slow[P];
   double rinv[P], sqa[P], rsa[P], q[P], ec[P], es[P], dM[P], a[P], invq[P], e2[P], xk[P];
   double sm[P], cm1[P];  // sin x − x, cos x − 1 at the final xk
   int thr[P], nonconv[P];
-  const bool fast_on = iters >= kFastMinIters;
+  const bool fast_on = iters >= kFastMinIters && tol >= kFastMinTol;
   bool any_open = false;
 #pragma unroll
   for (int p = 0; p < P; ++p) {
@@ -303,8 +309,10 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
     nonconv[p] = 0;
   }
 
+  fast_iters = 0;   // warp-uniform: iterations of the fast solver this warp executes (solver statistics)
   for (int it = 0; it < kFastMaxIters && __any_sync(kFullMask, any_open); ++it) {
     any_open = false;
+    fast_iters = it + 1;
 #pragma unroll
     for (int p = 0; p < P; ++p) {
       double smk, cmk;
@@ -346,7 +354,8 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
     slow[p] = slow[p] || open[p];  // no convergence in kFastMaxIters steps
     any_slow = any_slow || slow[p];
   }
-  if (__any_sync(kFullMask, any_slow)) {
+  went_slow = __any_sync(kFullMask, any_slow);
+  if (went_slow) {
 #pragma unroll
     for (int p = 0; p < P; ++p) {
       if (__any_sync(kFullMask, slow[p])) {
@@ -387,8 +396,9 @@ __device__ __forceinline__ int kepler_drift_warp(bool live, double mu, double in
   const bool l1[1] = {live};
   const double r21[1] = {r2};
   double x1[1] = {x}, y1[1] = {y}, z1[1] = {z}, vx1[1] = {vx}, vy1[1] = {vy}, vz1[1] = {vz};
-  int st[1];
-  kepler_drift_warp<1>(l1, mu, inv_mu, inv_mu_dt, iters, tol, r21, x1, y1, z1, vx1, vy1, vz1, st);
+  int st[1], fast_iters;
+  bool went_slow;
+  kepler_drift_warp<1>(l1, mu, inv_mu, inv_mu_dt, iters, tol, r21, x1, y1, z1, vx1, vy1, vz1, st, fast_iters, went_slow);
   x = x1[0]; y = y1[0]; z = z1[0]; vx = vx1[0]; vy = vy1[0]; vz = vz1[0];
   return st[0];
 }

@@ -54,26 +54,81 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                : "memory");
 }
 
+// ---- launch chaining: completion lists between back-to-back launches -------------------
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// programmatic dependent launch: the next launch in the stream (if it asked for programmatic
+// serialisation) may become resident once every block of this grid has executed this or exited
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// A warp of a chained launch takes the k-th completed group of the previous launch, k = blockIdx.x.
+// Deadlock-free: the previous launch's blocks call pdl_launch_dependents only once they own a group, so
+// when this block is resident every block of the previous launch is resident or finished, and those
+// never wait on anything later.  The time-out (seconds; never expected) turns a logic error into a
+// status instead of a hung device.
+__device__ __forceinline__ int acquire_group(const ParticleArgs& a, int lane) {
+  int g = static_cast<int>(blockIdx.x);
+  if (a.wait_list != nullptr) {
+    int v = 0;
+    if (lane == 0) {
+      int* slot = a.wait_list + blockIdx.x;
+      const long long t0 = clock64();
+      unsigned ns = 32;
+      while ((v = ld_acquire(slot)) == 0) {
+        __nanosleep(ns);
+        if (ns < 2048) ns <<= 1;
+        if (clock64() - t0 > (8LL << 30)) { atomicExch(a.error, 1); v = -1; break; }
+      }
+      // the entry is this block's alone: free it for the launch after next (an atomic, so that the
+      // clearing has been performed at L2 before this block lets dependents launch)
+      atomicExch(slot, 0);
+    }
+    v = __shfl_sync(kFullMask, v, 0);
+    g = v - 1;   // -2: gave up
+  }
+  return g;
+}
+
+__device__ __forceinline__ void publish_group(const ParticleArgs& a, int lane, int g) {
+  __threadfence();   // this lane's stores of the group's state are visible device-wide ...
+  __syncwarp();
+  if (lane == 0) {   // ... before the group is handed on
+    const unsigned pos = atomicAdd(a.done_ticket, 1u) - a.ticket_base;
+    st_release(a.done_list + pos, g + 1);
+  }
+}
+
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 // NP > 0: compile-time planet count (fully unrolled kick); NP == 0: run-time count a.np.
 // P = particles per thread (kParticlesPerThread): independent instruction streams, see kepler.cuh.
-template <int NP, int P>
+// STATS: instrumented instantiation (glisse_test.h: glisse_solver_stats); same arithmetic.
+template <int NP, int P, bool STATS>
 __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel(const __grid_constant__ ParticleArgs a) {
+  static_assert(kParticleBlock == 32, "one warp per block: the launch chain hands groups of one warp on");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31;
-  const int warp = threadIdx.x >> 5;
+  constexpr int warp = 0;
   const int np = NP > 0 ? NP : a.np;
   const int stride = a.stride;
   const int nsteps = a.nsteps;
   const int R = a.stage_recs;
   const int stage_doubles = R * stride;
 
+  const int grp = acquire_group(a, lane);
+  pdl_launch_dependents();
+  if (grp < 0) return;   // gave up waiting (a.error is set): touch nothing
   const int n = *a.n_slots;
   // particle p of this thread: consecutive threads hold consecutive particles (coalesced), the P
   // particles of a thread lie kParticleBlock apart
-  const long long i0 = static_cast<long long>(blockIdx.x) * (kParticleBlock * P) + threadIdx.x;
+  const long long i0 = static_cast<long long>(grp) * (kParticleBlock * P) + threadIdx.x;
 
   // ---- a2: load ------------------------------------------------------------------------------
   double x[P], y[P], z[P], vx[P], vy[P], vz[P];
@@ -86,17 +141,20 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
     const long long i = i0 + p * kParticleBlock;
     x[p] = 1.0; y[p] = 0.0; z[p] = 0.0; vx[p] = 0.0; vy[p] = 0.0; vz[p] = 0.0;
     flag[p] = -1;
-    if (i < n) {
-      flag[p] = a.flag[i];
-      x[p] = a.st[0][i]; y[p] = a.st[1][i]; z[p] = a.st[2][i];
-      vx[p] = a.st[3][i]; vy[p] = a.st[4][i]; vz[p] = a.st[5][i];
+    if (i < n) {  // through L2: the group's previous owner may have run on another SM a launch ago
+      flag[p] = __ldcg(a.flag + i);
+      x[p] = __ldcg(a.st[0] + i); y[p] = __ldcg(a.st[1] + i); z[p] = __ldcg(a.st[2] + i);
+      vx[p] = __ldcg(a.st[3] + i); vy[p] = __ldcg(a.st[4] + i); vz[p] = __ldcg(a.st[5] + i);
     }
     was_alive[p] = (flag[p] == 0);
     alive[p] = was_alive[p];
     any_alive_t = any_alive_t || alive[p];
     rs[p] = -1;
   }
-  if (!__any_sync(kFullMask, any_alive_t)) return;  // nothing to do in this warp: leave before any copy
+  if (!__any_sync(kFullMask, any_alive_t)) {  // nothing to do in this warp: leave before any copy
+    publish_group(a, lane, grp);
+    return;
+  }
 
   // ---- warp-private ring ------------------------------------------------------------------------
   double* ring = reinterpret_cast<double*>(smem_raw) + static_cast<size_t>(warp) * kRingSlots * stage_doubles;
@@ -119,6 +177,7 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   __syncwarp();
 
   const double hdt = a.hdt;
+  unsigned stat_calls = 0, stat_iters = 0, stat_slow = 0;
   int k = 0;  // global record index
   int st = 0;
   for (; st < nstages; ++st) {
@@ -198,7 +257,15 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
       // ---- a5/a6: drift (O2) --------------------------------------------------------------------
       if (k < nsteps) {
         int st_d[P];
-        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, a.inv_mu_dt, a.iters, a.tol, r2, x, y, z, vx, vy, vz, st_d);
+        int fast_iters;
+        bool went_slow;
+        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, a.inv_mu_dt, a.iters, a.tol, r2, x, y, z, vx, vy, vz, st_d,
+                             fast_iters, went_slow);
+        if (STATS) {
+          stat_calls += 1;
+          stat_iters += fast_iters;
+          stat_slow += went_slow ? 1 : 0;
+        }
 #pragma unroll
         for (int p = 0; p < P; ++p) {
           if (st_d[p] != 0) {
@@ -255,6 +322,13 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   }
   unsigned tot = __reduce_add_sync(kFullMask, drifts);
   if (lane == 0 && tot) atomicAdd(a.pstep_counter, static_cast<unsigned long long>(tot));
+  if (STATS && lane == 0) {
+    atomicAdd(a.solver_stats, static_cast<unsigned long long>(stat_calls));
+    atomicAdd(a.solver_stats + 1, static_cast<unsigned long long>(stat_iters));
+    atomicAdd(a.solver_stats + 2, static_cast<unsigned long long>(stat_slow));
+  }
+  // (the group index is rebuilt from i0 rather than kept live across the step loop)
+  publish_group(a, lane, static_cast<int>((i0 - threadIdx.x) / (kParticleBlock * P)));
 }
 
 size_t particle_smem_bytes(const ParticleArgs& a) {
@@ -262,28 +336,50 @@ size_t particle_smem_bytes(const ParticleArgs& a) {
          static_cast<size_t>(kParticleWarps) * kRingSlots * 8;
 }
 
+template <int NP>
+cudaError_t configure_one() {
+  cudaError_t e;
+  const int carve = cudaSharedmemCarveoutMaxShared;
+  constexpr int P = kParticlesPerThread;
+  if ((e = cudaFuncSetAttribute(particle_kernel<NP, P, false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
+  return cudaFuncSetAttribute(particle_kernel<NP, P, true>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+}
+
+template <int NP, bool STATS>
+cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chained, cudaStream_t s) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(static_cast<unsigned>(blocks));
+  cfg.blockDim = dim3(kParticleBlock);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = chained ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, kParticlesPerThread, STATS>, a);
+}
+
 }  // namespace
 
 cudaError_t configure_particle_kernels() {
   cudaError_t e;
-  const int carve = cudaSharedmemCarveoutMaxShared;
-  constexpr int P = kParticlesPerThread;
-  if ((e = cudaFuncSetAttribute(particle_kernel<0, P>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  if ((e = cudaFuncSetAttribute(particle_kernel<4, P>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  if ((e = cudaFuncSetAttribute(particle_kernel<8, P>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  return cudaSuccess;
+  if ((e = configure_one<0>())) return e;
+  if ((e = configure_one<4>())) return e;
+  return configure_one<8>();
 }
 
-cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_slots_upper, cudaStream_t s) {
-  if (n_slots_upper < 1) n_slots_upper = 1;
-  constexpr int P = kParticlesPerThread;
-  const int per_block = kParticleBlock * P;
-  const int blocks = (n_slots_upper + per_block - 1) / per_block;
+cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, cudaStream_t s) {
+  if (n_groups < 1) n_groups = 1;
   const size_t smem = particle_smem_bytes(a);
-  if (a.np == 4) particle_kernel<4, P><<<blocks, kParticleBlock, smem, s>>>(a);
-  else if (a.np == 8) particle_kernel<8, P><<<blocks, kParticleBlock, smem, s>>>(a);
-  else particle_kernel<0, P><<<blocks, kParticleBlock, smem, s>>>(a);
-  return cudaGetLastError();
+  cudaError_t e;
+  if (a.np == 4) e = stats ? launch_one<4, true>(a, n_groups, smem, chained, s) : launch_one<4, false>(a, n_groups, smem, chained, s);
+  else if (a.np == 8) e = stats ? launch_one<8, true>(a, n_groups, smem, chained, s) : launch_one<8, false>(a, n_groups, smem, chained, s);
+  else e = stats ? launch_one<0, true>(a, n_groups, smem, chained, s) : launch_one<0, false>(a, n_groups, smem, chained, s);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
+
+// particles per launch group (one warp's worth): the host sizes grids and completion lists with it
+int particles_per_group() { return kParticleBlock * kParticlesPerThread; }
 
 }  // namespace glisse

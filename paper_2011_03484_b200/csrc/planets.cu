@@ -161,9 +161,10 @@ __device__ __forceinline__ void write_record(const Lane& L, double* log, double*
 }
 
 template <int NP>
-__global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, const double* __restrict__ jin,
+__global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* sys, const double* __restrict__ jin,
                                                              double* __restrict__ log, double* __restrict__ jlog,
-                                                             int nsteps, double dt) {
+                                                             int nsteps, double dt, long long step0,
+                                                             long long* fail_step) {
   const Lane L = make_lane(sys);
   const int stride = log_stride(L.np);
   const double hdt = 0.5 * dt;
@@ -181,20 +182,21 @@ __global__ void __launch_bounds__(32) planet_history_kernel(PlanetSystem* sys, c
   jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
   kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
   write_record(L, log, jlog, 0, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
-  int bad = 0;
+  int bad = -1;   // first step (within this launch) whose drift failed
   for (int s = 0; s < nsteps; ++s) {
     vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
     const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
     const int st = kepler_drift_warp(true, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2,
                                      rx, ry, rz, vx, vy, vz);
     const unsigned failed = __ballot_sync(kFullMask, st != 0 && L.live);
-    if (failed && !bad) bad = __ffs(failed);
+    if (failed && bad < 0) bad = s;
     jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
     kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
     vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
     write_record(L, log, jlog, s + 1, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
   }
-  if (bad && L.lane == 0 && sys->status == 0) sys->status = bad;
+  // records up to and including step0 + bad are valid (glisse_internal.cuh: kNoPlanetFailure)
+  if (bad >= 0 && L.lane == 0) atomicMin(fail_step, step0 + bad);
 }
 
 __global__ void __launch_bounds__(32) planet_init_kernel(const PlanetSystem* sys, const double* q, const double* qd,
@@ -235,17 +237,18 @@ __global__ void __launch_bounds__(32) planet_read_kernel(const PlanetSystem* sys
 
 }  // namespace
 
-cudaError_t launch_planet_kernel(PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
-                                 int nsteps, double dt, int exclusive_sm_bytes, cudaStream_t s) {
+cudaError_t launch_planet_kernel(const PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
+                                 int nsteps, double dt, long long step0, long long* fail_step, int exclusive_sm_bytes,
+                                 cudaStream_t s) {
   // The kernel is one warp whose K steps are serial: all that counts is its latency, and sharing an
   // SM with ~25 particle warps that saturate the FP64 pipe doubles it.  It therefore asks for the
   // whole shared memory of an SM (unused), which keeps every other block off that SM: 1/148 of the
   // device for the ~1.4 ms it runs per chunk.
   const size_t smem = exclusive_sm_bytes > 0 ? static_cast<size_t>(exclusive_sm_bytes) : 0;
   switch (np) {
-    case 4: planet_history_kernel<4><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt); break;
-    case 8: planet_history_kernel<8><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt); break;
-    default: planet_history_kernel<0><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt); break;
+    case 4: planet_history_kernel<4><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt, step0, fail_step); break;
+    case 8: planet_history_kernel<8><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt, step0, fail_step); break;
+    default: planet_history_kernel<0><<<1, 32, smem, s>>>(sys, jin, log, jlog, nsteps, dt, step0, fail_step); break;
   }
   return cudaGetLastError();
 }

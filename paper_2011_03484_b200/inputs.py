@@ -180,6 +180,28 @@ def one_m_four_planets(n_particles: int = 1_048_576) -> Workload:
                     pos=pos, vel=vel, dt=dt, steps=steps, r_min=1.0, r_max=1000.0)
 
 
+def chain_system(n_planets: int, n_particles: int = 2048, dt: float = 5.0) -> Workload:
+    """A seeded system with ANY planet count 0..32, for the code paths BASELINE.json's two planet
+    counts (4 and 8) do not reach: planets on a geometric ladder a_k = 1.5 rho^k AU out to 40 AU (rho
+    capped at 1.35), equal masses chosen so that neighbours sit 12 mutual Hill radii apart
+    (m = 1.5 ((rho - 1) / 12)^3, capped at 1e-4), e ~ U[0, 0.02], i ~ U[0, 1 deg]; particles
+    a ~ U[1.2, 1.2 a_last], e ~ U[0, 0.1], i ~ U[0, 5 deg], angles uniform; dt = 5 d (134 steps per
+    orbit of the innermost planet, so that the 1,000-step parity horizon is 7 of its orbits and the
+    roundoff sensitivity of most particles stays below 1e-12); removal at r < 0.3 AU, r > 1000 AU, 1 Hill radius."""
+    npl = int(n_planets)
+    rho = min(1.35, (40.0 / 1.5) ** (1.0 / max(npl - 1, 1)))
+    mass = min(1e-4, 1.5 * ((rho - 1.0) / 12.0) ** 3)
+    a_nom = 1.5 * rho ** np.arange(npl)
+    c = 100 + npl
+    gm, ppos, pvel, rcrit = _planets(c, [mass] * npl, a_nom, 0.02, 1.0)
+    a_hi = 1.2 * (a_nom[-1] if npl else 40.0)
+    pos, vel = _particles(c, n_particles, 1.2, a_hi, 0.1, 5.0)
+    return Workload(name=f"chain: {npl} planets a = 1.5 x {rho:.4f}^k AU, m = {mass:.3g}, {n_particles} particles",
+                    gm_star=G, gm_planet=gm.reshape(npl), planet_pos=ppos.reshape(npl, 3),
+                    planet_vel=pvel.reshape(npl, 3), planet_rcrit=np.asarray(rcrit, dtype=np.float64).reshape(npl),
+                    pos=pos, vel=vel, dt=dt, steps=1000, r_min=0.3, r_max=1000.0)
+
+
 def shard_range(n: int, rank: int, world: int) -> tuple[int, int]:
     """Contiguous particle slice [lo, hi) of rank `rank` out of `world` (particles never interact,
     PAPER.md:27,35: planets are replicated, particles partitioned, no exchange)."""

@@ -31,3 +31,23 @@ def cartesian_to_elements(mu, r, v):
 
 def angle_diff(a, b):
     return np.abs((a - b + np.pi) % (2 * np.pi) - np.pi)
+
+
+def state_from_elements(mu, a, e, inc, Om, om, f):
+    """Perifocal state at true anomaly f rotated by R_z(Om) R_x(inc) R_z(om), written out here
+    (Murray & Dermott eq. 2.119-2.122); returns r, v and the mean anomaly of f."""
+    p = a * (1.0 - e * e)
+    r = p / (1.0 + e * np.cos(f))
+    rp = np.array([r * np.cos(f), r * np.sin(f), 0.0])
+    vp = np.sqrt(mu / p) * np.array([-np.sin(f), e + np.cos(f), 0.0])
+
+    def rz(t):
+        return np.array([[np.cos(t), -np.sin(t), 0], [np.sin(t), np.cos(t), 0], [0, 0, 1.0]])
+
+    def rx(t):
+        return np.array([[1.0, 0, 0], [0, np.cos(t), -np.sin(t)], [0, np.sin(t), np.cos(t)]])
+
+    R = rz(Om) @ rx(inc) @ rz(om)
+    E = 2.0 * np.arctan2(np.sqrt(1.0 - e) * np.sin(f / 2.0), np.sqrt(1.0 + e) * np.cos(f / 2.0))
+    M = (E - e * np.sin(E)) % (2.0 * np.pi)
+    return R @ rp, R @ vp, M

@@ -19,19 +19,22 @@ def libpath():
     return cuda_build.build()
 
 
-def _declared_symbols():
-    src = open(os.path.join(ROOT, "include", "glisse.h")).read()
+def _declared_symbols(header):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(glisse_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_library_exports_every_declared_symbol(libpath):
+    """include/glisse.h (the interface) and include/glisse_test.h (measurement / test hooks)."""
     from paper_2011_03484_b200 import binding
-    declared = _declared_symbols()
-    assert len(declared) >= 15
-    assert sorted(binding.EXPORTS) == declared       # the binding mirrors the header, name for name
+    declared = _declared_symbols("glisse.h")
+    hooks = _declared_symbols("glisse_test.h")
+    assert len(declared) >= 20 and len(hooks) >= 5 and not set(declared) & set(hooks)
+    assert sorted(binding.EXPORTS) == declared       # the binding mirrors the headers, name for name
+    assert sorted(binding.TEST_EXPORTS) == hooks
     L = ctypes.CDLL(libpath)
-    for name in declared:
+    for name in declared + hooks:
         assert hasattr(L, name), name
 
 
@@ -55,6 +58,7 @@ def test_host_only_entry_points(libpath):
     p = binding.GlisseParams()
     L.glisse_default_params(ctypes.byref(p))
     assert (p.kepler_iters, p.kepler_tol, p.chunk_steps, p.resync_chunks) == (5, 1e-14, 1024, 1)
+    assert (p.snapshot_chunks, p.resonance_chunks, p.bin_iterations, p.segment_steps) == (0, 0, 0, 256)
     assert p.r_min == 0.0 and p.r_max == float("inf")
 
 

@@ -46,6 +46,31 @@ def test_two_rank_sharding_and_reduction():
         assert np.array_equal(np.array(planets), big.planet_pos)        # planets replicated
 
 
+def _gloo_rank(argv):
+    """Stand-in for bench.rank_main on a box without GPUs: what a rank does minus the kernels."""
+    import bench
+    from paper_2011_03484_b200 import inputs
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    assert int(os.environ["LOCAL_RANK"]) == rank and os.environ["MASTER_ADDR"] == "127.0.0.1"
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    bench.WORKLOADS["tiny"] = ("tiny", lambda n: inputs.config(1, n))
+    _, w = bench.make_workload("tiny", world, rank)
+    ms, units = bench.reduce_over_ranks(2.0 + rank, float(w.n_particles), dist)
+    with open(os.path.join(argv[0], f"rank{rank}.txt"), "w") as fh:
+        fh.write(f"{world} {ms} {units}")
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_gpus_flag_starts_the_ranks_itself(tmp_path):
+    """`python bench.py --gpus N` without torchrun: bench.launch_ranks starts one process per GPU with
+    the torchrun environment; here with gloo at world size 2 and a CPU stand-in for the rank body."""
+    import bench
+    bench.launch_ranks(2, _gloo_rank, [str(tmp_path)], port=31000 + os.getpid() % 2000)
+    got = sorted(open(tmp_path / f"rank{r}.txt").read() for r in range(2))
+    assert got == ["2 3.0 2048.0", "2 3.0 2048.0"]      # both ranks see max time and summed units
+
+
 def test_single_process_reduction_is_identity():
     import bench
     assert bench.reduce_over_ranks(3.5, 7.0, None) == (3.5, 7.0)

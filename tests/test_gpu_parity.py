@@ -2,14 +2,20 @@
 same seeded inputs (BASELINE.json north_star: positions/velocities <= 1e-10 relative after 1,000
 steps, removal flags and removal steps bit-exact).
 
-Tolerance rule (DESIGN.md §5 "P-risk"): two independent fp64 implementations of a chaotic map
-differ by roundoff (about 1e-16 per operation, 1e-14 accumulated over the 1,000-step horizon) that
-close planetary approaches amplify by many orders of magnitude.  The oracle is therefore also run
-on three twins of the input, each component moved by a relative 1e-14 with seeded random signs;
-sigma_i = the largest deviation of a twin from the oracle's own result is particle i's
-sensitivity.  Required: dev_i <= max(1e-10, 10 sigma_i) for every particle — which is the plain
-1e-10 bound wherever sigma_i <= 1e-11 — and flags / removal steps identical wherever every
-twin's agree.  On the quiet configurations (1-3) the plain bound is required of every particle.
+Tolerance rule (SURVEY.md §8(c) "P-risk"): two independent fp64 implementations of a
+chaotic map differ by roundoff that close planetary approaches amplify by many orders of magnitude.
+The oracle is therefore also run on TWINS of the input, every component moved by exactly 1 ulp in a
+seeded direction; sigma_i = the largest deviation of a twin from the oracle's own result is particle
+i's sensitivity.  Required of every particle: dev_i <= max(1e-10, 100 sigma_i) — which is the plain
+1e-10 bound wherever sigma_i <= 1e-12 — and flags / removal steps identical wherever every twin's
+agree.  On the quiet configurations (1, 2, 3, 1m_x4) the plain bound and exact flags are required of
+EVERY particle, twins or not.  Three twins are used: the survey proposed one, and one 1-ulp twin
+is a single draw of a heavy-tailed sensitivity that under-estimates it for 5 of the 8,211 particles
+of the config-5 case (measured); with the maximum over three nothing fails.
+
+Every parity test records what it MEASURED (max deviation, max dev/sigma, particles above 1e-10,
+excluded particles) through the `record` fixture: printed, and appended to
+gpurun_out/parity_stats.jsonl when that directory exists; DESIGN.md §5 tabulates one such run.
 """
 import numpy as np
 import pytest
@@ -20,11 +26,15 @@ pytestmark = pytest.mark.gpu
 
 TOL = 1e-10          # BASELINE.json north_star
 HORIZON = 1000       # steps
-# Planets over the horizon: a 1-ulp (1.1e-16) roundoff per step in a planet's energy
-# random-walks to 1.1e-16 sqrt(s) and integrates to an along-track error of about
-# 1.5 (n dt) 1.1e-16 s^1.5 / sqrt(3) = 1e-12 at s = 1000, n dt = 0.29 (the innermost planets); two
-# independent fp64 implementations differ by a small multiple of that.
-PLANET_TOL = 1e-11
+# Planet log over the horizon, per planet system: a 1-ulp roundoff per step in a
+# planet's energy random-walks into an along-track error of about 1.5 (n dt) 1.1e-16 s^1.5 / sqrt(3)
+# = 1e-12 at s = 1000 for n dt = 0.29; the oracle and the kernel each carry their own.  Tolerance =
+# 3 x the deviation measured on B200 (profiles/r02_parity_stats.md), keyed by (config, N_p).
+PLANET_TOL = {(1, 4): 4.1e-12,    # measured 1.35e-12 (SURVEY.md §7 step 4 hoped for 1e-12)
+              (4, 8): 3.3e-12,    # measured 1.08e-12
+              (1, 1): 1.7e-11,    # measured 5.42e-12: Jupiter alone, exact Kepler orbit, pure drift roundoff
+              (1, 3): 7.0e-12,    # measured 2.32e-12
+              (1, 2): 1.7e-11, (1, 0): 0.0}
 
 
 @pytest.fixture(scope="module")
@@ -49,19 +59,20 @@ def _oracle_run(oracle_mod, w, steps, **kw):
     return out, ps
 
 
-TWIN_EPS = 1e-14     # accumulated roundoff of 1,000 fp64 steps
-TWIN_FACTOR = 10.0
+TWIN_COUNT = 3
+TWIN_FACTOR = 100.0      # dev_i <= max(1e-10, 100 sigma_i)
+SIGMA_PLAIN = 1e-12      # ... and <= 1e-10 outright wherever sigma_i <= 1e-12 (the same inequality)
 
 
-def _twins(w, k=3):
-    """k copies of the workload, every particle component moved by a relative 1e-14 (seeded signs)."""
+def _twins(w, k=TWIN_COUNT):
+    """k copies of the workload, every particle component moved by exactly 1 ulp (seeded directions)."""
     import dataclasses
     rng = np.random.default_rng(20201103)
     out = []
     for _ in range(k):
-        sp = rng.choice([-1.0, 1.0], size=w.pos.shape)
-        sv = rng.choice([-1.0, 1.0], size=w.vel.shape)
-        out.append(dataclasses.replace(w, pos=w.pos * (1.0 + TWIN_EPS * sp), vel=w.vel * (1.0 + TWIN_EPS * sv)))
+        sp = rng.choice([-np.inf, np.inf], size=w.pos.shape)
+        sv = rng.choice([-np.inf, np.inf], size=w.vel.shape)
+        out.append(dataclasses.replace(w, pos=np.nextafter(w.pos, sp), vel=np.nextafter(w.vel, sv)))
     return out
 
 
@@ -76,7 +87,35 @@ def _sensitivity(oracle_mod, w, steps, po, vo, fo, ro):
     return sigma, agree
 
 
-def _check_parity(gl, oracle_mod, w, steps=HORIZON, expect_quiet=False, min_plain=0.99, **simkw):
+def _judge(record, case, dev, sigma, twin_agrees, f, r, fo, ro, expect_quiet, min_plain):
+    """The tolerance rule of the module docstring on one run; records what was measured."""
+    n = len(dev)
+    flags_equal = (f == fo) & (r == ro)
+    excluded = int((~twin_agrees).sum())
+    ok = twin_agrees & flags_equal
+    bound = np.maximum(TOL, TWIN_FACTOR * sigma)
+    plain = ok & (sigma <= SIGMA_PLAIN)
+    above = ok & (dev > TOL)
+    stats = dict(case=case, n=n, removed=int((fo != 0).sum()), flag_mismatches=int((~flags_equal).sum()),
+                 flag_mismatches_where_twins_agree=int((~flags_equal & twin_agrees).sum()), excluded_by_twins=excluded,
+                 dev_max=float(dev.max()), dev_median=float(np.median(dev)), dev_p99=float(np.quantile(dev, 0.99)),
+                 n_dev_above_1e10=int((dev > TOL).sum()), sigma_max=float(sigma.max()),
+                 max_dev_over_sigma_where_dev_above_1e10=float((dev[above] / sigma[above]).max()) if above.any() else 0.0,
+                 max_dev_over_bound=float((dev[ok] / bound[ok]).max()), frac_held_to_plain_bound=float(plain.mean()))
+    record(stats)
+    # flags / removal steps: bit-exact wherever the problem itself is not roundoff-sensitive
+    assert stats["flag_mismatches_where_twins_agree"] == 0
+    assert excluded <= max(1, int(2e-3 * n))
+    assert np.all(dev[ok] <= bound[ok]), stats
+    assert np.all(dev[plain] <= TOL), stats
+    assert plain.sum() >= min_plain * n, stats
+    if expect_quiet:  # the plain north_star bound and exact flags, every particle
+        assert excluded == 0 and flags_equal.all(), stats
+        assert dev.max() <= TOL, stats
+    return stats
+
+
+def _check_parity(gl, oracle_mod, record, case, w, steps=HORIZON, expect_quiet=False, min_plain=0.99, **simkw):
     (po, vo, fo, ro), ps_o = _oracle_run(oracle_mod, w, steps)
     sigma, twin_agrees = _sensitivity(oracle_mod, w, steps, po, vo, fo, ro)
     S = gl.GlisseSim.from_workload(w, **simkw)
@@ -86,22 +125,12 @@ def _check_parity(gl, oracle_mod, w, steps=HORIZON, expect_quiet=False, min_plai
     active_g = S.active_count()
     S.close()
     dev = np.maximum(_dev(p, po), _dev(v, vo))
-    # flags / removal steps: bit-exact wherever the problem itself is not roundoff-sensitive
-    assert np.array_equal(f[twin_agrees], fo[twin_agrees])
-    assert np.array_equal(r[twin_agrees], ro[twin_agrees])
-    excluded = int((~twin_agrees).sum())
-    assert excluded <= max(1, int(2e-3 * w.n_particles))
-    ok = twin_agrees & (f == fo)
-    bound = np.maximum(TOL, TWIN_FACTOR * sigma)
-    assert np.all(dev[ok] <= bound[ok]), float(np.max(dev[ok] / bound[ok]))
-    plain = ok & (bound <= TOL)          # particles held to the plain north_star bound
-    assert plain.sum() >= min_plain * w.n_particles, plain.mean()
-    if expect_quiet:  # the plain north_star bound, every particle
-        assert excluded == 0 and np.array_equal(f, fo) and np.array_equal(r, ro)
-        assert dev.max() <= TOL, dev.max()
+    st = _judge(record, case, dev, sigma, twin_agrees, f, r, fo, ro, expect_quiet, min_plain)
+    if expect_quiet:
         assert ps_g == ps_o
         assert active_g == int((fo == 0).sum())
-    return dict(dev_max=float(dev.max()), excluded=excluded, removed=int((fo != 0).sum()), calm=int(plain.sum()))
+    return dict(dev_max=st["dev_max"], excluded=st["excluded_by_twins"], removed=st["removed"],
+                calm=int(round(st["frac_held_to_plain_bound"] * w.n_particles)))
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -134,7 +163,7 @@ def test_primitive_sincos_differences(gl):
             assert abs(cm - ec) <= 5e-16
 
 
-def test_kepler_drift_matches_oracle_per_body(gl, oracle_mod):
+def test_kepler_drift_matches_oracle_per_body(gl, oracle_mod, record):
     """Step a5 alone, over the whole range: e up to 0.97, dM from tiny to beyond 2 pi, both time
     directions; unbound and non-converged bodies must get the oracle's flag."""
     rng = np.random.default_rng(6)
@@ -165,9 +194,10 @@ def test_kepler_drift_matches_oracle_per_body(gl, oracle_mod):
                         np.linalg.norm(out[i, 4:7] - v1) / np.linalg.norm(v1))
         else:   # state untouched
             assert np.array_equal(out[i, 1:4], pos[i]) and np.array_equal(out[i, 4:7], vel[i])
-    assert n_flag[4] >= 50 and n_flag[0] > 5000
-    # a residual sitting within roundoff of the tolerance may fall either side: none expected here
-    assert mism <= 2, (mism, n_flag)
+    record(dict(case="kepler_drift_per_body", n=n, flag_mismatches=mism, dev_max=float(worst),
+                flags={str(k): v for k, v in n_flag.items()}))
+    assert n_flag[4] >= 50 and n_flag[0] > 5000 and n_flag[3] > 0
+    assert mism == 0, (mism, n_flag)   # flag 3 / 4 decided exactly as the definition decides it
     assert worst <= 1e-12, worst   # one drift: roundoff times the e <= 0.97 conditioning
 
 
@@ -175,7 +205,7 @@ def test_kepler_drift_matches_oracle_per_body(gl, oracle_mod):
 # planet-history kernel (a1) against the oracle's planet integrator
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("c,npl", [(1, 4), (4, 8), (1, 1), (1, 3), (1, 0)])
-def test_planet_log_matches_oracle(gl, oracle_mod, c, npl):
+def test_planet_log_matches_oracle(gl, oracle_mod, record, c, npl):
     import dataclasses
     w = inputs.config(c, n_particles=64)
     w = dataclasses.replace(w, gm_planet=w.gm_planet[:npl], planet_pos=w.planet_pos[:npl],
@@ -188,11 +218,15 @@ def test_planet_log_matches_oracle(gl, oracle_mod, c, npl):
     if npl:
         q = log[:, :3 * npl].reshape(-1, npl, 3)
         qr = ref[:, :3 * npl].reshape(-1, npl, 3)
+        tol = PLANET_TOL[(c, npl)]
         d = np.linalg.norm(q - qr, axis=2) / np.linalg.norm(qr, axis=2)
-        assert d.max() <= PLANET_TOL, d.max()
         h = log[:, 3 * npl:3 * npl + 3]
         hr = ref[:, 3 * npl:3 * npl + 3]
-        assert np.max(np.linalg.norm(h - hr, axis=1) / np.linalg.norm(hr, axis=1)) <= 1e-11
+        dh = np.linalg.norm(h - hr, axis=1) / np.linalg.norm(hr, axis=1)
+        record(dict(case=f"planet_log_c{c}_np{npl}", q_dev_max=float(d.max()), h0_dev_max=float(dh.max()),
+                    q_dev_max_per_planet=[float(x) for x in d.max(axis=0)], tol=tol))
+        assert d.max() <= tol, d.max()
+        assert dh.max() <= tol, dh.max()
     else:
         assert np.all(log == 0.0)
     assert np.all(log[:, 3 * npl + 3:] == 0.0)   # padding
@@ -202,8 +236,8 @@ def test_planet_log_matches_oracle(gl, oracle_mod, c, npl):
     qp, qv = S.read_planets()
     oq, ov = O.read_planets()
     if npl:
-        assert np.max(np.linalg.norm(qp - oq, axis=1) / np.linalg.norm(oq, axis=1)) <= PLANET_TOL
-        assert np.max(np.linalg.norm(qv - ov, axis=1) / np.linalg.norm(ov, axis=1)) <= PLANET_TOL
+        assert np.max(np.linalg.norm(qp - oq, axis=1) / np.linalg.norm(oq, axis=1)) <= tol
+        assert np.max(np.linalg.norm(qv - ov, axis=1) / np.linalg.norm(ov, axis=1)) <= tol
     assert S.step() == HORIZON
     S.close()
 
@@ -211,9 +245,9 @@ def test_planet_log_matches_oracle(gl, oracle_mod, c, npl):
 # ---------------------------------------------------------------------------------------------------
 # whole path, BASELINE.json config shapes at sizes the oracle finishes in seconds
 # ---------------------------------------------------------------------------------------------------
-def test_config1_full_parity(gl, oracle_mod):
+def test_config1_full_parity(gl, oracle_mod, record):
     """configs[0] exactly as stated: 1,024 particles, 4 giants, dt = 180 d; 1,000-step horizon."""
-    st = _check_parity(gl, oracle_mod, inputs.config(1), expect_quiet=True)
+    st = _check_parity(gl, oracle_mod, record, "c1", inputs.config(1), expect_quiet=True)
     assert st["removed"] >= 5   # flag parity is not vacuous
 
 
@@ -237,15 +271,71 @@ def test_config1_ten_thousand_steps_flags_and_fractions(gl, oracle_mod):
 
 @pytest.mark.parametrize("c,n,quiet", [(2, 4096 + 77, True), (3, 4096 + 5, True), (4, 2048 + 33, False),
                                         (5, 8192 + 19, False)])
-def test_config_shapes_parity(gl, oracle_mod, c, n, quiet):
+def test_config_shapes_parity(gl, oracle_mod, record, c, n, quiet):
     """configs[1..4] shapes at reduced N (several blocks and a ragged tail)."""
-    # config 5: planet-crossing orbits, a fifth of the particles are roundoff-sensitive within the horizon
-    st = _check_parity(gl, oracle_mod, inputs.config(c, n_particles=n), expect_quiet=quiet,
-                       min_plain=0.75 if c == 5 else 0.99)
+    # config 5: planet-crossing orbits; measured on B200: 83.0 % of the 8,211 particles have
+    # sigma <= 1e-12 and are held to the plain bound (DESIGN.md §5) -> required 0.80
+    st = _check_parity(gl, oracle_mod, record, f"c{c}_{n}", inputs.config(c, n_particles=n), expect_quiet=quiet,
+                       min_plain=0.80 if c == 5 else 0.99)
     if c == 5:
         assert st["removed"] > 200      # heavy removal exercised (5 % by step 10^3)
     if c == 4:
         assert st["calm"] > 0.9 * n
+
+
+@pytest.mark.parametrize("npl", [1, 2, 5, 16, 32])
+def test_runtime_planet_count_parity(gl, oracle_mod, record, npl):
+    """The generic particle kernel (run-time N_p: every N_p other than 0, 4, 8 — log stride up to 100
+    doubles, 2-record ring stages at N_p = 32) and the generic planet-history kernel, whole path
+    against the oracle on inputs.chain_system: N_p planets on a geometric ladder, particles threaded
+    between them (a tenth of them removed at N_p = 1)."""
+    w = inputs.chain_system(npl, 2048 + 17)
+    # measured fraction of particles with sigma <= 1e-12 (oracle twins): 0.96 at N_p = 1, >= 0.99 from 5 up
+    st = _check_parity(gl, oracle_mod, record, f"chain_np{npl}", w, min_plain=0.93 if npl <= 2 else 0.97,
+                       chunk_steps=200)
+    if npl <= 5:
+        assert st["removed"] >= 20   # encounter flags of the generic kernel exercised
+    # the planets of the same run
+    S = gl.GlisseSim.from_workload(w, chunk_steps=200)
+    O = oracle_mod.OracleSim.from_workload(w)
+    log, ref = S.planet_log(HORIZON), O.planet_log(HORIZON)
+    S.close()
+    q, qr = log[:, :3 * npl].reshape(-1, npl, 3), ref[:, :3 * npl].reshape(-1, npl, 3)
+    d = np.linalg.norm(q - qr, axis=2) / np.linalg.norm(qr, axis=2)
+    record(dict(case=f"planet_log_chain_np{npl}", q_dev_max=float(d.max())))
+    assert d.max() <= 2e-11, d.max()
+
+
+def test_resume_from_read(gl, oracle_mod, record):
+    """Checkpoint / resume (the paper's multi-phase runs):
+    advance(a), glisse_read + glisse_read_planets, glisse_create from what was read, advance(b) equals
+    advance(a + b).  Not bit for bit — the planets go through heliocentric coordinates and back to
+    Jacobi — but to 1e-12; particles removed before the checkpoint stay out of the second sim."""
+    w = inputs.config(1)
+    a, b = 300, 500
+    S = gl.GlisseSim.from_workload(w, chunk_steps=128)
+    S.advance(a)
+    p, v, f, r = S.read()
+    qp, qv = S.read_planets()
+    S.advance(b)
+    p2, v2, f2, r2 = S.read()
+    qp2, qv2 = S.read_planets()
+    S.close()
+    keep = f == 0
+    assert 0 < (~keep).sum() < 100
+    R = gl.GlisseSim(w.gm_star, w.gm_planet, qp, qv, w.planet_rcrit, np.ascontiguousarray(p[:, keep]),
+                     np.ascontiguousarray(v[:, keep]), w.dt, r_min=w.r_min, r_max=w.r_max, chunk_steps=128)
+    R.advance(b)
+    p3, v3, f3, r3 = R.read()
+    qp3, qv3 = R.read_planets()
+    R.close()
+    assert np.array_equal(f3, f2[keep])
+    assert np.array_equal(np.where(r3 >= 0, r3 + a, r3), r2[keep])      # the resumed sim counts from 0
+    dev = max(_dev(p3, p2[:, keep]).max(), _dev(v3, v2[:, keep]).max())
+    dpl = max(np.max(np.linalg.norm(qp3 - qp2, axis=1) / np.linalg.norm(qp2, axis=1)),
+              np.max(np.linalg.norm(qv3 - qv2, axis=1) / np.linalg.norm(qv2, axis=1)))
+    record(dict(case="resume_c1_300+500", dev_max=float(dev), planet_dev_max=float(dpl)))
+    assert dev <= 1e-12 and dpl <= 1e-12, (dev, dpl)
 
 
 def test_particle_kernel_alone_with_oracle_log(gl, oracle_mod):
@@ -264,6 +354,162 @@ def test_particle_kernel_alone_with_oracle_log(gl, oracle_mod):
     with pytest.raises(gl.GlisseError):   # the internal planet clock is stale now
         S.advance(1)
     S.close()
+
+
+def test_external_log_is_streamed_and_the_planet_clock_can_be_reseeded(gl, oracle_mod, record):
+    """glisse_advance_with_log as a feature: a 2,000-step history (host array,
+    then a device tensor) streamed through the two log buffers in K = 300 chunks, asynchronously;
+    with the library's own planet log as the history the result is bit-identical to glisse_advance.
+    Then glisse_set_planets re-seeds the internal clock and glisse_advance carries on."""
+    import torch
+    w = inputs.config(1)
+    ref, _, _ = _run_gpu(gl, w, [2000], chunk_steps=300)
+    A = gl.GlisseSim.from_workload(w, chunk_steps=300)
+    log = A.planet_log(2000)
+    A.advance(2000)
+    qp, qv = A.read_planets()
+    A.advance(500)
+    ref2 = A.read()
+    A.close()
+    for make in (lambda x: x, lambda x: torch.from_numpy(x).cuda()):
+        S = gl.GlisseSim.from_workload(w, chunk_steps=300)
+        S.advance_with_log(700, make(log[:701]))            # two calls, the second starts mid-history
+        S.advance_with_log(1300, make(np.ascontiguousarray(log[700:])))
+        out = S.read()
+        for a, b in zip(out, ref):
+            assert np.array_equal(a, b)
+        assert S.step() == 2000
+        with pytest.raises(gl.GlisseError):                  # the internal planet clock is stale ...
+            S.advance(1)
+        with pytest.raises(gl.GlisseError):
+            S.read_planets()
+        S.set_planets(qp, qv)                                # ... until it is re-seeded
+        S.advance(500)
+        out2 = S.read()
+        S.close()
+        assert np.array_equal(out2[2], ref2[2]) and np.array_equal(out2[3], ref2[3])
+        dev = max(_dev(out2[0], ref2[0]).max(), _dev(out2[1], ref2[1]).max())
+        record(dict(case="reseeded_planet_clock_500_steps", dev_max=float(dev)))
+        assert dev <= 1e-12     # heliocentric -> Jacobi -> heliocentric round trip of the planets
+
+
+def test_periodic_output_ring(gl):
+    """params.snapshot_chunks ("copied back to the CPU after a user-configurable number of
+    planetary chunk calculations"): ONE glisse_advance of 10 chunks emits a snapshot every 2 chunks
+    into the caller's ring with no host round trip; every slot must hold, bit for bit, what a
+    glisse_snapshot taken by hand at that step returns, and slot_step names the step."""
+    import torch
+    w = inputs.config(5, n_particles=5000)
+    K = 64
+    n = w.n_particles
+    data = torch.empty((5, 6, n), dtype=torch.float64).pin_memory()
+    flag = torch.empty((5, n), dtype=torch.int32).pin_memory()
+    rst = torch.empty((5, n), dtype=torch.int64).pin_memory()
+    steps = torch.full((5,), -1, dtype=torch.int64).pin_memory()
+    S = gl.GlisseSim.from_workload(w, chunk_steps=K, snapshot_chunks=2)
+    S.snapshot_ring("cartesian", 5, data.numpy(), flag.numpy(), rst.numpy(), steps.numpy())
+    S.advance(10 * K)
+    assert S.snapshots_emitted() == 5
+    S.snapshot_wait()
+    S.close()
+    assert steps.tolist() == [2 * K, 4 * K, 6 * K, 8 * K, 10 * K]
+    M = gl.GlisseSim.from_workload(w, chunk_steps=K)
+    for k in range(5):
+        M.advance(2 * K)
+        d, f, r = M.snapshot("cartesian")
+        M.snapshot_wait()
+        assert np.array_equal(data[k].numpy(), d) and np.array_equal(flag[k].numpy(), f)
+        assert np.array_equal(rst[k].numpy(), r)
+    M.close()
+    assert (flag[4] != 0).sum() > 20
+    # a ring smaller than the number of snapshots wraps round; elements kind; detaching stops the output
+    S = gl.GlisseSim.from_workload(w, chunk_steps=K, snapshot_chunks=1)
+    d2, f2, r2, s2 = S.snapshot_ring("elements", 2)
+    S.advance(3 * K)
+    S.snapshot_wait()
+    assert list(s2) == [3 * K, 2 * K] and S.snapshots_emitted() == 3
+    el, _, _ = S.snapshot("elements")
+    S.snapshot_wait()
+    assert np.array_equal(d2[0], el, equal_nan=True)
+    S.snapshot_ring("elements", 0)
+    S.advance(K)
+    assert S.snapshots_emitted() == 0
+    S.close()
+
+
+def test_libration_record_matches_oracle(gl, oracle_mod, record):
+    """the device's running libration record — window test,
+    running extrema of phi, amplitude from successive turning points — built by ONE long glisse_advance
+    that samples phi_31 every chunk (params.resonance_chunks = 1), against the oracle's summary of the
+    phi series the ORACLE integrates and evaluates itself, 60 samples."""
+    w = inputs.config(3, n_particles=1536)
+    K, n_samp = 40, 60
+    nep, window = 3, np.deg2rad(10.0)
+    mu_pl = w.gm_star + w.gm_planet[nep]
+    S = gl.GlisseSim.from_workload(w, chunk_steps=K, resonance_chunks=1)
+    S.resonance_begin(nep, 3, 1, window)
+    S.advance(K * n_samp)
+    s0, s180, phi_last, ns = S.resonance_read()
+    lo, hi, amean, amax, namp = S.libration_read()
+    _, _, f, _ = S.read()
+    S.close()
+    assert ns == n_samp
+    O = oracle_mod.OracleSim.from_workload(w)
+    series = np.empty((n_samp, w.n_particles))
+    for k in range(n_samp):
+        O.advance(K)
+        pos, vel, fo, _ = O.read()
+        qp, qv = O.read_planets()
+        series[k] = oracle_mod.resonant_argument(w.gm_star, pos, vel, mu_pl, qp[nep], qv[nep], 3, 1)
+    assert not fo.any() and not f.any()        # config 3 loses nobody: every particle has all 60 samples
+    ref = oracle_mod.libration_summary(series, window)
+    # particles whose series has a near-tie between neighbours, or a sample on a window edge, may
+    # legitimately differ (the two phi series agree to ~1e-10, not bit for bit): leave those out
+    gaps = np.abs(np.diff(series, axis=0)).min(axis=0)
+    d0 = np.minimum(series, 2 * np.pi - series)
+    edge = (np.abs(d0 - window) < 1e-8).any(axis=0) | (np.abs(np.abs(series - np.pi) - window) < 1e-8).any(axis=0)
+    ok = (gaps > 1e-8) & ~edge
+    assert ok.mean() > 0.98
+    assert np.array_equal(s0.astype(bool)[ok], ref["seen0"][ok]) and np.array_equal(s180.astype(bool)[ok], ref["seen180"][ok])
+    assert np.array_equal(namp[ok], ref["n_amp"][ok])
+    has = ok & (ref["n_amp"] > 0)
+    el = oracle_mod.elements(w.gm_star, pos, vel)
+    scale = 1.0 / np.maximum(el[1], 1e-3)      # omega and M are conditioned by e
+    worst = dict(phi_min=float(np.max(np.abs(lo - ref["phi_min"])[ok] / scale[ok])),
+                 phi_max=float(np.max(np.abs(hi - ref["phi_max"])[ok] / scale[ok])),
+                 amp_mean=float(np.max(np.abs(amean - ref["amp_mean"])[has] / scale[has])),
+                 amp_max=float(np.max(np.abs(amax - ref["amp_max"])[has] / scale[has])),
+                 phi_last=float(np.max(np.abs((phi_last - series[-1] + np.pi) % (2 * np.pi) - np.pi)[ok] / scale[ok])))
+    record(dict(case="libration_c3_60_samples", n=int(ok.sum()), with_amplitude=int(has.sum()), **worst))
+    assert has.sum() > 1000 and max(worst.values()) < 1e-9, worst
+    assert np.isnan(amean[ok & (ref["n_amp"] == 0)]).all()
+    assert (ref["seen0"][ok]).any() and (~ref["seen0"][ok]).any()
+
+
+def test_iteration_binning_is_invisible_and_groups_hard_orbits(gl, oracle_mod, record):
+    """with params.bin_iterations the survivors are ordered by the
+    Kepler-solver iterations their orbit can need, hardest first.  Results must be BIT-identical to the
+    unbinned run (and so keep their parity with the oracle), and the warps must do less solver work:
+    the mean number of fast-solver iterations per warp-step (glisse_solver_stats) must drop."""
+    w = inputs.config(5, n_particles=40_000)
+    out = {}
+    for binned in (0, 1):
+        S = gl.GlisseSim.from_workload(w, chunk_steps=128, resync_chunks=1, bin_iterations=binned)
+        S.solver_stats_enable(True)
+        S.advance(1024)
+        calls, iters, slow = S.solver_stats()
+        out[binned] = (S.read(), S.particle_steps(), calls, iters, slow)
+        S.close()
+    for a, b in zip(out[0][0], out[1][0]):
+        assert np.array_equal(a, b)
+    assert out[0][1] == out[1][1]
+    mean0, mean1 = out[0][3] / out[0][2], out[1][3] / out[1][2]
+    record(dict(case="binning_c5_40000", warp_steps=[out[0][2], out[1][2]], mean_fast_iters_per_warp_step=[mean0, mean1],
+                slow_path_fraction=[out[0][4] / out[0][2], out[1][4] / out[1][2]]))
+    assert mean1 < mean0 - 0.05
+    # and the binned run against the oracle on a subset the oracle finishes quickly
+    ws = inputs.config(5, n_particles=4096 + 3)
+    _check_parity(gl, oracle_mod, record, "c5_4099_binned", ws, min_plain=0.80, chunk_steps=128, bin_iterations=1)
 
 
 def test_surviving_fraction_long_run_config5_shape(gl, oracle_mod):
@@ -316,7 +562,14 @@ def test_bit_exact_under_chunking_splitting_and_compaction(gl):
                       (dict(chunk_steps=1024, resync_chunks=1), [63, 2, 62, 130, 443]),
                       (dict(chunk_steps=256, resync_chunks=1), [700]),
                       (dict(chunk_steps=300, resync_chunks=0), [1, 299, 301, 99]),
-                      (dict(chunk_steps=100, resync_chunks=0), [699, 1])]:
+                      (dict(chunk_steps=100, resync_chunks=0), [699, 1]),
+                      # launch chaining (segment_steps): one launch per chunk, many short chained launches,
+                      # a segment length that does not divide the chunk; with and without binning
+                      (dict(chunk_steps=1024, resync_chunks=1, segment_steps=0), [700]),
+                      (dict(chunk_steps=1024, resync_chunks=1, segment_steps=16), [700]),
+                      (dict(chunk_steps=512, resync_chunks=2, segment_steps=100), [300, 400]),
+                      (dict(chunk_steps=256, resync_chunks=1, segment_steps=64, bin_iterations=1), [700]),
+                      (dict(chunk_steps=1024, resync_chunks=0, segment_steps=37, bin_iterations=1), [700])]:
         out, ps, pl = _run_gpu(gl, w, sched, **kw)
         for a, b in zip(out, ref):
             assert np.array_equal(a, b), (kw, sched)
@@ -513,29 +766,59 @@ def test_invalid_arguments_are_refused(gl):
 
 
 def test_planet_failure_is_reported(gl):
-    """A planet on a hyperbolic orbit violates PAPER.md:67: GLISSE_EPLANET at the next sync."""
+    """A planet on a hyperbolic orbit violates PAPER.md:67: GLISSE_EPLANET once the particles have gone
+    past the failed step — not before: the look-ahead planet kernel has already failed when the state
+    at step 0 is read, and that state is valid."""
     w = inputs.config(1).subset(8)
     pv = w.planet_vel.copy()
     pv[1] *= 2.0
+    S = gl.GlisseSim(w.gm_star, w.gm_planet, w.planet_pos, pv, None, w.pos, w.vel, w.dt)
+    p, v, f, r = S.read()                       # step 0: readable
+    assert np.array_equal(p, w.pos) and np.array_equal(v, w.vel)
+    with pytest.raises(gl.GlisseError) as ei:   # a look-ahead that fails says so without poisoning the sim
+        S.planet_log(5)
+    assert ei.value.status == gl.EPLANET
+    S.read()
     with pytest.raises(gl.GlisseError) as ei:
-        S = gl.GlisseSim(w.gm_star, w.gm_planet, w.planet_pos, pv, None, w.pos, w.vel, w.dt)
         S.advance(10)
         S.read()
     assert ei.value.status == gl.EPLANET
+    with pytest.raises(gl.GlisseError):         # sticky from here on
+        S.read()
+
+
+def test_kepler_tol_below_roundoff_goes_through_the_definition(gl, oracle_mod):
+    """kepler_tol = 1e-16 asks the residual test to decide on roundoff: the fast solver (which does not
+    evaluate the residual) must stand aside, and flag 3 must come out as the oracle's does on all but
+    the bodies whose residual sits within roundoff of the tolerance."""
+    w = inputs.config(5, n_particles=2000)
+    kw = dict(kepler_tol=1e-16)
+    (po, vo, fo, ro), _ = _oracle_run(oracle_mod, w, 30, **kw)
+    S = gl.GlisseSim.from_workload(w, **kw)
+    S.advance(30)
+    p, v, f, r = S.read()
+    S.close()
+    assert (fo == 3).sum() > 200                       # the tolerance really bites
+    assert ((f == 3) == (fo == 3)).mean() > 0.8        # decided by the same test (roundoff differs)
+    S = gl.GlisseSim.from_workload(w)                  # the default tolerance flags nothing here
+    S.advance(30)
+    assert (S.read()[2] == 3).sum() == 0
+    S.close()
 
 
 # ---------------------------------------------------------------------------------------------------
 # full BASELINE.json sizes, in the launch configuration bench.py times, on sampled particles
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("name", ["c2", "1m_x4", "c4", "c5"])
-def test_full_size_sampled_parity(gl, oracle_mod, name):
+@pytest.mark.parametrize("name", ["c2", "1m_x4", "c3", "c4", "c5"])
+def test_full_size_sampled_parity(gl, oracle_mod, record, name):
     """Particles never interact, so the oracle can compute any sample of a full-size
-    run one by one: 384 seeded indices out of N, full planet system, 1,000 steps."""
+    run one by one: 2,048 seeded indices out of N (first and last particle included), full planet
+    system, 1,000 steps, in the launch configuration bench.py times."""
     import dataclasses
-    w = {"c2": lambda: inputs.config(2), "1m_x4": inputs.one_m_four_planets, "c4": lambda: inputs.config(4),
-         "c5": lambda: inputs.config(5)}[name]()
+    w = {"c2": lambda: inputs.config(2), "1m_x4": inputs.one_m_four_planets, "c3": lambda: inputs.config(3),
+         "c4": lambda: inputs.config(4), "c5": lambda: inputs.config(5)}[name]()
     n = w.n_particles
-    idx = np.sort(np.random.default_rng(99).choice(n, 384, replace=False))
+    idx = np.sort(np.random.default_rng(99).choice(n, 2048, replace=False))
     idx[0], idx[-1] = 0, n - 1
     S = gl.GlisseSim.from_workload(w, chunk_steps=1024, resync_chunks=1)   # bench.py's configuration
     S.advance(HORIZON)
@@ -549,14 +832,10 @@ def test_full_size_sampled_parity(gl, oracle_mod, name):
     assert ps == int(np.where(r < 0, HORIZON, r + ((f == 3) | (f == 4))).sum())
     ws = dataclasses.replace(w, pos=np.ascontiguousarray(w.pos[:, idx]), vel=np.ascontiguousarray(w.vel[:, idx]))
     (po, vo, fo, ro), _ = _oracle_run(oracle_mod, ws, HORIZON)
-    sigma, ok = _sensitivity(oracle_mod, ws, HORIZON, po, vo, fo, ro)
-    assert np.array_equal(f[idx][ok], fo[ok]) and np.array_equal(r[idx][ok], ro[ok])
+    sigma, agree = _sensitivity(oracle_mod, ws, HORIZON, po, vo, fo, ro)
     dev = np.maximum(_dev(p[:, idx], po), _dev(v[:, idx], vo))
-    bound = np.maximum(TOL, TWIN_FACTOR * sigma)
-    assert np.all(dev[ok] <= bound[ok]), float(np.max(dev[ok] / bound[ok]))
-    assert (ok & (bound <= TOL)).sum() >= (0.75 if name == "c5" else 0.99) * len(idx)
-    if name in ("c2", "1m_x4"):
-        assert ok.all() and dev.max() <= TOL
+    _judge(record, f"full_{name}", dev, sigma, agree, f[idx], r[idx], fo, ro,
+           expect_quiet=name in ("c2", "1m_x4", "c3"), min_plain=0.80 if name == "c5" else 0.99)
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -610,6 +889,88 @@ def test_snapshot_elements_match_oracle(gl, oracle_mod):
     assert np.max(ang(el[3] + el[4], ref[3] + ref[4]) * e) < 1e-11          # longitude of pericentre
     assert np.max(ang((el[3] + el[4] + el[5])[bound], (ref[3] + ref[4] + ref[5])[bound])) < 1e-11  # mean longitude
     assert ((el[3:5] >= 0) & (el[3:5] < 2 * np.pi)).all()
+
+
+def test_snapshot_elements_match_textbook_construction(gl, record):
+    """The device's osculating elements against the TEXTBOOK, not against the oracle: states are built
+    here from chosen (a, e, i, Omega, omega, f) by the perifocal construction and rotations (tests/
+    orbital.py, Murray & Dermott eq. 2.119-2.122 — the construction T9 pins the oracle with), fed to
+    glisse_create, and read back by an ELEMENTS snapshot at step 0.  Special cases per
+    include/glisse.h: equatorial, circular, retrograde, hyperbolic."""
+    from tests.orbital import angle_diff, state_from_elements
+    mu = inputs.G
+    rng = np.random.default_rng(9)
+    n = 4000
+    want = np.empty((6, n))
+    pos, vel = np.empty((3, n)), np.empty((3, n))
+    for k in range(n):
+        a, e = rng.uniform(0.5, 80.0), rng.uniform(0.01, 0.9)
+        inc, Om, om, f = rng.uniform(0.05, 3.0), *rng.uniform(0.0, 2.0 * np.pi, 3)
+        pos[:, k], vel[:, k], M = state_from_elements(mu, a, e, inc, Om, om, f)
+        want[:, k] = (a, e, inc, Om, om, M)
+    # special cases appended: pericentre on +x of an equatorial orbit; circular equatorial a quarter turn
+    # on; the same retrograde; hyperbolic
+    a0, e0 = 30.0, 0.25
+    sp = [([a0 * (1 - e0), 0, 0], [0, np.sqrt(mu * (1 + e0) / (a0 * (1 - e0))), 0]),
+          ([0, 7.0, 0], [-np.sqrt(mu / 7.0), 0, 0]),
+          ([0, 7.0, 0], [np.sqrt(mu / 7.0), 0, 0]),
+          ([0, 7.0, 0], [-2.0 * np.sqrt(mu / 7.0), 0, 0])]
+    pos = np.concatenate([pos, np.array([s_[0] for s_ in sp], dtype=float).T], axis=1)
+    vel = np.concatenate([vel, np.array([s_[1] for s_ in sp], dtype=float).T], axis=1)
+    S = gl.GlisseSim(mu, [], np.zeros((0, 3)), np.zeros((0, 3)), None, pos, vel, 180.0)
+    el, flag, _ = S.snapshot("elements")
+    S.snapshot_wait()
+    S.close()
+    assert not flag.any()
+    g = el[:, :n]
+    si, e = np.sin(want[2]), want[1]
+    worst = dict(a=float(np.max(np.abs(g[0] / want[0] - 1.0))), e=float(np.max(np.abs(g[1] - want[1]))),
+                 inc=float(np.max(np.abs(g[2] - want[2]))), Omega_sin_i=float(np.max(angle_diff(g[3], want[3]) * si)),
+                 omega_e_sin_i=float(np.max(angle_diff(g[4], want[4]) * e * si)),
+                 M_e=float(np.max(angle_diff(g[5], want[5]) * e)))
+    record(dict(case="device_elements_vs_perifocal_construction", n=n, **worst))
+    assert max(worst.values()) < 5e-13, worst          # the bound T9 holds the oracle to
+    assert ((g[3:] >= 0) & (g[3:] < 2 * np.pi)).all()
+    s0, s1, s2, s3 = (el[:, n + k] for k in range(4))
+    assert abs(s0[0] - a0) < 1e-12 and abs(s0[1] - e0) < 1e-14 and s0[2] == 0.0 and s0[3] == 0.0
+    assert min(s0[4], 2 * np.pi - s0[4]) < 1e-14 and min(s0[5], 2 * np.pi - s0[5]) < 1e-14
+    assert abs(s1[0] - 7.0) < 1e-12 and s1[1] < 1e-15 and s1[2] == 0.0 and s1[3] == 0.0
+    assert angle_diff(s1[4] + s1[5], np.pi / 2) < 1e-12          # omega = 0 by convention, M = the longitude
+    assert abs(s2[2] - np.pi) < 1e-15                              # retrograde
+    assert s3[0] < 0 and s3[1] > 1 and np.isnan(s3[5])             # hyperbolic: M undefined
+
+
+def test_resonant_argument_matches_textbook_formula(gl, record):
+    """phi = p lambda - q lambda_pl - (p - q) varpi of the device against the formula typed out here on
+    CHOSEN elements (not via the oracle): one planet and particles built by the perifocal construction,
+    sampled at step 0."""
+    from tests.orbital import angle_diff, state_from_elements
+    mu = inputs.G
+    m_pl = 5.1514e-5
+    mu_pl = mu * (1.0 + m_pl)
+    rng = np.random.default_rng(10)
+    ep, ip, Op, wp, fp = 0.01, 0.03, *rng.uniform(0, 2 * np.pi, 3)
+    rp, vp, Mp = state_from_elements(mu_pl, 30.1, ep, ip, Op, wp, fp)
+    n = 1500
+    pos, vel = np.empty((3, n)), np.empty((3, n))
+    lam, varpi = np.empty(n), np.empty(n)
+    ecc = np.empty(n)
+    for k in range(n):
+        e, inc, Om, om, f = rng.uniform(0.05, 0.6), rng.uniform(0.1, 1.0), *rng.uniform(0, 2 * np.pi, 3)
+        pos[:, k], vel[:, k], M = state_from_elements(mu, rng.uniform(40.0, 70.0), e, inc, Om, om, f)
+        lam[k], varpi[k], ecc[k] = Om + om + M, Om + om, e
+    worst = 0.0
+    for p, q in ((3, 1), (5, 2), (3, 2)):
+        S = gl.GlisseSim(mu, [mu * m_pl], rp[None, :], vp[None, :], None, pos, vel, 180.0)
+        S.resonance_begin(0, p, q, np.deg2rad(10.0))
+        S.resonance_sample()
+        _, _, phi, ns = S.resonance_read()[:4]
+        S.close()
+        want = (p * lam - q * (Op + wp + Mp) - (p - q) * varpi) % (2 * np.pi)
+        worst = max(worst, float(np.max(angle_diff(phi, want))))
+        assert ns == 1
+    record(dict(case="device_phi_vs_formula", n=n, dev_max=worst))
+    assert worst < 1e-10 / ep        # T10's bound: the planet's own M and omega are conditioned by e_pl = 0.01
 
 
 def test_snapshot_to_device_buffers_and_bad_kind(gl):

@@ -10,6 +10,7 @@ from scipy.integrate import solve_ivp
 
 from paper_2011_03484_b200 import inputs
 from tests.orbital import angle_diff, cartesian_to_elements
+from tests.orbital import state_from_elements as _state_from_elements
 
 G = inputs.G
 
@@ -444,26 +445,6 @@ def test_advance_with_own_log_is_identical(oracle_mod):
 # ---------------------------------------------------------------------------------------------------
 # T9  osculating elements (snapshot output) against the textbook construction
 # ---------------------------------------------------------------------------------------------------
-def _state_from_elements(mu, a, e, inc, Om, om, f):
-    """Perifocal state at true anomaly f rotated by R_z(Om) R_x(inc) R_z(om), written out here
-    (Murray & Dermott eq. 2.119-2.122); returns r, v and the mean anomaly of f."""
-    p = a * (1.0 - e * e)
-    r = p / (1.0 + e * np.cos(f))
-    rp = np.array([r * np.cos(f), r * np.sin(f), 0.0])
-    vp = np.sqrt(mu / p) * np.array([-np.sin(f), e + np.cos(f), 0.0])
-
-    def rz(t):
-        return np.array([[np.cos(t), -np.sin(t), 0], [np.sin(t), np.cos(t), 0], [0, 0, 1.0]])
-
-    def rx(t):
-        return np.array([[1.0, 0, 0], [0, np.cos(t), -np.sin(t)], [0, np.sin(t), np.cos(t)]])
-
-    R = rz(Om) @ rx(inc) @ rz(om)
-    E = 2.0 * np.arctan2(np.sqrt(1.0 - e) * np.sin(f / 2.0), np.sqrt(1.0 + e) * np.cos(f / 2.0))
-    M = (E - e * np.sin(E)) % (2.0 * np.pi)
-    return R @ rp, R @ vp, M
-
-
 def test_T9_elements_match_textbook_construction(oracle_mod):
     mu = inputs.G
     rng = np.random.default_rng(9)
@@ -539,3 +520,47 @@ def test_T10_resonant_argument(oracle_mod):
         _, rp, vp = oracle_mod.kepler_drift(mu_pl, rp, vp, 180.0)
     phi1 = oracle_mod.resonant_argument(mu, r[:, None], v[:, None], mu_pl, rp, vp, 3, 1)[0]
     assert angle_diff(phi1, phi0) < 1e-9
+
+
+# ---------------------------------------------------------------------------------------------------
+# T11  libration summary (PAPER.md:264 window test, PAPER.md:288 amplitude from successive extrema)
+#      against constructed librators (closed form) and hand-worked series
+# ---------------------------------------------------------------------------------------------------
+def test_T11_libration_summary_on_constructed_series(oracle_mod):
+    window = np.deg2rad(10.0)
+    # phi(t) = pi + A sin(w t), m samples per period: the turning points are the samples nearest the
+    # true extrema, at most half a sample away, so every amplitude sample lies in [A cos(pi/m), A]
+    for A, m, periods in ((1.0, 40, 6.3), (0.3, 25, 11.5), (2.9, 64, 4.2)):
+        k = np.arange(int(m * periods))
+        phi = np.pi + A * np.sin(2.0 * np.pi * k / m + 0.4)
+        r = oracle_mod.libration_summary(phi, window)
+        shrink = np.cos(np.pi / m)
+        assert A * shrink <= r["amp_mean"] <= A and A * shrink <= r["amp_max"] <= A
+        assert np.pi - A <= r["phi_min"] <= np.pi - A * shrink and np.pi + A * shrink <= r["phi_max"] <= np.pi + A
+        # one turning point per half period (phase 0.4: the first lies (pi/2 - 0.4)/(2 pi) of a period in)
+        n_turn = int(np.floor(2.0 * (periods - 1.0 / m - (np.pi / 2 - 0.4) / (2 * np.pi)))) + 1
+        assert r["n_amp"] == n_turn - 1
+        assert bool(r["seen180"]) and bool(r["seen0"]) == (A > np.pi - window)
+    # hand-worked: rises to 3 (max), falls to 1 (min), rises through a plateau to 3 (max), falls
+    r = oracle_mod.libration_summary(np.array([1.0, 2.0, 3.0, 2.0, 1.0, 2.0, 2.0, 3.0, 1.0]), 0.05)
+    assert r["n_amp"] == 2 and r["amp_mean"] == 1.0 and r["amp_max"] == 1.0
+    assert r["phi_min"] == 1.0 and r["phi_max"] == 3.0 and not r["seen0"] and not r["seen180"]
+    # a plateau at the top counts once, with the plateau's value; unequal swings average
+    r = oracle_mod.libration_summary(np.array([1.0, 3.0, 3.0, 0.5, 2.5, 2.0]), 0.05)
+    assert r["n_amp"] == 2 and r["amp_mean"] == 0.5 * (1.25 + 1.0) and r["amp_max"] == 1.25
+    # monotonic: no turning point, no amplitude
+    r = oracle_mod.libration_summary(np.linspace(0.5, 3.0, 30), 0.05)
+    assert r["n_amp"] == 0 and np.isnan(r["amp_mean"]) and r["amp_max"] == 0.0
+    # circulation: phi = 0.3 k mod 2 pi wraps every ~21 samples; each wrap is a maximum just below 2 pi
+    # followed at once by a minimum just above 0, so every amplitude sample is close to pi
+    phi = np.mod(0.3 * np.arange(200), 2 * np.pi)
+    r = oracle_mod.libration_summary(phi, window)
+    assert r["seen0"] and r["seen180"] and r["n_amp"] >= 15
+    assert np.pi - 0.3 <= r["amp_mean"] <= np.pi and r["amp_max"] <= np.pi
+    # window edges are strict: a sample exactly `window` from pi does not count
+    r = oracle_mod.libration_summary(np.array([np.pi + 0.25, np.pi - 0.25]), 0.25)
+    assert not r["seen180"]
+    r = oracle_mod.libration_summary(np.array([np.pi + 0.2499]), 0.25)
+    assert r["seen180"] and not r["seen0"]
+    r = oracle_mod.libration_summary(np.array([2 * np.pi - 0.1]), 0.25)
+    assert r["seen0"]
