@@ -6,8 +6,8 @@
 
 A "step" is one pass of the whole hot path over one chunk: the planet-history kernel writes
 CHUNK = 1,024 integrator steps of planet positions (one chunk ahead, on its own stream), the
-particle kernel advances every active particle through those 1,024 steps (as four chained launches
-of 256 steps), and the survivor compaction runs.
+particle kernel advances every active particle through those 1,024 steps (as eight chained launches
+of 128 steps), and the survivor compaction runs.
 Default workload: BASELINE.json north_star's target, 1,048,576 particles x 4 planets; the
 BASELINE.json configs[1..4] (c2, c3, c4, c5) are measured in the same run and reported under
 "workloads", each with its own roofline figures.
@@ -234,7 +234,7 @@ def roofline_of(name: str, n_planets: int, res: dict, peak_probe: float) -> dict
     achieved = fl * (res["psteps"] / runs) / (k_ms * 1e-3) / 1e12
     r = {"bound": "alu", "achieved": achieved, "peak": FP64_NOMINAL_TFLOPS, "unit": "TFLOP/s",
          "frac": achieved / FP64_NOMINAL_TFLOPS, "traffic": traffic,
-         "kernel": "particle_kernel (4 chained launches of 256 steps per chunk, timed together)",
+         "kernel": "particle_kernel (8 chained launches of 128 steps per chunk, timed together)",
          "kernel_ms_per_chunk": k_ms, "kernel_share_of_step": res["kernel_ms"] / res["ms"],
          "flops_per_particle_step": fl,
          "flops_source": "algorithmic: SURVEY.md 8(d) / DESIGN.md 7 count of the defined step with 2 Newton updates",
@@ -396,7 +396,7 @@ def run_ablations(binding, torch, device, flush):
     for name in ("c2", "1m_x4"):
         _, w = make_workload(name)
         out["long_advance_16_chunks_no_flush"][name] = {
-            str(sg): rate(w, steps=2, warmup=1, fl=None, chunks_per_step=16, segment_steps=sg) for sg in (0, 256)}
+            str(sg): rate(w, steps=2, warmup=1, fl=None, chunks_per_step=16, segment_steps=sg) for sg in (0, 128)}
     # fixed-count Newton of the definition (kepler_iters = 4 switches the fast solver off) vs the fast solver
     out["kepler_solver"] = {"fast_solver_iters5": rate(c2), "definition_newton_iters4": rate(c2, kepler_iters=4)}
     # config 5: resync on / off, binning on / off, after 8 warm-up chunks (about 20 % removed)
@@ -519,9 +519,9 @@ def rank_main(argv):
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": desc, "n_particles_per_gpu": w.n_particles, "n_planets": w.n_planets,
-                   "chunk_steps": CHUNK, "dt_days": w.dt, "resync_chunks": 1, "segment_steps": 256,
-                   "step": "one chunk of 1,024 integrator steps: planet-history + particle kernel (4 chained "
-                           "launches of 256 steps) + compaction",
+                   "chunk_steps": CHUNK, "dt_days": w.dt, "resync_chunks": 1, "segment_steps": 128,
+                   "step": "one chunk of 1,024 integrator steps: planet-history + particle kernel (8 chained "
+                           "launches of 128 steps) + compaction",
                    "l2": "flushed between timed steps (256 MiB write, untimed)",
                    "parallelism": "particles sharded across ranks, planets replicated, no collectives"},
         "nominal_particle_steps_per_s": w.n_particles * world * CHUNK * args.steps / (ms * 1e-3),

@@ -88,7 +88,7 @@ typedef struct {
                            (PAPER.md:127).  Performance only: results are bit-identical.       */
   int    segment_steps;    /* a chunk is issued as back-to-back launches of this many steps whose
                            warps hand particles on through per-group completion flags, so the
-                           tail of one launch is filled by the next; default 256,
+                           tail of one launch is filled by the next; default 128,
                            0 = one launch per chunk.  Performance only, results do not depend
                            on it                                                               */
 } glisse_params;

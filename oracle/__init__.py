@@ -32,7 +32,7 @@ def build(force: bool = False) -> str:
 
 class _Params(ctypes.Structure):
     _fields_ = [("r_min", c_double), ("r_max", c_double), ("kepler_iters", c_int),
-                ("kepler_tol", c_double)]
+                ("kepler_tol", c_double), ("scheme", c_int)]
 
 
 _lib = None
@@ -103,7 +103,7 @@ class OracleSim:
     """Same call sequence as the CUDA binding's GlisseSim: create / advance / read."""
 
     def __init__(self, gm_star, gm_planet, planet_pos, planet_vel, planet_rcrit, pos, vel, dt,
-                 r_min=0.0, r_max=float("inf"), kepler_iters=5, kepler_tol=1e-14):
+                 r_min=0.0, r_max=float("inf"), kepler_iters=5, kepler_tol=1e-14, scheme="kdk"):
         L = lib()
         gm_planet = _f64(gm_planet).reshape(-1)
         self.np_ = int(gm_planet.shape[0])
@@ -114,7 +114,8 @@ class OracleSim:
         vel = _f64(vel)
         assert pos.shape == vel.shape and pos.shape[0] == 3
         self.n = int(pos.shape[1])
-        prm = _Params(float(r_min), float(r_max), int(kepler_iters), float(kepler_tol))
+        prm = _Params(float(r_min), float(r_max), int(kepler_iters), float(kepler_tol),
+                      {"kdk": 0, "dkd": 1}[scheme])
         h = c_void_p()
         xs = [np.ascontiguousarray(pos[k]) for k in range(3)]
         vs = [np.ascontiguousarray(vel[k]) for k in range(3)]

@@ -46,6 +46,7 @@ struct Params {
   double r_min, r_max;
   int kepler_iters;
   double kepler_tol;
+  int scheme; /* 0 = kick-drift-kick, 1 = drift-kick-drift (BASELINE.json's wording, reading S20) */
 };
 
 /* ---------------------------------------------------------------------------------------------
@@ -251,6 +252,10 @@ struct Sim {
   Params P{};
   long long step = 0;
   long long particle_steps = 0;
+  /* drift-kick-drift only: q, qd above hold the planets at t_{step - 1/2} once step > 0 (the instants
+   * at which the scheme samples them); q0, qd0 keep the state at t_0 */
+  std::vector<double> q_half, qd_half;
+  bool half_started = false;
 };
 
 /* kick every active particle by h·a evaluated with planets (q, h0); `completed` = number of
@@ -270,12 +275,12 @@ void kick_particles(Sim& S, const double* q, const double h0[3], double h, long 
   }
 }
 
-void drift_particles(Sim& S) {
+void drift_particles(Sim& S, double dt) {
   for (long long i = 0; i < S.n; ++i) {
     if (S.flag[i] != ACTIVE) continue;
     double r[3] = {S.x[0][i], S.x[1][i], S.x[2][i]};
     double v[3] = {S.v[0][i], S.v[1][i], S.v[2][i]};
-    const int st = kepler_drift(S.gm0, r, v, S.dt, S.P.kepler_iters, S.P.kepler_tol);
+    const int st = kepler_drift(S.gm0, r, v, dt, S.P.kepler_iters, S.P.kepler_tol);
     if (st != ACTIVE) {
       S.flag[i] = st;
       S.rstep[i] = S.step; /* flagged during step `step`: that many steps were completed */
@@ -309,6 +314,7 @@ typedef struct {
   double r_min, r_max;
   int kepler_iters;
   double kepler_tol;
+  int scheme; /* 0 kick-drift-kick (default), 1 drift-kick-drift */
 } oracle_params;
 
 void oracle_default_params(oracle_params* p) {
@@ -317,6 +323,7 @@ void oracle_default_params(oracle_params* p) {
   p->r_max = std::numeric_limits<double>::infinity();
   p->kepler_iters = 5;   /* PAPER.md:123 */
   p->kepler_tol = 1e-14; /* PAPER.md:123 */
+  p->scheme = 0;
 }
 
 int oracle_log_stride(int n_planets) {
@@ -361,7 +368,8 @@ int oracle_create(oracle_sim** out, double gm_star, int n_planets, const double*
   oracle_params d;
   oracle_default_params(&d);
   if (params) d = *params;
-  if (d.kepler_iters < 0 || !(d.kepler_tol > 0.0)) { delete S; return -1; }
+  if (d.kepler_iters < 0 || !(d.kepler_tol > 0.0) || d.scheme < 0 || d.scheme > 1) { delete S; return -1; }
+  S->P.scheme = d.scheme;
   S->P.r_min = d.r_min;
   S->P.r_max = (std::isfinite(d.r_max) ? d.r_max : 0.0);
   S->P.kepler_iters = d.kepler_iters;
@@ -370,10 +378,46 @@ int oracle_create(oracle_sim** out, double gm_star, int n_planets, const double*
   return 0;
 }
 
+/* Drift-kick-drift variant (BASELINE.json north_star's wording; reading S20 of DESIGN.md §2): the same
+ * second-order splitting with the roles exchanged,
+ *   D1. drift every active particle for dt/2 (O2's routine);
+ *   D2. planets at the half step t_{s+1/2}: the planets are carried by the same Wisdom-Holman step as in
+ *       the kick-drift-kick scheme, started with ONE step of size dt/2 (t_0 -> t_{1/2}) and continued with
+ *       steps of size dt (t_{s-1/2} -> t_{s+1/2}), so that they are sampled where the kick needs them
+ *       (the log may hold the planets at whatever instants the scheme asks for);
+ *   D3. kick every active particle by dt a(r, q(t_{s+1/2})), tests O5 on this evaluation; a hit records
+ *       `step` completed steps and freezes the state of that instant (after D1, without this kick);
+ *   D4. drift for dt/2.
+ * A particle flagged in D1 or D4 keeps the state it had on entry to that drift. */
+static int advance_dkd(Sim& S, long long n_steps) {
+  const double hdt = 0.5 * S.dt;
+  double h0[3];
+  for (long long s = 0; s < n_steps; ++s) {
+    S.particle_steps += count_active(S);
+    drift_particles(S, hdt);                                                     /* D1 */
+    if (!S.half_started) {                                                       /* D2 */
+      S.q_half = S.q; S.qd_half = S.qd;
+      if (planet_step(S.np, S.gm0, S.gm.data(), S.q_half.data(), S.qd_half.data(), hdt)) return -4;
+      S.half_started = true;
+    } else {
+      if (planet_step(S.np, S.gm0, S.gm.data(), S.q_half.data(), S.qd_half.data(), S.dt)) return -4;
+    }
+    common_term_h0(S.np, S.gm.data(), S.q_half.data(), h0);
+    kick_particles(S, S.q_half.data(), h0, S.dt, S.step);                        /* D3 */
+    drift_particles(S, hdt);                                                     /* D4 */
+    S.step += 1;
+    /* planets at the integer time t_step, for oracle_read_planets: half a step on from t_{step-1/2} */
+    S.q = S.q_half; S.qd = S.qd_half;
+    if (planet_step(S.np, S.gm0, S.gm.data(), S.q.data(), S.qd.data(), hdt)) return -4;
+  }
+  return 0;
+}
+
 /* One full step s -> s+1 for everything, in the order O1, O2, O3, O4 of DESIGN.md §2. */
 int oracle_advance(oracle_sim* sim, long long n_steps) {
   if (!sim || n_steps < 0) return -1;
   Sim& S = *reinterpret_cast<Sim*>(sim);
+  if (S.P.scheme == 1) return advance_dkd(S, n_steps);
   const double h = 0.5 * S.dt;
   double h0[3];
   for (long long s = 0; s < n_steps; ++s) {
@@ -382,7 +426,7 @@ int oracle_advance(oracle_sim* sim, long long n_steps) {
     kick_particles(S, S.q.data(), h0, h, S.step);
     S.particle_steps += count_active(S);
     /* O2: drift */
-    drift_particles(S);
+    drift_particles(S, S.dt);
     /* O3: planets t_s -> t_{s+1} */
     const int bad = planet_step(S.np, S.gm0, S.gm.data(), S.q.data(), S.qd.data(), S.dt);
     if (bad) return -4;
@@ -402,6 +446,23 @@ int oracle_planet_log(oracle_sim* sim, long long n_steps, double* log) {
   const Sim& S = *reinterpret_cast<Sim*>(sim);
   std::vector<double> q = S.q, qd = S.qd;
   const int st = log_stride(S.np);
+  if (S.P.scheme == 1) {
+    /* drift-kick-drift: record k = planets at t_{step + k + 1/2}, k = 0 .. n_steps (D2) */
+    if (S.half_started) {
+      q = S.q_half; qd = S.qd_half;
+      if (planet_step(S.np, S.gm0, S.gm.data(), q.data(), qd.data(), S.dt)) return -4;
+    } else {
+      if (planet_step(S.np, S.gm0, S.gm.data(), q.data(), qd.data(), 0.5 * S.dt)) return -4;
+    }
+    for (long long s = 0; s <= n_steps; ++s) {
+      double* rec = log + s * st;
+      for (int i = 0; i < st; ++i) rec[i] = 0.0;
+      for (int i = 0; i < 3 * S.np; ++i) rec[i] = q[i];
+      common_term_h0(S.np, S.gm.data(), q.data(), rec + 3 * S.np);
+      if (s < n_steps && planet_step(S.np, S.gm0, S.gm.data(), q.data(), qd.data(), S.dt)) return -4;
+    }
+    return 0;
+  }
   for (long long s = 0; s <= n_steps; ++s) {
     double* rec = log + s * st;
     for (int i = 0; i < st; ++i) rec[i] = 0.0;
@@ -421,12 +482,23 @@ int oracle_advance_with_log(oracle_sim* sim, long long n_steps, const double* lo
   Sim& S = *reinterpret_cast<Sim*>(sim);
   const double h = 0.5 * S.dt;
   const int st = log_stride(S.np);
+  if (S.P.scheme == 1) { /* drift-kick-drift: record s = planets at the half step of step s */
+    for (long long s = 0; s < n_steps; ++s) {
+      const double* rec = log + s * st;
+      S.particle_steps += count_active(S);
+      drift_particles(S, h);
+      kick_particles(S, rec, rec + 3 * S.np, S.dt, S.step);
+      drift_particles(S, h);
+      S.step += 1;
+    }
+    return 0;
+  }
   for (long long s = 0; s < n_steps; ++s) {
     const double* r0 = log + s * st;
     const double* r1 = log + (s + 1) * st;
     kick_particles(S, r0, r0 + 3 * S.np, h, S.step);
     S.particle_steps += count_active(S);
-    drift_particles(S);
+    drift_particles(S, S.dt);
     kick_particles(S, r1, r1 + 3 * S.np, h, S.step + 1);
     S.step += 1;
   }
@@ -494,7 +566,7 @@ int oracle_planet_step(int np, double gm0, const double* gm, double* q, double* 
 /* O1/O5 on one particle: returns the flag, fills a[3] when it is 0. */
 int oracle_particle_accel(int np, const double* gm, const double* q, const double* rcrit,
                           double r_min, double r_max, const double* r, double* a) {
-  Params P{r_min, std::isfinite(r_max) ? r_max : 0.0, 5, 1e-14};
+  Params P{r_min, std::isfinite(r_max) ? r_max : 0.0, 5, 1e-14, 0};
   std::vector<double> rc2(np);
   for (int j = 0; j < np; ++j) rc2[j] = rcrit ? rcrit[j] * rcrit[j] : 0.0;
   double h0[3];

@@ -544,7 +544,7 @@ void glisse_default_params(glisse_params* p) {
   p->snapshot_chunks = 0;
   p->resonance_chunks = 0;
   p->bin_iterations = 0;
-  p->segment_steps = 256;
+  p->segment_steps = 128;
 }
 
 int glisse_log_stride(int n_planets) {

@@ -180,14 +180,14 @@ def _jacobi_constant(mu0, mu1, n1, r, v, q1, qd1):
             - mu1 / np.linalg.norm(r - q1, axis=-1) - n1 * (rb[..., 0] * vb[..., 1] - rb[..., 1] * vb[..., 0]))
 
 
-def _cr3bp_max_error(oracle_mod, dt, total_days, pos, vel, sample_every):
+def _cr3bp_max_error(oracle_mod, dt, total_days, pos, vel, sample_every, scheme="kdk"):
     m1 = 9.5479e-4
     mu0, mu1 = G, G * m1
     a1 = 5.2
     n1 = np.sqrt((mu0 + mu1) / a1 ** 3)
     q = np.array([[a1, 0.0, 0.0]])
     qd = np.array([[0.0, a1 * n1, 0.0]])
-    S = oracle_mod.OracleSim(mu0, [mu1], q, qd, None, pos.T, vel.T, dt)
+    S = oracle_mod.OracleSim(mu0, [mu1], q, qd, None, pos.T, vel.T, dt, scheme=scheme)
     C0 = _jacobi_constant(mu0, mu1, n1, pos, vel, q[0], qd[0])
     nblocks = int(round(total_days / dt / sample_every))
     errs = []
@@ -201,12 +201,15 @@ def _cr3bp_max_error(oracle_mod, dt, total_days, pos, vel, sample_every):
     return np.array(errs)  # [nblocks, N]
 
 
-def test_T4_cr3bp_jacobi_constant_bounded_and_second_order(oracle_mod):
+@pytest.mark.parametrize("scheme", ["kdk", "dkd"])
+def test_T4_cr3bp_jacobi_constant_bounded_and_second_order(oracle_mod, scheme):
+    """Both splittings (kick-drift-kick of PAPER.md:91-95; drift-kick-drift, reading S20) are symplectic
+    and of order 2: the same pin holds for each."""
     _, pos, vel = _random_particles(21, 48, 7.5, 12.0, 0.05, 0.0)  # planar, outside the planet
     total = 180.0 * 4000
-    e180 = _cr3bp_max_error(oracle_mod, 180.0, total, pos, vel, 100)
-    e90 = _cr3bp_max_error(oracle_mod, 90.0, total, pos, vel, 200)
-    e45 = _cr3bp_max_error(oracle_mod, 45.0, total, pos, vel, 400)
+    e180 = _cr3bp_max_error(oracle_mod, 180.0, total, pos, vel, 100, scheme)
+    e90 = _cr3bp_max_error(oracle_mod, 90.0, total, pos, vel, 200, scheme)
+    e45 = _cr3bp_max_error(oracle_mod, 45.0, total, pos, vel, 400, scheme)
     m180, m90, m45 = (np.median(e.max(axis=0)) for e in (e180, e90, e45))
     # symplectic: no secular drift -> the maximum over the second half is not larger than ~ the first half's
     half = e180.shape[0] // 2
@@ -221,16 +224,18 @@ def test_T4_cr3bp_jacobi_constant_bounded_and_second_order(oracle_mod):
 # ---------------------------------------------------------------------------------------------
 # T5  time reversal of the whole map (planets and particles)
 # ---------------------------------------------------------------------------------------------
-def test_T5_time_reversal(oracle_mod):
+@pytest.mark.parametrize("scheme", ["kdk", "dkd"])
+def test_T5_time_reversal(oracle_mod, scheme):
     w = inputs.config(1)
     _, pos, vel = _random_particles(31, 512, 23.0, 26.0, 0.02, 1.0)  # quiet band between Uranus and Neptune
     n = 1000
-    S = oracle_mod.OracleSim(w.gm_star, w.gm_planet, w.planet_pos, w.planet_vel, None, pos.T, vel.T, w.dt)
+    S = oracle_mod.OracleSim(w.gm_star, w.gm_planet, w.planet_pos, w.planet_vel, None, pos.T, vel.T, w.dt,
+                             scheme=scheme)
     S.advance(n)
     p1, v1, flag, _ = S.read()
     q1, qd1 = S.read_planets()
     assert np.all(flag == 0)
-    B = oracle_mod.OracleSim(w.gm_star, w.gm_planet, q1, qd1, None, p1, v1, -w.dt)
+    B = oracle_mod.OracleSim(w.gm_star, w.gm_planet, q1, qd1, None, p1, v1, -w.dt, scheme=scheme)
     B.advance(n)
     p2, v2, flag2, _ = B.read()
     q2, qd2 = B.read_planets()
@@ -271,7 +276,8 @@ def _direct_rhs(gm0, gm, npl, npart):
     return rhs
 
 
-def test_T6_second_order_convergence_to_direct_integration(oracle_mod):
+@pytest.mark.parametrize("scheme", ["kdk", "dkd"])
+def test_T6_second_order_convergence_to_direct_integration(oracle_mod, scheme):
     w = inputs.config(1)
     _, pos, vel = _random_particles(41, 6, 12.0, 27.0, 0.1, 3.0)
     T = 7200.0
@@ -283,7 +289,8 @@ def test_T6_second_order_convergence_to_direct_integration(oracle_mod):
     yT = sol.y[:, -1].reshape(-1, 6)
     errs_pl, errs_pa = [], []
     for dt in (180.0, 90.0, 45.0, 22.5):
-        S = oracle_mod.OracleSim(w.gm_star, w.gm_planet, w.planet_pos, w.planet_vel, None, pos.T, vel.T, dt)
+        S = oracle_mod.OracleSim(w.gm_star, w.gm_planet, w.planet_pos, w.planet_vel, None, pos.T, vel.T, dt,
+                                 scheme=scheme)
         S.advance(int(round(T / dt)))
         p, v, flag, _ = S.read()
         q, _qd = S.read_planets()
@@ -292,7 +299,14 @@ def test_T6_second_order_convergence_to_direct_integration(oracle_mod):
         errs_pa.append(np.max(np.linalg.norm(p.T - yT[npl:, :3], axis=1)))
     for errs in (errs_pl, errs_pa):
         ratios = [errs[i] / errs[i + 1] for i in range(3)]
-        assert all(3.6 < r < 4.4 for r in ratios), (errs, ratios)
+        if scheme == "kdk":
+            assert all(3.6 < r < 4.4 for r in ratios), (errs, ratios)
+        else:
+            # drift-kick-drift carries the planets as S(dt/2) S(dt)^(n-1) S(dt/2): still second order, but
+            # at dt = 180 d (24 steps per Jupiter orbit) the next term of the error expansion is still
+            # visible in the PLANETS' error; its ratio climbs to 4 as dt falls (measured 3.42, 3.77, 3.90; the
+            # particles' is 4.00 throughout)
+            assert 3.3 < ratios[0] < 4.4 and 3.6 < ratios[1] < 4.4 and 3.8 < ratios[2] < 4.2, (errs, ratios)
     assert errs_pl[-1] < 1e-4 and errs_pa[-1] < 1e-4
 
 
@@ -440,6 +454,50 @@ def test_advance_with_own_log_is_identical(oracle_mod):
         assert np.array_equal(x, y)
     qa, _ = A.read_planets()
     assert np.array_equal(log[200, :12].reshape(4, 3), qa)
+
+
+def test_dkd_removal_semantics_split_invariance_and_own_log(oracle_mod):
+    """Drift-kick-drift (reading S20): hand-worked removal cases, split-advance identity, and
+    advance_with_log on the scheme's own half-step planet log."""
+    w = inputs.config(1)
+    q, rc = w.planet_pos, w.planet_rcrit
+    pos, vel = w.pos[:, :8].copy(), w.vel[:, :8].copy()
+    # particle 0: unbound at t0 -> the first half drift refuses it: flag 4, step 0, state untouched
+    vel[:, 0] *= 1.2 * np.sqrt(2.0 * w.gm_star / np.linalg.norm(pos[:, 0])) / np.linalg.norm(vel[:, 0])
+    # particle 1: far outside r_max -> caught at the first force evaluation (after half a drift): flag 2,
+    # step 0, frozen at t_{1/2}: position moved, the velocity of a pure Kepler half drift (no kick)
+    pos[:, 1] = [900.0, 500.0, 0.0]
+    S = oracle_mod.OracleSim(w.gm_star, w.gm_planet, q, w.planet_vel, rc, pos, vel, w.dt, r_min=1.0, r_max=1000.0,
+                             scheme="dkd")
+    S.advance(3)
+    p, v, f, r = S.read()
+    assert f[0] == 4 and r[0] == 0 and np.array_equal(p[:, 0], pos[:, 0]) and np.array_equal(v[:, 0], vel[:, 0])
+    fl, r_half, v_half = oracle_mod.kepler_drift(w.gm_star, pos[:, 1], vel[:, 1], 0.5 * w.dt)
+    assert fl == 0 and f[1] == 2 and r[1] == 0
+    assert np.array_equal(p[:, 1], r_half) and np.array_equal(v[:, 1], v_half)
+    assert (f[2:] == 0).all() and S.particle_steps() == 2 + 6 * 3     # two particles started one step each
+    # split advances and the scheme's own log
+    A = oracle_mod.OracleSim.from_workload(w, scheme="dkd")
+    A.advance(150)
+    B = oracle_mod.OracleSim.from_workload(w, scheme="dkd")
+    B.advance(70); B.advance(0); B.advance(80)
+    C = oracle_mod.OracleSim.from_workload(w, scheme="dkd")
+    log = C.planet_log(150)
+    C.advance_with_log(150, log)
+    for x, y, z in zip(A.read(), B.read(), C.read()):
+        assert np.array_equal(x, y) and np.array_equal(x, z)
+    qa, qda = A.read_planets()
+    qb, qdb = B.read_planets()
+    assert np.array_equal(qa, qb) and np.array_equal(qda, qdb)
+    # the log's records are the planets at the half steps: record 0 = one Wisdom-Holman step of dt/2
+    st, q_half, _ = oracle_mod.planet_step(w.gm_star, w.gm_planet, w.planet_pos, w.planet_vel, 0.5 * w.dt)
+    assert st == 0 and np.array_equal(log[0, :12].reshape(4, 3), q_half)
+    # no planets at all: D(dt/2) D(dt/2) is the same Kepler flow as D(dt) to roundoff, so both schemes agree
+    K = oracle_mod.OracleSim(w.gm_star, [], np.zeros((0, 3)), np.zeros((0, 3)), None, w.pos, w.vel, w.dt)
+    D = oracle_mod.OracleSim(w.gm_star, [], np.zeros((0, 3)), np.zeros((0, 3)), None, w.pos, w.vel, w.dt, scheme="dkd")
+    K.advance(100); D.advance(100)
+    pk, pd = K.read()[0], D.read()[0]
+    assert np.max(np.linalg.norm(pk - pd, axis=0) / np.linalg.norm(pk, axis=0)) < 1e-12
 
 
 # ---------------------------------------------------------------------------------------------------
