@@ -55,6 +55,18 @@ extern "C" {
 
 #define GLISSE_MAX_PLANETS   32
 
+/* ---- splitting of the step (params.scheme) ------------------------------------------------- */
+#define GLISSE_SCHEME_KDK 0   /* kick 1/2 - drift - kick 1/2, planets sampled at the integer steps t_s:
+                                 the step list of PAPER.md:91-95 (default)                        */
+#define GLISSE_SCHEME_DKD 1   /* drift 1/2 - kick - drift 1/2, planets sampled at the half steps
+                                 t_{s+1/2}: BASELINE.json's wording of the same second-order
+                                 splitting (reading S20).  The planets are carried by the
+                                 same Wisdom-Holman step, started with one step of dt/2.  The tests
+                                 run at the one force evaluation of the step; a hit freezes the state
+                                 of that instant (after the first half drift).  Planet-log record k
+                                 then holds the planets at t_{s+k+1/2}; glisse_advance_with_log still
+                                 takes n_steps+1 records (the last one is not used).               */
+
 typedef struct glisse_sim glisse_sim; /* opaque */
 
 /* User-configurable quantities the paper names: Kepler iteration count (fn 5 at
@@ -86,6 +98,7 @@ typedef struct {
                            particles by the expected number of iterations ... the most eccentric
                            group would be launched first"); 0 (default): particle-ID order
                            (PAPER.md:127).  Performance only: results are bit-identical.       */
+  int    scheme;           /* GLISSE_SCHEME_KDK (default) or GLISSE_SCHEME_DKD                          */
   int    segment_steps;    /* a chunk is issued as back-to-back launches of this many steps whose
                            warps hand particles on through per-group completion flags, so the
                            tail of one launch is filled by the next; default 128,

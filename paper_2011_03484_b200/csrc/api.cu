@@ -103,7 +103,12 @@ struct glisse_sim {
   int status = GLISSE_OK;  // sticky
 
   PlanetSystem* d_sys = nullptr;
-  double* d_j0 = nullptr;    // Jacobi state the planet clock was (re-)seeded with
+  double* d_j0 = nullptr;    // Jacobi state the planet clock was (re-)seeded with (time of `origin`)
+  bool dkd = false;          // GLISSE_SCHEME_DKD: log records are the planets at the HALF steps
+  double* d_jhalf = nullptr; // DKD: Jacobi state at origin + 1/2 (start of the half-step clock)
+  double* d_jprev = nullptr; // DKD: Jacobi state at step - 1/2 (the last record the particles used)
+  double* d_scratch_log = nullptr;   // DKD: 2 records of a one-step planet launch
+  double* d_scratch_jlog = nullptr;
   double* d_ptmp = nullptr;  // [6 Np] scratch: heliocentric planet state in / out
   long long* d_fail = nullptr;  // [2] first failed planet step: [0] the sim's clock, [1] scratch of glisse_planet_log
   LogBuffer buf[2];
@@ -318,7 +323,7 @@ int launch_particles(glisse_sim* s, const double* log, int nsteps) {
     a.log = log + static_cast<size_t>(off) * s->stride;
     a.step0 = s->step + off;
     a.nsteps = m;
-    CKS(s, launch_particle_kernel(a, groups, !first, s->stats_on, s->q));
+    CKS(s, launch_particle_kernel(a, groups, !first, s->stats_on, s->dkd, s->q));
     s->launches += 1;
     s->chain_len += 1;
   }
@@ -383,6 +388,51 @@ int fill_log_buffer(glisse_sim* s, int b, const double* jin, long long start) {
   s->launches += 1;
   CKS(s, cudaEventRecord(B.ready, s->p));
   B.start = start;
+  return GLISSE_OK;
+}
+
+// (Re-)start the planet clock at step `start` from the synchronised Jacobi state in d_j0, into buffer 0.
+// KDK: record 0 is that state.  DKD: the log holds the planets at the half steps, so the clock starts
+// with ONE Wisdom-Holman step of dt/2 (a one-step planet launch into scratch) and goes on from there.
+int start_planet_clock(glisse_sim* s, long long start) {
+  s->origin = start;
+  s->cur = 0;
+  s->ahead = false;
+  const double* j0 = s->d_j0;
+  if (s->dkd && s->np > 0) {
+    CKS(s, launch_planet_kernel(s->d_sys, s->np, s->d_j0, s->d_scratch_log, s->d_scratch_jlog, 1, 0.5 * s->dt, start,
+                                s->d_fail, 0, s->p));
+    s->launches += 1;
+    CKS(s, cudaMemcpyAsync(s->d_jhalf, s->d_scratch_jlog + 6 * s->np, sizeof(double) * 6 * s->np,
+                           cudaMemcpyDeviceToDevice, s->p));
+    j0 = s->d_jhalf;
+  }
+  return fill_log_buffer(s, 0, j0, start);
+}
+
+// Heliocentric planet positions / velocities at the CURRENT step into d_ptmp (q | qd), on stream q.
+// KDK: the Jacobi state of the current record.  DKD: the records sit at the half steps, so the state at
+// the integer step is half a Wisdom-Holman step on from the last record the particles used (d_jprev),
+// or the seed itself at the clock's origin.
+int planets_at_current_step(glisse_sim* s) {
+  const int np = s->np;
+  double* d_out = s->d_ptmp;
+  const double* js = nullptr;
+  if (!s->dkd) {
+    const LogBuffer& B = s->buf[s->cur];
+    const long long off = s->step - B.start;
+    CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+    js = B.jlog + static_cast<size_t>(off) * 6 * np;
+  } else if (s->step == s->origin) {
+    js = s->d_j0;
+  } else {
+    CKS(s, launch_planet_kernel(s->d_sys, np, s->d_jprev, s->d_scratch_log, s->d_scratch_jlog, 1, 0.5 * s->dt,
+                                s->step, s->d_fail + 1, 0, s->q));
+    s->launches += 1;
+    js = s->d_scratch_jlog + 6 * np;
+  }
+  CKS(s, launch_planet_read(s->d_sys, js, d_out, d_out + 3 * np, s->q));
+  s->launches += 1;
   return GLISSE_OK;
 }
 
@@ -463,14 +513,11 @@ int enqueue_sample(glisse_sim* s, bool snapshot, int kind, double* const out[6],
   a.kind = kind;
   a.do_resonance = resonance ? 1 : 0;
   if (resonance) {
-    // planets at the current step: heliocentric q, qd from the Jacobi state of this record
+    // planets at the current step: heliocentric q, qd
     const int np = s->np;
-    const LogBuffer& B = s->buf[s->cur];
-    const long long off = s->step - B.start;
     double* d_out = s->d_ptmp;
-    CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
-    CKS(s, launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q));
-    s->launches += 1;
+    const int sp = planets_at_current_step(s);
+    if (sp != GLISSE_OK) return sp;
     a.planet_q = d_out + 3 * s->res_planet;
     a.planet_qd = d_out + 3 * np + 3 * s->res_planet;
     a.mu_planet = s->gm0 + s->gm_planet_host[s->res_planet];
@@ -544,6 +591,7 @@ void glisse_default_params(glisse_params* p) {
   p->snapshot_chunks = 0;
   p->resonance_chunks = 0;
   p->bin_iterations = 0;
+  p->scheme = GLISSE_SCHEME_KDK;
   p->segment_steps = 128;
 }
 
@@ -586,7 +634,8 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   if (params) prm = *params;
   if (prm.kepler_iters < 0 || !(prm.kepler_tol > 0.0) || prm.chunk_steps < 1 || prm.chunk_steps > 16384 ||
       prm.resync_chunks < 0 || prm.device < 0 || std::isnan(prm.r_min) || std::isnan(prm.r_max) ||
-      prm.snapshot_chunks < 0 || prm.resonance_chunks < 0 || prm.segment_steps < 0)
+      prm.snapshot_chunks < 0 || prm.resonance_chunks < 0 || prm.segment_steps < 0 ||
+      (prm.scheme != GLISSE_SCHEME_KDK && prm.scheme != GLISSE_SCHEME_DKD))
     return GLISSE_EINVAL;
 
   int ndev = 0;
@@ -605,6 +654,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   s->dt = dt;
   s->gm0 = gm_star;
   s->K = prm.chunk_steps;
+  s->dkd = prm.scheme == GLISSE_SCHEME_DKD;
   s->stride = log_stride(n_planets);
   const long long N = n_particles;
   const int np = n_planets;
@@ -674,6 +724,10 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     need(&s->d_fail, 2);
     need(&s->d_sys, 1);
     need(&s->d_j0, static_cast<size_t>(6 * np));
+    need(&s->d_jhalf, static_cast<size_t>(6 * np));
+    need(&s->d_jprev, static_cast<size_t>(6 * np));
+    need(&s->d_scratch_log, static_cast<size_t>(2 * s->stride));
+    need(&s->d_scratch_jlog, static_cast<size_t>(2 * 6 * np));
     need(&s->d_ptmp, static_cast<size_t>(6 * np));
     size_t total = 0;
     for (auto& r : reqs) total += (r.bytes + 255) & ~static_cast<size_t>(255);
@@ -729,7 +783,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   }
   CKF(cudaStreamSynchronize(s->p));  // the caller's planet arrays and `hs` are consumed
   // chunk 0 into buffer 0; the chunk after it is started by the first advance (s->ahead)
-  if (fill_log_buffer(s, 0, s->d_j0, 0) != GLISSE_OK) {
+  if (start_planet_clock(s, 0) != GLISSE_OK) {
     const int st = s->status;
     free_sim(s);
     return st;
@@ -778,6 +832,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   a.mu = gm_star;
   a.inv_mu = 1.0 / gm_star;
   a.inv_mu_dt = dt / gm_star;
+  a.inv_mu_hdt = 0.5 * dt / gm_star;
   a.rmin2 = (prm.r_min > 0.0) ? prm.r_min * prm.r_min : 0.0;
   a.rmax2 = (prm.r_max > 0.0 && std::isfinite(prm.r_max)) ? prm.r_max * prm.r_max
                                                            : std::numeric_limits<double>::infinity();
@@ -827,6 +882,11 @@ int glisse_advance(glisse_sim* s, long long n_steps) {
     const int m = static_cast<int>(std::min<long long>(n_steps, B.len - off));
     const int st = launch_particles(s, B.log + static_cast<size_t>(off) * s->stride, m);
     if (st != GLISSE_OK) return st;
+    if (s->dkd && np > 0) {  // the Jacobi state at (new step) - 1/2: record off + m - 1 of this buffer
+      CKS(s, cudaMemcpyAsync(s->d_jprev, B.jlog + static_cast<size_t>(off + m - 1) * 6 * np, sizeof(double) * 6 * np,
+                             cudaMemcpyDeviceToDevice, s->q));
+      break_chain(s);
+    }
     s->step += m;
     n_steps -= m;
     if (off + m == B.len) {  // this buffer is used up: the planet stream may overwrite it
@@ -927,11 +987,8 @@ int glisse_set_planets(glisse_sim* s, const double* planet_pos, const double* pl
   const long long no_fail = kNoPlanetFailure;
   CKS(s, cudaMemcpyAsync(s->d_fail, &no_fail, sizeof(no_fail), cudaMemcpyHostToDevice, s->p));
   CKS(s, cudaStreamSynchronize(s->p));   // the caller's arrays and `no_fail` are consumed
-  s->origin = s->step;
-  s->cur = 0;
-  s->ahead = false;
   s->planets_stale = false;
-  return fill_log_buffer(s, 0, s->d_j0, s->step);
+  return start_planet_clock(s, s->step);
 }
 
 int glisse_planet_log(glisse_sim* s, long long n_steps, double* log) {
@@ -1085,12 +1142,9 @@ int glisse_read_planets(glisse_sim* s, double* pos, double* vel) {
   const int np = s->np;
   if (np == 0 || (!pos && !vel)) return sync_all(s);
   break_chain(s);
-  const LogBuffer& B = s->buf[s->cur];
-  const long long off = s->step - B.start;
   double* d_out = s->d_ptmp;
-  CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
-  CKS(s, launch_planet_read(s->d_sys, B.jlog + static_cast<size_t>(off) * 6 * np, d_out, d_out + 3 * np, s->q));
-  s->launches += 1;
+  const int sp = planets_at_current_step(s);
+  if (sp != GLISSE_OK) return sp;
   if (pos) CKS(s, cudaMemcpyAsync(pos, d_out, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q));
   if (vel) CKS(s, cudaMemcpyAsync(vel, d_out + 3 * np, sizeof(double) * 3 * np, cudaMemcpyDefault, s->q));
   return sync_all(s);

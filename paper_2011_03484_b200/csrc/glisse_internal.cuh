@@ -49,6 +49,7 @@ struct ParticleArgs {
   int np;
   int iters;
   double hdt, mu, inv_mu, inv_mu_dt, rmin2, rmax2, tol;
+  double inv_mu_hdt;                   // (dt / 2) / mu: the half drifts of the drift-kick-drift scheme
   double gm[kMaxPlanets];
   double rc2[kMaxPlanets];
   // high words of rmin2, rmax2, rc2[]: the hot path's integer superset of the distance tests
@@ -86,7 +87,9 @@ inline int jstate_stride(int np) { return 6 * np; }
 // launchers (each returns the cudaError_t of the launch); *launches += kernels launched
 // chained: launch with programmatic stream serialisation behind the previous particle-kernel launch
 // stats: the instrumented instantiation (glisse_test.h: glisse_solver_stats)
-cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, cudaStream_t s);
+// dkd: the drift-kick-drift instantiation (include/glisse.h: GLISSE_SCHEME_DKD)
+cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd,
+                                   cudaStream_t s);
 cudaError_t configure_particle_kernels();
 int particles_per_group();
 

@@ -110,7 +110,10 @@ __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier
 // NP > 0: compile-time planet count (fully unrolled kick); NP == 0: run-time count a.np.
 // P = particles per thread (kParticlesPerThread): independent instruction streams, see kepler.cuh.
 // STATS: instrumented instantiation (glisse_test.h: glisse_solver_stats); same arithmetic.
-template <int NP, int P, bool STATS>
+// DKD: the drift-kick-drift splitting (GLISSE_SCHEME_DKD): per step a half drift, the force evaluation
+// with the tests at the half-step record, a full kick, a half drift; nsteps records are read, not
+// nsteps + 1, and the state between launches is synchronised at the integer steps as in KDK.
+template <int NP, int P, bool STATS, bool DKD>
 __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel(const __grid_constant__ ParticleArgs a) {
   static_assert(kParticleBlock == 32, "one warp per block: the launch chain hands groups of one warp on");
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -161,7 +164,7 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<double*>(smem_raw) +
                                                static_cast<size_t>(kParticleWarps) * kRingSlots * stage_doubles) +
                    warp * kRingSlots;
-  const int nrec = nsteps + 1;
+  const int nrec = DKD ? nsteps : nsteps + 1;
   const int nstages = (nrec + R - 1) / R;
   if (lane == 0) {
     for (int sl = 0; sl < kRingSlots; ++sl) mbar_init(&bars[sl], 1);
@@ -188,6 +191,23 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
     bool any_alive = true;
     for (int kk = 0; kk < recs; ++kk, ++k) {
       const double* rec = stage + kk * stride;
+      if (DKD) {  // ---- first half drift of step k (D1): flags 3 / 4 freeze the state of t_k
+        double r2h[P];
+        int st_h[P], fi;
+        bool ws;
+#pragma unroll
+        for (int p = 0; p < P; ++p) r2h[p] = fma(x[p], x[p], fma(y[p], y[p], z[p] * z[p]));
+        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, a.inv_mu_hdt, a.iters, a.tol, r2h, x, y, z, vx, vy, vz, st_h, fi, ws);
+        if (STATS) { stat_calls += 1; stat_iters += fi; stat_slow += ws ? 1 : 0; }
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+          if (st_h[p] != 0) {
+            flag[p] = st_h[p];
+            rs[p] = k;
+            alive[p] = false;
+          }
+        }
+      }
       // ---- a3/a4: force evaluation with the tests (O1/O4/O5) at time t_{step0+k} ----------------
       // The tests compare squared distances (O5).  On the hot path they are taken on the HIGH WORDS
       // in the integer pipe, as a superset (d2 < R2 implies hi(d2) <= hi(R2) for non-negative
@@ -249,18 +269,19 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
         }
         if (alive[p]) {
           vx[p] = fma(ax[p], hdt, vx[p]); vy[p] = fma(ay[p], hdt, vy[p]); vz[p] = fma(az[p], hdt, vz[p]);
-          if (k > 0 && k < nsteps) {  // interior: closing half kick of step k-1 and opening of step k
+          // KDK interior: closing half kick of step k-1 and opening of step k; DKD: the one full kick (D3)
+          if (DKD || (k > 0 && k < nsteps)) {
             vx[p] = fma(ax[p], hdt, vx[p]); vy[p] = fma(ay[p], hdt, vy[p]); vz[p] = fma(az[p], hdt, vz[p]);
           }
         }
       }
-      // ---- a5/a6: drift (O2) --------------------------------------------------------------------
-      if (k < nsteps) {
+      // ---- a5/a6: drift (O2; in DKD the second half drift, D4) ---------------------------------------
+      if (DKD || k < nsteps) {
         int st_d[P];
         int fast_iters;
         bool went_slow;
-        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, a.inv_mu_dt, a.iters, a.tol, r2, x, y, z, vx, vy, vz, st_d,
-                             fast_iters, went_slow);
+        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, DKD ? a.inv_mu_hdt : a.inv_mu_dt, a.iters, a.tol, r2, x, y, z, vx,
+                             vy, vz, st_d, fast_iters, went_slow);
         if (STATS) {
           stat_calls += 1;
           stat_iters += fast_iters;
@@ -310,15 +331,16 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
       }
     }
   }
-  // drifts started by this thread's particles: all nsteps for a survivor; for a particle flagged at
-  // record k, k if a force-evaluation test caught it and k + 1 if its drift did (flags 3 and 4)
+  // steps started by this thread's particles: all nsteps for a survivor; for a particle flagged at
+  // record k, KDK: k if a force-evaluation test caught it and k + 1 if its drift did (flags 3 and 4);
+  // DKD: k + 1 whatever caught it (the step had begun with its first half drift)
   unsigned drifts = 0;
 #pragma unroll
   for (int p = 0; p < P; ++p) {
     if (was_alive[p])
       drifts += flag[p] == 0 ? static_cast<unsigned>(nsteps)
                              : static_cast<unsigned>(rs[p]) +
-                                   ((flag[p] == GLISSE_FLAG_NONCONV || flag[p] == GLISSE_FLAG_UNBOUND) ? 1u : 0u);
+                                   ((DKD || flag[p] == GLISSE_FLAG_NONCONV || flag[p] == GLISSE_FLAG_UNBOUND) ? 1u : 0u);
   }
   unsigned tot = __reduce_add_sync(kFullMask, drifts);
   if (lane == 0 && tot) atomicAdd(a.pstep_counter, static_cast<unsigned long long>(tot));
@@ -341,11 +363,12 @@ cudaError_t configure_one() {
   cudaError_t e;
   const int carve = cudaSharedmemCarveoutMaxShared;
   constexpr int P = kParticlesPerThread;
-  if ((e = cudaFuncSetAttribute(particle_kernel<NP, P, false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  return cudaFuncSetAttribute(particle_kernel<NP, P, true>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+  if ((e = cudaFuncSetAttribute(particle_kernel<NP, P, false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
+  if ((e = cudaFuncSetAttribute(particle_kernel<NP, P, false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
+  return cudaFuncSetAttribute(particle_kernel<NP, P, true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
 }
 
-template <int NP, bool STATS>
+template <int NP, bool STATS, bool DKD>
 cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chained, cudaStream_t s) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(static_cast<unsigned>(blocks));
@@ -357,7 +380,7 @@ cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chai
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = chained ? 1 : 0;
-  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, kParticlesPerThread, STATS>, a);
+  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, kParticlesPerThread, STATS, DKD>, a);
 }
 
 }  // namespace
@@ -369,13 +392,21 @@ cudaError_t configure_particle_kernels() {
   return configure_one<8>();
 }
 
-cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, cudaStream_t s) {
+template <int NP>
+cudaError_t launch_np(const ParticleArgs& a, int n_groups, size_t smem, bool chained, bool stats, bool dkd, cudaStream_t s) {
+  if (dkd) return launch_one<NP, false, true>(a, n_groups, smem, chained, s);   // (no instrumented DKD instantiation)
+  return stats ? launch_one<NP, true, false>(a, n_groups, smem, chained, s)
+               : launch_one<NP, false, false>(a, n_groups, smem, chained, s);
+}
+
+cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd,
+                                   cudaStream_t s) {
   if (n_groups < 1) n_groups = 1;
   const size_t smem = particle_smem_bytes(a);
   cudaError_t e;
-  if (a.np == 4) e = stats ? launch_one<4, true>(a, n_groups, smem, chained, s) : launch_one<4, false>(a, n_groups, smem, chained, s);
-  else if (a.np == 8) e = stats ? launch_one<8, true>(a, n_groups, smem, chained, s) : launch_one<8, false>(a, n_groups, smem, chained, s);
-  else e = stats ? launch_one<0, true>(a, n_groups, smem, chained, s) : launch_one<0, false>(a, n_groups, smem, chained, s);
+  if (a.np == 4) e = launch_np<4>(a, n_groups, smem, chained, stats, dkd, s);
+  else if (a.np == 8) e = launch_np<8>(a, n_groups, smem, chained, stats, dkd, s);
+  else e = launch_np<0>(a, n_groups, smem, chained, stats, dkd, s);
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 

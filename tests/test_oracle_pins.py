@@ -467,6 +467,7 @@ def test_dkd_removal_semantics_split_invariance_and_own_log(oracle_mod):
     # particle 1: far outside r_max -> caught at the first force evaluation (after half a drift): flag 2,
     # step 0, frozen at t_{1/2}: position moved, the velocity of a pure Kepler half drift (no kick)
     pos[:, 1] = [900.0, 500.0, 0.0]
+    vel[:, 1] = np.sqrt(w.gm_star / np.hypot(900.0, 500.0)) * np.array([-500.0, 900.0, 0.0]) / np.hypot(900.0, 500.0)
     S = oracle_mod.OracleSim(w.gm_star, w.gm_planet, q, w.planet_vel, rc, pos, vel, w.dt, r_min=1.0, r_max=1000.0,
                              scheme="dkd")
     S.advance(3)
