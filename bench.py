@@ -420,11 +420,14 @@ def run_ablations(binding, torch, device, flush):
     n = c2.n_particles
     ring = (torch.empty((4, 6, n), dtype=torch.float64).pin_memory(), torch.empty((4, n), dtype=torch.int32).pin_memory(),
             torch.empty((4, n), dtype=torch.int64).pin_memory(), torch.empty(4, dtype=torch.int64).pin_memory())
-    for label, kw in (("off", {}), ("snapshot_and_resonance_every_chunk", dict(snapshot_chunks=1, resonance_chunks=1))):
+    for label, kw in (("off", {}), ("snapshot_every_chunk", dict(snapshot_chunks=1)),
+                      ("resonance_every_chunk", dict(resonance_chunks=1)),
+                      ("snapshot_and_resonance_every_chunk", dict(snapshot_chunks=1, resonance_chunks=1))):
         stream = torch.cuda.Stream(device=device)
         sim = binding.GlisseSim.from_workload(c2, chunk_steps=CHUNK, device=device.index, stream=stream.cuda_stream, **kw)
-        if kw:
+        if "snapshot_chunks" in kw:
             sim.snapshot_ring("elements", 4, *(t.numpy() for t in ring))
+        if "resonance_chunks" in kw:
             sim.resonance_begin(3, 3, 1, np.deg2rad(10.0))
         with torch.cuda.stream(stream):
             sim.advance(3 * CHUNK)
@@ -440,6 +443,28 @@ def run_ablations(binding, torch, device, flush):
         out.setdefault("periodic_output_c2_16_chunks", {})[label] = {
             "value": (sim.particle_steps() - ps0) / (ms * 1e-3), "ms_per_chunk": ms / 16}
         sim.close()
+    # particle-count sweep (BASELINE.json configs[4]: "Also sweep particle count over 2^10 to 2^22"): config
+    # 5's planet-crossing distribution, compaction every chunk, wall clock per chunk after 2 warm-up chunks
+    out["particle_count_sweep_config5"] = {}
+    for lg in range(10, 23):
+        n = 1 << lg
+        wn = inputs.config(5, n)
+        sim = binding.GlisseSim.from_workload(wn, chunk_steps=CHUNK, resync_chunks=1, device=device.index)
+        sim.advance(2 * CHUNK)
+        sim.sync()
+        sim.particle_kernel_time()
+        ps0 = sim.particle_steps()
+        chunks = 8 if lg < 21 else 4
+        t0 = time.perf_counter()
+        sim.advance(chunks * CHUNK)
+        sim.sync()
+        dt = time.perf_counter() - t0
+        kms, kruns = sim.particle_kernel_time()
+        out["particle_count_sweep_config5"][str(n)] = {
+            "value": (sim.particle_steps() - ps0) / dt, "ms_per_chunk": 1e3 * dt / chunks,
+            "kernel_ms_per_chunk": kms / max(kruns, 1), "active_fraction_end": sim.active_count() / n}
+        sim.close()
+        del wn
     # external planet history streamed from pinned host memory, 10^5 steps at N = 131,072, vs the
     # internal planet clock over the same steps
     steps = 100_000

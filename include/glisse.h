@@ -99,6 +99,13 @@ typedef struct {
                            group would be launched first"); 0 (default): particle-ID order
                            (PAPER.md:127).  Performance only: results are bit-identical.       */
   int    scheme;           /* GLISSE_SCHEME_KDK (default) or GLISSE_SCHEME_DKD                          */
+  int    guess_order;      /* starting point of the Kepler solve ("a judicious initial guess",
+                           PAPER.md:123): 1 = dE = dM a/r for every body; 3 = the series reversion
+                           of Kepler's equation to third order for bodies with e dE^2 above ~6e-5
+                           (eccentric orbits at small a: saves them a solver iteration, costs
+                           quiet workloads 4 %); 0 (default) = chosen once, at create, from the
+                           initial conditions: 3 if more than 5 % of the particles would take it.
+                           The root is the same; results differ at roundoff between 1 and 3      */
   int    segment_steps;    /* a chunk is issued as back-to-back launches of this many steps whose
                            warps hand particles on through per-group completion flags, so the
                            tail of one launch is filled by the next; default 128,

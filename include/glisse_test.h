@@ -34,7 +34,7 @@ int glisse_fp64_peak_probe(int device, void* stream, double millis, double* flop
  * Evaluate one device primitive of the CUDA path on an array, on device 0.
  * in/out are HOST or device arrays.  which = 0 rsqrt (in[n] -> out[n]), 1 reciprocal, 2 reciprocal
  * to 2^-39 (Newton updates only), 3 sin x - x and cos x - 1 (in[n] -> out[2n], interleaved),
- * 4 one Kepler drift (step a5) per body: in[10n] = {mu, dt, kepler_iters, kepler_tol, x, y, z, vx,
+ * 4 (5: with the third-order starting point, guess_order 3) one Kepler drift (step a5) per body: in[10n] = {mu, dt, kepler_iters, kepler_tol, x, y, z, vx,
  * vy, vz}, out[7n] = {flag, x, y, z, vx, vy, vz}; mu, kepler_iters and kepler_tol are taken from
  * body 0 for all bodies (constants of a run, warp-uniform in the kernel); dt is per body.  Synchronises.
  */

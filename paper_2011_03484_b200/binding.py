@@ -40,7 +40,7 @@ class GlisseParams(ctypes.Structure):
     _fields_ = [("r_min", c_double), ("r_max", c_double), ("kepler_iters", c_int), ("kepler_tol", c_double),
                 ("chunk_steps", c_int), ("resync_chunks", c_int), ("device", c_int), ("stream", c_void_p),
                 ("snapshot_chunks", c_int), ("resonance_chunks", c_int), ("bin_iterations", c_int),
-                ("scheme", c_int), ("segment_steps", c_int)]
+                ("scheme", c_int), ("guess_order", c_int), ("segment_steps", c_int)]
 
 
 class GlisseError(RuntimeError):
@@ -169,7 +169,7 @@ class GlisseSim:
     def __init__(self, gm_star, gm_planet, planet_pos, planet_vel, planet_rcrit, pos, vel, dt, *, r_min=0.0,
                  r_max=float("inf"), kepler_iters=5, kepler_tol=1e-14, chunk_steps=1024, resync_chunks=1,
                  device=0, stream=None, snapshot_chunks=0, resonance_chunks=0, bin_iterations=0,
-                 segment_steps=None, scheme="kdk"):
+                 segment_steps=None, scheme="kdk", guess_order=0):
         L = lib()
         gm_planet = np.ascontiguousarray(gm_planet, dtype=np.float64).reshape(-1)
         self.n_planets = int(gm_planet.shape[0])
@@ -191,6 +191,7 @@ class GlisseSim:
         prm.snapshot_chunks, prm.resonance_chunks = int(snapshot_chunks), int(resonance_chunks)
         prm.bin_iterations = int(bin_iterations)
         prm.scheme = {"kdk": 0, "dkd": 1}[scheme]
+        prm.guess_order = int(guess_order)
         if segment_steps is not None:
             prm.segment_steps = int(segment_steps)
         h = c_void_p()
@@ -379,7 +380,8 @@ def fp64_peak_probe(device=0, millis=200.0, stream=None) -> float:
     return out.value
 
 
-_PRIM = {"rsqrt": (0, 1, 1), "rcp": (1, 1, 1), "rcp1": (2, 1, 1), "sincosm": (3, 1, 2), "kepler_drift": (4, 10, 7)}
+_PRIM = {"rsqrt": (0, 1, 1), "rcp": (1, 1, 1), "rcp1": (2, 1, 1), "sincosm": (3, 1, 2), "kepler_drift": (4, 10, 7),
+         "kepler_drift_refined": (5, 10, 7)}
 
 
 def test_primitive(name, x):

@@ -142,6 +142,7 @@ struct glisse_sim {
   int chain_len = 0;              // launches in the open chain (0 = the next launch starts one)
   int chain_groups = 0;
   bool stats_on = false;
+  bool refine = false;            // particle-kernel instantiation with the third-order Kepler starting point
   unsigned long long* d_stats = nullptr;  // [3]
 
   // snapshot staging (glisse_snapshot): a copy in original order that stream r ships to the caller
@@ -159,8 +160,8 @@ struct glisse_sim {
   long long* ring_rstep = nullptr;
   long long* ring_step = nullptr;
   long long ring_emitted = 0;
-  long long* h_ring_steps = nullptr;   // pinned [kRingStepWords]: sources of the slot_step copies
-  int ring_step_next = 0;
+  long long* d_ring_steps = nullptr;   // device [kRingStepWords]: sources of the slot_step copies (written by the
+  int ring_step_next = 0;              // sample pass, so the copy on stream r is an ordinary async D2H / D2D)
 
   // resonant-argument record (glisse_resonance_*), original order
   LibrationRecord lib{};
@@ -224,7 +225,6 @@ void free_sim(glisse_sim* s) {
   if (s->snap_ready) cudaEventDestroy(s->snap_ready);
   if (s->snap_done) cudaEventDestroy(s->snap_done);
   if (s->r) cudaStreamDestroy(s->r);
-  if (s->h_ring_steps) cudaFreeHost(s->h_ring_steps);
   for (int b = 0; b < 2; ++b) {
     if (s->buf[b].ready) cudaEventDestroy(s->buf[b].ready);
     if (s->buf[b].consumed) cudaEventDestroy(s->buf[b].consumed);
@@ -323,7 +323,7 @@ int launch_particles(glisse_sim* s, const double* log, int nsteps) {
     a.log = log + static_cast<size_t>(off) * s->stride;
     a.step0 = s->step + off;
     a.nsteps = m;
-    CKS(s, launch_particle_kernel(a, groups, !first, s->stats_on, s->dkd, s->q));
+    CKS(s, launch_particle_kernel(a, groups, !first, s->stats_on, s->dkd, s->refine, s->q));
     s->launches += 1;
     s->chain_len += 1;
   }
@@ -350,16 +350,19 @@ int run_compaction(glisse_sim* s) {
   c.fin_flag = s->fin_flag; c.fin_rstep = s->fin_rstep;
   c.n_in = s->d_nslots + w;
   c.n_out = s->d_nslots + o;
+  c.n_out_host = s->h_nslots;
   c.block_counts = s->d_block_counts;
   c.bin = s->d_bin;
   c.bins = s->prm.bin_iterations ? kCompactBins : 1;
   c.mu = s->gm0;
-  c.dt = s->dt;
+  c.dt = s->dkd ? 0.5 * s->dt : s->dt;
+  c.refine = s->refine ? 1 : 0;
   CKS(s, launch_compaction(c, s->nslots_upper, s->q, &s->launches));
   s->w = o;
-  // survivor count to the host without blocking (stream order keeps an older copy into the same pinned
-  // word ahead of this one); the next launches use it once it has arrived
-  CKS(s, cudaMemcpyAsync(s->h_nslots, s->d_nslots + o, sizeof(int), cudaMemcpyDeviceToHost, s->q));
+  // survivor count to the host without blocking: the scan kernel stores it into the mapped pinned word
+  // itself (no copy in this stream: a device-to-host copy here queues behind a snapshot's copies on
+  // the same copy engine and held the next chunk back by 0.2 ms); the next launches use it once the
+  // event says it has arrived
   CKS(s, cudaEventRecord(s->nslots_ready, s->q));
   s->nslots_pending = true;
   return GLISSE_OK;
@@ -512,6 +515,12 @@ int enqueue_sample(glisse_sim* s, bool snapshot, int kind, double* const out[6],
   a.do_snapshot = snapshot ? 1 : 0;
   a.kind = kind;
   a.do_resonance = resonance ? 1 : 0;
+  long long* step_word = nullptr;
+  if (snapshot && slot_step) {  // the step count travels with the staging copy (no host-to-host copy: that
+    step_word = s->d_ring_steps + (s->ring_step_next++ % kRingStepWords);   // one would stall the enqueueing thread)
+    a.step = s->step;
+    a.step_out = step_word;
+  }
   if (resonance) {
     // planets at the current step: heliocentric q, qd
     const int np = s->np;
@@ -538,11 +547,8 @@ int enqueue_sample(glisse_sim* s, bool snapshot, int kind, double* const out[6],
   if (flag) CKS(s, cudaMemcpyAsync(flag, s->snap_flag, N * sizeof(int), cudaMemcpyDefault, s->r));
   if (removal_step)
     CKS(s, cudaMemcpyAsync(removal_step, s->snap_rstep, N * sizeof(long long), cudaMemcpyDefault, s->r));
-  if (slot_step) {  // after the data, same stream: a host polling a pinned slot_step sees complete slots
-    long long* src = s->h_ring_steps + (s->ring_step_next++ % kRingStepWords);
-    *src = s->step;
-    CKS(s, cudaMemcpyAsync(slot_step, src, sizeof(long long), cudaMemcpyDefault, s->r));
-  }
+  if (step_word)  // after the data, same stream: a host polling a pinned slot_step sees complete slots
+    CKS(s, cudaMemcpyAsync(slot_step, step_word, sizeof(long long), cudaMemcpyDefault, s->r));
   CKS(s, cudaEventRecord(s->snap_done, s->r));
   s->snap_in_flight = true;
   return GLISSE_OK;
@@ -592,6 +598,7 @@ void glisse_default_params(glisse_params* p) {
   p->resonance_chunks = 0;
   p->bin_iterations = 0;
   p->scheme = GLISSE_SCHEME_KDK;
+  p->guess_order = 0;
   p->segment_steps = 128;
 }
 
@@ -635,7 +642,8 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   if (prm.kepler_iters < 0 || !(prm.kepler_tol > 0.0) || prm.chunk_steps < 1 || prm.chunk_steps > 16384 ||
       prm.resync_chunks < 0 || prm.device < 0 || std::isnan(prm.r_min) || std::isnan(prm.r_max) ||
       prm.snapshot_chunks < 0 || prm.resonance_chunks < 0 || prm.segment_steps < 0 ||
-      (prm.scheme != GLISSE_SCHEME_KDK && prm.scheme != GLISSE_SCHEME_DKD))
+      (prm.scheme != GLISSE_SCHEME_KDK && prm.scheme != GLISSE_SCHEME_DKD) ||
+      (prm.guess_order != 0 && prm.guess_order != 1 && prm.guess_order != 3))
     return GLISSE_EINVAL;
 
   int ndev = 0;
@@ -717,10 +725,11 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     need(&s->d_nslots, 2);
     need(&s->d_block_counts, static_cast<size_t>(kCompactBins) * ((N + 255) / 256 + 1) + 1);
     need(&s->d_bin, N);
-    need(&s->d_counters, 2);
+    need(&s->d_counters, 3);
     need(&s->d_ticket, 2);
     need(&s->d_error, 1);
     need(&s->d_stats, 3);
+    need(&s->d_ring_steps, kRingStepWords);
     need(&s->d_fail, 2);
     need(&s->d_sys, 1);
     need(&s->d_j0, static_cast<size_t>(6 * np));
@@ -796,7 +805,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     CKF(cudaMemcpyAsync(s->work[0][k], pos[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
     CKF(cudaMemcpyAsync(s->work[0][3 + k], vel[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
   }
-  CKF(cudaMemsetAsync(s->d_counters, 0, 2 * sizeof(unsigned long long), s->q));
+  CKF(cudaMemsetAsync(s->d_counters, 0, 3 * sizeof(unsigned long long), s->q));
   CKF(cudaMemsetAsync(s->d_error, 0, sizeof(int), s->q));
   CKF(cudaMemsetAsync(s->d_stats, 0, 3 * sizeof(unsigned long long), s->q));
   {
@@ -804,13 +813,20 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
       CKF(launch_count_nonfinite(s->work[0][k], N, s->d_counters + 1, s->q));
       s->launches += 1;
     }
-    unsigned long long bad = 0;
-    CKF(cudaMemcpyAsync(&bad, s->d_counters + 1, sizeof(bad), cudaMemcpyDeviceToHost, s->q));
+    // guess_order = 0: the Kepler starting point is chosen here, once, from the initial conditions
+    // (deterministic: the same inputs always give the same instantiation, whatever K, R or the schedule)
+    if (prm.guess_order == 0) {
+      CKF(launch_count_refine(s->work[0], N, gm_star, (s->dkd ? 0.5 : 1.0) * dt, s->d_counters + 2, s->q));
+      s->launches += 1;
+    }
+    unsigned long long cnt[2] = {0, 0};   // non-finite inputs, bodies wanting the third-order starting point
+    CKF(cudaMemcpyAsync(cnt, s->d_counters + 1, sizeof(cnt), cudaMemcpyDeviceToHost, s->q));
     CKF(cudaStreamSynchronize(s->q));
-    if (bad) {
+    if (cnt[0]) {
       free_sim(s);
       return GLISSE_EINVAL;
     }
+    s->refine = prm.guess_order == 3 || (prm.guess_order == 0 && 20 * cnt[1] > static_cast<unsigned long long>(N));
   }
   CKF(launch_init_ids(s->id[0], s->flag[0], s->rstep[0], s->fin_flag, s->fin_rstep, static_cast<int>(N), s->q));
   s->launches += 1;
@@ -1066,8 +1082,6 @@ int glisse_snapshot_ring(glisse_sim* s, int kind, int n_slots, double* data, int
   if (s->status != GLISSE_OK) return s->status;
   CKS(s, cudaSetDevice(s->device));
   if (s->r) CKS(s, cudaStreamSynchronize(s->r));   // copies into the ring being replaced are done
-  if (n_slots > 0 && !s->h_ring_steps)
-    CKS(s, cudaMallocHost(reinterpret_cast<void**>(&s->h_ring_steps), kRingStepWords * sizeof(long long)));
   s->ring_kind = kind;
   s->ring_slots = n_slots;
   s->ring_data = n_slots ? data : nullptr;
@@ -1239,13 +1253,13 @@ int glisse_fp64_peak_probe(int device, void* stream, double millis, double* flop
 }
 
 int glisse_test_primitive(int which, long long n, const double* in, double* out) {
-  if (which < 0 || which > 4 || n < 1 || !in || !out) return GLISSE_EINVAL;
+  if (which < 0 || which > 5 || n < 1 || !in || !out) return GLISSE_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
     (void)cudaGetLastError();
     return GLISSE_ECUDA;
   }
-  const size_t in_per = (which == 4) ? 10 : 1, out_per = (which == 4) ? 7 : (which == 3 ? 2 : 1);
+  const size_t in_per = (which >= 4) ? 10 : 1, out_per = (which >= 4) ? 7 : (which == 3 ? 2 : 1);
   double *d_in = nullptr, *d_out = nullptr;
   CK(dmalloc(&d_in, static_cast<size_t>(n) * in_per));
   cudaError_t e = dmalloc(&d_out, static_cast<size_t>(n) * out_per);

@@ -16,6 +16,7 @@
 // within a bin.  Every survivor is moved by the partition anyway, so the ordering is free; a particle's
 // arithmetic never depends on its warp-mates, so results are bit-identical to the unbinned run.
 #include "glisse_internal.cuh"
+#include "kepler.cuh"
 
 namespace glisse {
 namespace {
@@ -27,9 +28,11 @@ constexpr unsigned kFull = 0xffffffffu;
 // is accepted at every phase of the orbit, 1 = some phases need more, 2 = some phase leaves the fast
 // solver (e >= 0.8, |x0| > pi/4, unbound).  The fast solver starts from x0 = dM/q, q = 1 - e cos E0,
 // and accepts once the Newton update delta = f(x0)/f'(x0) is below an eccentricity-tiered bound;
-// here delta is evaluated at 12 phases E0 of the orbit with a safety factor of 2.  A heuristic: it
-// decides only which particles share a warp.
-__device__ int hardness_bin(double mu, double dt, double x, double y, double z, double vx, double vy, double vz) {
+// here delta is evaluated at 12 phases E0 of the orbit with a safety factor of 2, from the starting
+// point the run's instantiation would use (first order, or the third-order reversion where the body
+// qualifies for it: kepler.cuh).  A heuristic: it decides only which particles share a warp.
+__device__ int hardness_bin(double mu, double dt, bool refine, double x, double y, double z, double vx, double vy,
+                            double vz) {
   const double r = sqrt(x * x + y * y + z * z);
   const double v2 = vx * vx + vy * vy + vz * vz;
   const double u = x * vx + y * vy + z * vz;
@@ -48,10 +51,15 @@ __device__ int hardness_bin(double mu, double dt, double x, double y, double z, 
   for (int k = 0; k < 12; ++k) {
     double s0, c0;
     sincos(kTwoPi * k / 12.0, &s0, &c0);
-    const double q = 1.0 - e * c0, es = e * s0, x0 = dM / q;
+    const double q = 1.0 - e * c0, es = e * s0;
+    double x0 = dM / q;
+    if (refine && wants_refined_guess(hi_word(e2), hi_abs(x0))) {
+      const double b2 = 0.5 * es / q, b3 = e * c0 / (6.0 * q);
+      x0 = x0 + x0 * x0 * (-b2 + (2.0 * b2 * b2 - b3) * x0);
+    }
     double sx, cx;
     sincos(x0, &sx, &cx);
-    const double f = e * c0 * (x0 - sx) + es * (1.0 - cx);
+    const double f = (x0 - dM) - e * c0 * sx + es * (1.0 - cx);   // Kepler's equation at x0
     const double f1 = 1.0 - e * c0 * cx + es * sx;
     worst = fmax(worst, fabs(f / f1));
   }
@@ -68,7 +76,8 @@ __global__ void __launch_bounds__(kBlock) count_block_actives(const CompactArgs 
   __syncthreads();
   int b = 0;
   if (act && a.bins > 1)
-    b = hardness_bin(a.mu, a.dt, a.src[0][i], a.src[1][i], a.src[2][i], a.src[3][i], a.src[4][i], a.src[5][i]);
+    b = hardness_bin(a.mu, a.dt, a.refine != 0, a.src[0][i], a.src[1][i], a.src[2][i], a.src[3][i], a.src[4][i],
+                     a.src[5][i]);
   if (i < n) a.bin[i] = static_cast<unsigned char>(b);
   for (int k = 0; k < a.bins; ++k) {
     const unsigned m = __ballot_sync(kFull, act && b == k);
@@ -80,8 +89,11 @@ __global__ void __launch_bounds__(kBlock) count_block_actives(const CompactArgs 
 }
 
 // exclusive scan of block_counts[0..nb) in place (one block), total -> *n_out
+// n_out_host (may be null): mapped pinned word that also receives the total — the host learns the
+// survivor count without a device-to-host copy in the particle stream (a copy there would queue behind
+// a snapshot's multi-megabyte copies on the same copy engine and hold the next chunk back)
 __global__ void __launch_bounds__(1024) scan_block_counts(int* __restrict__ block_counts, int nb,
-                                                           int* __restrict__ n_out) {
+                                                           int* __restrict__ n_out, volatile int* n_out_host) {
   __shared__ int warp_sums[32];
   __shared__ int carry_s;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -115,7 +127,13 @@ __global__ void __launch_bounds__(1024) scan_block_counts(int* __restrict__ bloc
     if (threadIdx.x == 0) carry_s = carry + warp_sums[31];
     __syncthreads();
   }
-  if (threadIdx.x == 0) *n_out = carry_s;
+  if (threadIdx.x == 0) {
+    *n_out = carry_s;
+    if (n_out_host) {
+      *n_out_host = carry_s;
+      __threadfence_system();
+    }
+  }
 }
 
 __global__ void __launch_bounds__(kBlock) scatter_partition(const CompactArgs a, int nb) {
@@ -201,7 +219,7 @@ cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStrea
   if (n_slots_upper < 1) n_slots_upper = 1;
   const int nb = (n_slots_upper + kBlock - 1) / kBlock;
   count_block_actives<<<nb, kBlock, 0, s>>>(a, nb);
-  scan_block_counts<<<1, 1024, 0, s>>>(a.block_counts, a.bins * nb, a.n_out);
+  scan_block_counts<<<1, 1024, 0, s>>>(a.block_counts, a.bins * nb, a.n_out, a.n_out_host);
   scatter_partition<<<nb, kBlock, 0, s>>>(a, nb);
   if (launches) *launches += 3;
   return cudaGetLastError();

@@ -88,8 +88,12 @@ inline int jstate_stride(int np) { return 6 * np; }
 // chained: launch with programmatic stream serialisation behind the previous particle-kernel launch
 // stats: the instrumented instantiation (glisse_test.h: glisse_solver_stats)
 // dkd: the drift-kick-drift instantiation (include/glisse.h: GLISSE_SCHEME_DKD)
-cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd,
+// refine: the instantiation with the third-order starting point of the Kepler solve (guess_order 3)
+cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd, bool refine,
                                    cudaStream_t s);
+// *out += number of the n bodies that would take the third-order starting point at this instant
+cudaError_t launch_count_refine(const double* const st[6], long long n, double mu, double dt, unsigned long long* out,
+                                cudaStream_t s);
 cudaError_t configure_particle_kernels();
 int particles_per_group();
 
@@ -119,12 +123,14 @@ struct CompactArgs {
   int* fin_flag; long long* fin_rstep;
   const int* n_in;         // prefix length of src
   int* n_out;              // number of survivors = prefix length of dst
+  int* n_out_host;         // mapped pinned word that receives the same count (or null)
   int* block_counts;       // scratch [kCompactBins * ceil(n_upper/256) + 1]
   // iteration-count binning (include/glisse.h bin_iterations): bins > 1 orders the
   // survivors by bin (hardest first), particle order within a bin
   unsigned char* bin;      // scratch [n_upper]: bin of every slot (written by the count pass)
   int bins;                // 1 = plain stable partition, kCompactBins = binned
   double mu, dt;           // for the hardness key
+  int refine;              // the run uses the third-order Kepler starting point (kepler.cuh)
 };
 constexpr int kCompactBins = 3;
 cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStream_t s, long long* launches);
@@ -167,6 +173,8 @@ struct SampleArgs {
   double mu;
   // snapshot part (do_snapshot)
   int do_snapshot, kind;
+  long long step;           // written to *step_out (if not null) by the pass: the snapshot's step count
+  long long* step_out;
   double* out[6];
   int* out_flag; long long* out_rstep;
   // resonance part (do_resonance)

@@ -236,6 +236,24 @@ static __device__ __noinline__ ExactSolve kepler_solve_exact(bool live, double e
 // Kepler's equation has one root (f1 >= 1 − e > 0), so both solvers return the same x to roundoff.
 // Thresholds and range tests are taken on the high words (integer pipe): the FP64 pipe is the
 // roofline.
+// Refined starting point.  x0 = dM/q is the first term of the reversion of
+//     q x + (es/2) x^2 + (ec/6) x^3 + ... = dM,
+// and the Newton update it leaves is ~ es x0^2 / (2 q): too large for one quartic step once e x0^2
+// reaches ~1e-4 (planet-crossing orbits at small a, config 5; Jupiter itself at dt = 180 d).  Those
+// bodies start instead from the reversion carried to third order,
+//     x = y - b2 y^2 + (2 b2^2 - b3) y^3,   y = dM/q,  b2 = es/(2q),  b3 = ec/(6q)      (9 FP64 operations)
+// whose error is O(y^4) (~1e-5 at y = 0.3), so that ONE quartic step is accepted where two were needed.
+// Which bodies take it is decided per body from its own numbers (so a body's arithmetic still never
+// depends on its warp-mates), in the integer pipe: log2(e^2)/4 + log2|y| = log2(sqrt(e) |y|) read off the
+// high words (piecewise-linear in the mantissa, good to 0.15 in log2) against log2(sqrt(6e-5)) = -7.0.
+// It is a compile-time variant of the drift (template REFINE): in the kernels of quiet workloads even a
+// never-taken branch around these nine operations cost 4 % (measured), so they do not contain it; the
+// instantiation is chosen per simulation (include/glisse.h: guess_order), never per launch.
+constexpr int kRefineLevel = static_cast<int>((1023.0 * 1.25 - 7.0) * 1048576.0);
+__device__ __forceinline__ bool wants_refined_guess(int e2_hi, int x_hi_abs) {
+  return (e2_hi >> 2) + x_hi_abs > kRefineLevel;
+}
+
 constexpr int kFastMinIters = 5;   // the paper's count; below it the definition may not converge
 constexpr int kFastMaxIters = 4;
 // The fast solver does not evaluate the residual: what it accepts has a residual below 2e-17 plus the
@@ -264,7 +282,7 @@ constexpr int kHiThr3 = 0x3ef4f8b5;     // 2e-5   = 0x3ef4f8b588e368f1
 // and inv_mu_dt = dt/mu are constants of the run.  st[p] returns 0, GLISSE_FLAG_NONCONV (3) or
 // GLISSE_FLAG_UNBOUND (4); on a non-zero status, or for !live bodies, the state is untouched.
 // A body's arithmetic never depends on the other bodies of its lane or warp.
-template <int P>
+template <int P, bool REFINE = false>
 __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], double mu, double inv_mu,
                                                   double inv_mu_dt, int iters, double tol, const double (&r2)[P],
                                                   double (&x)[P], double (&y)[P], double (&z)[P], double (&vx)[P],
@@ -302,13 +320,20 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
     const int e2h = hi_word(e2[p]);
     thr[p] = e2h < kHiE2_010 ? kHiThr0 : (e2h < kHiE2_030 ? kHiThr1 : (e2h < kHiE2_050 ? kHiThr2 : kHiThr3));
     open[p] = live[p] && fast_on && e2h < kHiE2_080 && is_small_angle(xk[p]);
+    if (REFINE && open[p] && wants_refined_guess(e2h, hi_abs(xk[p]))) {
+      const double yy = xk[p];
+      const double hq = 0.5 * invq[p];
+      const double b2 = es[p] * hq;
+      const double b3 = (ec[p] * hq) * (1.0 / 3.0);
+      const double c3 = fma(2.0 * b2, b2, -b3);
+      xk[p] = fma(yy * yy, fma(c3, yy, -b2), yy);
+    }
     slow[p] = live[p] && !open[p];
     any_open = any_open || open[p];
     sm[p] = 0.0;
     cm1[p] = 0.0;
     nonconv[p] = 0;
   }
-
   fast_iters = 0;   // warp-uniform: iterations of the fast solver this warp executes (solver statistics)
   for (int it = 0; it < kFastMaxIters && __any_sync(kFullMask, any_open); ++it) {
     any_open = false;
@@ -390,15 +415,17 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
 }
 
 // One body per lane (the planet-history kernel and the primitive test hook).
-__device__ __forceinline__ int kepler_drift_warp(bool live, double mu, double inv_mu, double inv_mu_dt, int iters,
-                                                 double tol, double r2, double& x, double& y, double& z,
-                                                 double& vx, double& vy, double& vz) {
+template <bool REFINE>
+__device__ __forceinline__ int kepler_drift_one(bool live, double mu, double inv_mu, double inv_mu_dt, int iters,
+                                                double tol, double r2, double& x, double& y, double& z,
+                                                double& vx, double& vy, double& vz) {
   const bool l1[1] = {live};
   const double r21[1] = {r2};
   double x1[1] = {x}, y1[1] = {y}, z1[1] = {z}, vx1[1] = {vx}, vy1[1] = {vy}, vz1[1] = {vz};
   int st[1], fast_iters;
   bool went_slow;
-  kepler_drift_warp<1>(l1, mu, inv_mu, inv_mu_dt, iters, tol, r21, x1, y1, z1, vx1, vy1, vz1, st, fast_iters, went_slow);
+  kepler_drift_warp<1, REFINE>(l1, mu, inv_mu, inv_mu_dt, iters, tol, r21, x1, y1, z1, vx1, vy1, vz1, st, fast_iters,
+                               went_slow);
   x = x1[0]; y = y1[0]; z = z1[0]; vx = vx1[0]; vy = vy1[0]; vz = vz1[0];
   return st[0];
 }

@@ -113,7 +113,8 @@ __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier
 // DKD: the drift-kick-drift splitting (GLISSE_SCHEME_DKD): per step a half drift, the force evaluation
 // with the tests at the half-step record, a full kick, a half drift; nsteps records are read, not
 // nsteps + 1, and the state between launches is synchronised at the integer steps as in KDK.
-template <int NP, int P, bool STATS, bool DKD>
+// REFINE: third-order starting point of the Kepler solve (kepler.cuh; include/glisse.h: guess_order).
+template <int NP, int P, bool STATS, bool DKD, bool REFINE>
 __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel(const __grid_constant__ ParticleArgs a) {
   static_assert(kParticleBlock == 32, "one warp per block: the launch chain hands groups of one warp on");
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -197,7 +198,8 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
         bool ws;
 #pragma unroll
         for (int p = 0; p < P; ++p) r2h[p] = fma(x[p], x[p], fma(y[p], y[p], z[p] * z[p]));
-        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, a.inv_mu_hdt, a.iters, a.tol, r2h, x, y, z, vx, vy, vz, st_h, fi, ws);
+        kepler_drift_warp<P, REFINE>(alive, a.mu, a.inv_mu, a.inv_mu_hdt, a.iters, a.tol, r2h, x, y, z, vx, vy, vz, st_h,
+                                     fi, ws);
         if (STATS) { stat_calls += 1; stat_iters += fi; stat_slow += ws ? 1 : 0; }
 #pragma unroll
         for (int p = 0; p < P; ++p) {
@@ -280,8 +282,8 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
         int st_d[P];
         int fast_iters;
         bool went_slow;
-        kepler_drift_warp<P>(alive, a.mu, a.inv_mu, DKD ? a.inv_mu_hdt : a.inv_mu_dt, a.iters, a.tol, r2, x, y, z, vx,
-                             vy, vz, st_d, fast_iters, went_slow);
+        kepler_drift_warp<P, REFINE>(alive, a.mu, a.inv_mu, DKD ? a.inv_mu_hdt : a.inv_mu_dt, a.iters, a.tol, r2, x, y,
+                                     z, vx, vy, vz, st_d, fast_iters, went_slow);
         if (STATS) {
           stat_calls += 1;
           stat_iters += fast_iters;
@@ -358,17 +360,50 @@ size_t particle_smem_bytes(const ParticleArgs& a) {
          static_cast<size_t>(kParticleWarps) * kRingSlots * 8;
 }
 
+// Bodies that would take the third-order starting point at this instant (guess_order = 0 chooses the
+// instantiation from their share at create).  Plain arithmetic: off the hot path.
+__global__ void __launch_bounds__(256) count_refine_kernel(const double* x, const double* y, const double* z,
+                                                            const double* vx, const double* vy, const double* vz,
+                                                            long long n, double mu, double dt,
+                                                            unsigned long long* out) {
+  const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  bool want = false;
+  if (i < n) {
+    const double r0 = sqrt(x[i] * x[i] + y[i] * y[i] + z[i] * z[i]);
+    const double v2 = vx[i] * vx[i] + vy[i] * vy[i] + vz[i] * vz[i];
+    const double u = x[i] * vx[i] + y[i] * vy[i] + z[i] * vz[i];
+    const double alpha = 2.0 * mu / r0 - v2;
+    if (alpha > 0.0) {
+      const double q = r0 * alpha / mu;
+      const double ec = 1.0 - q, es = u * sqrt(alpha) / mu;
+      const double e2 = ec * ec + es * es;
+      const double ndt = alpha * sqrt(alpha) * dt / mu;
+      const double xk = fma(-rint(ndt * kInvTwoPi), kTwoPi, ndt) / q;
+      want = hi_word(e2) < kHiE2_080 && is_small_angle(xk) && wants_refined_guess(hi_word(e2), hi_abs(xk));
+    }
+  }
+  const int c = __syncthreads_count(want);
+  if (threadIdx.x == 0 && c) atomicAdd(out, static_cast<unsigned long long>(c));
+}
+
+template <int NP, bool STATS, bool DKD, bool REFINE>
+cudaError_t configure_kernel() {
+  return cudaFuncSetAttribute(particle_kernel<NP, kParticlesPerThread, STATS, DKD, REFINE>,
+                              cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+}
+
 template <int NP>
 cudaError_t configure_one() {
   cudaError_t e;
-  const int carve = cudaSharedmemCarveoutMaxShared;
-  constexpr int P = kParticlesPerThread;
-  if ((e = cudaFuncSetAttribute(particle_kernel<NP, P, false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  if ((e = cudaFuncSetAttribute(particle_kernel<NP, P, false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, carve))) return e;
-  return cudaFuncSetAttribute(particle_kernel<NP, P, true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+  if ((e = configure_kernel<NP, false, false, false>())) return e;
+  if ((e = configure_kernel<NP, false, false, true>())) return e;
+  if ((e = configure_kernel<NP, false, true, false>())) return e;
+  if ((e = configure_kernel<NP, false, true, true>())) return e;
+  if ((e = configure_kernel<NP, true, false, false>())) return e;
+  return configure_kernel<NP, true, false, true>();
 }
 
-template <int NP, bool STATS, bool DKD>
+template <int NP, bool STATS, bool DKD, bool REFINE>
 cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chained, cudaStream_t s) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(static_cast<unsigned>(blocks));
@@ -380,7 +415,14 @@ cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chai
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = chained ? 1 : 0;
-  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, kParticlesPerThread, STATS, DKD>, a);
+  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, kParticlesPerThread, STATS, DKD, REFINE>, a);
+}
+
+template <int NP, bool REFINE>
+cudaError_t launch_np(const ParticleArgs& a, int n_groups, size_t smem, bool chained, bool stats, bool dkd, cudaStream_t s) {
+  if (dkd) return launch_one<NP, false, true, REFINE>(a, n_groups, smem, chained, s);   // (no instrumented DKD instantiation)
+  return stats ? launch_one<NP, true, false, REFINE>(a, n_groups, smem, chained, s)
+               : launch_one<NP, false, false, REFINE>(a, n_groups, smem, chained, s);
 }
 
 }  // namespace
@@ -392,22 +434,21 @@ cudaError_t configure_particle_kernels() {
   return configure_one<8>();
 }
 
-template <int NP>
-cudaError_t launch_np(const ParticleArgs& a, int n_groups, size_t smem, bool chained, bool stats, bool dkd, cudaStream_t s) {
-  if (dkd) return launch_one<NP, false, true>(a, n_groups, smem, chained, s);   // (no instrumented DKD instantiation)
-  return stats ? launch_one<NP, true, false>(a, n_groups, smem, chained, s)
-               : launch_one<NP, false, false>(a, n_groups, smem, chained, s);
-}
-
-cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd,
+cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd, bool refine,
                                    cudaStream_t s) {
   if (n_groups < 1) n_groups = 1;
   const size_t smem = particle_smem_bytes(a);
   cudaError_t e;
-  if (a.np == 4) e = launch_np<4>(a, n_groups, smem, chained, stats, dkd, s);
-  else if (a.np == 8) e = launch_np<8>(a, n_groups, smem, chained, stats, dkd, s);
-  else e = launch_np<0>(a, n_groups, smem, chained, stats, dkd, s);
+  if (a.np == 4) e = refine ? launch_np<4, true>(a, n_groups, smem, chained, stats, dkd, s) : launch_np<4, false>(a, n_groups, smem, chained, stats, dkd, s);
+  else if (a.np == 8) e = refine ? launch_np<8, true>(a, n_groups, smem, chained, stats, dkd, s) : launch_np<8, false>(a, n_groups, smem, chained, stats, dkd, s);
+  else e = refine ? launch_np<0, true>(a, n_groups, smem, chained, stats, dkd, s) : launch_np<0, false>(a, n_groups, smem, chained, stats, dkd, s);
   return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+cudaError_t launch_count_refine(const double* const st[6], long long n, double mu, double dt, unsigned long long* out,
+                                cudaStream_t s) {
+  count_refine_kernel<<<static_cast<int>((n + 255) / 256), 256, 0, s>>>(st[0], st[1], st[2], st[3], st[4], st[5], n, mu, dt, out);
+  return cudaGetLastError();
 }
 
 // particles per launch group (one warp's worth): the host sizes grids and completion lists with it

@@ -186,8 +186,9 @@ __global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* 
   for (int s = 0; s < nsteps; ++s) {
     vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
     const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
-    const int st = kepler_drift_warp(true, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2,
-                                     rx, ry, rz, vx, vy, vz);
+    // third-order starting point (kepler.cuh): Jupiter at dt = 180 d needs one quartic step instead of two
+    const int st = kepler_drift_one<true>(true, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2,
+                                          rx, ry, rz, vx, vy, vz);
     const unsigned failed = __ballot_sync(kFullMask, st != 0 && L.live);
     if (failed && bad < 0) bad = s;
     jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);

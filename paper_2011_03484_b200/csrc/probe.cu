@@ -54,7 +54,8 @@ __global__ void primitive_kernel(int which, long long n, const double* __restric
       if (live) { out[2 * i] = sm; out[2 * i + 1] = cm; }
       break;
     }
-    case 4: {  // kepler drift: in = [mu, dt, iters, tol, x,y,z,vx,vy,vz] per body; out = [flag, x..vz]
+    case 4:    // kepler drift: in = [mu, dt, iters, tol, x,y,z,vx,vy,vz] per body; out = [flag, x..vz]
+    case 5: {  // the same with the third-order starting point (guess_order 3)
       // mu, kepler_iters and kepler_tol are constants of a run and must be warp-uniform (the solver's
       // loop exits on warp votes): taken from body 0; dt may differ per body
       const double* p = in + 10 * ii;
@@ -63,7 +64,8 @@ __global__ void primitive_kernel(int which, long long n, const double* __restric
       const double tol = in[3];
       double x = p[4], y = p[5], z = p[6], vx = p[7], vy = p[8], vz = p[9];
       const double r2 = fma(x, x, fma(y, y, z * z));
-      const int st = kepler_drift_warp(live, mu, 1.0 / mu, dt / mu, iters, tol, r2, x, y, z, vx, vy, vz);
+      const int st = which == 5 ? kepler_drift_one<true>(live, mu, 1.0 / mu, dt / mu, iters, tol, r2, x, y, z, vx, vy, vz)
+                                : kepler_drift_one<false>(live, mu, 1.0 / mu, dt / mu, iters, tol, r2, x, y, z, vx, vy, vz);
       if (live) {
         double* o = out + 7 * i;
         o[0] = st; o[1] = x; o[2] = y; o[3] = z; o[4] = vx; o[5] = vy; o[6] = vz;

@@ -93,6 +93,7 @@ __device__ __forceinline__ Osculating osculating_elements(double mu, double X, d
 __global__ void __launch_bounds__(256) sample_kernel(SampleArgs a) {
   const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (i >= a.n) return;
+  if (i == 0 && a.step_out != nullptr) *a.step_out = a.step;
   const double X = a.fin[0][i], Y = a.fin[1][i], Z = a.fin[2][i];
   const double U = a.fin[3][i], V = a.fin[4][i], W = a.fin[5][i];
   const int fl = a.fin_flag[i];
