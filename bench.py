@@ -61,12 +61,15 @@ FLOPS_PER_PLANET = 25.0
 # EXECUTED flops per particle-step of the particle kernel and its DRAM traffic per launch, per workload,
 # from that workload's own ncu capture (2 DFMA + DMUL + DADD thread-instructions / thread-steps;
 # dram__bytes_read.sum + dram__bytes_write.sum): (flops, bytes per launch, profile it was read from).
+#   flops per thread-step = (2 DFMA + DMUL + DADD of a launch) / (grid x 32 threads x 128 steps of the launch):
+#   1m_x4 3.657e10 / (31670 x 32 x 128), c2 4.575e9 / (3961 x ...), c3 9.455e9 / (8192 x ...),
+#   c4 5.064e10 / (32492 x ...), c5 1.486e11 / (116553 x ...)
 NCU = {
-    "1m_x4": (281.0, 5.6e7, "profiles/r02_particle_kernel_1m_x4.md"),
-    "c2": (281.0, 6.9e6, "profiles/r02_particle_kernel_c2.md"),
-    "c3": (281.0, 1.4e7, "profiles/r02_particle_kernel_c3.md"),
-    "c4": (377.0, 5.7e7, "profiles/r02_particle_kernel_c4.md"),
-    "c5": (340.0, 2.2e8, "profiles/r02_particle_kernel_c5.md"),
+    "1m_x4": (281.9, 5.41e7, "profiles/r02_particle_kernel_1m_x4.md"),
+    "c2": (282.0, 6.65e6, "profiles/r02_particle_kernel_c2.md"),
+    "c3": (281.8, 1.37e7, "profiles/r02_particle_kernel_c3.md"),
+    "c4": (380.5, 5.60e7, "profiles/r02_particle_kernel_c4.md"),
+    "c5": (311.3, 3.20e8, "profiles/r02_particle_kernel_c5.md"),
 }
 # FP64 peak: ncu reports sm__sass_thread_inst_executed_op_dfma_pred_on.sum.peak_sustained = 64 per SM
 # per cycle; x 148 SMs x 2 flops x 1.965 GHz (clocks.max.sm of B200_PROFILING.md)
@@ -588,6 +591,10 @@ def rank_main(argv):
                                 "roofline": {k: rf[k] for k in ("achieved", "frac", "executed_frac", "executed_source",
                                                                 "flops_per_particle_step",
                                                                 "executed_flops_per_particle_step") if k in rf}}
+                if name == "c2":   # the paper-sized workload end to end as well (one wave: the costliest case)
+                    ec = time_e2e(binding, torch, wo, 5, 3, device)
+                    others[name]["e2e"] = {"value": ec["psteps"] / ec["seconds"], "unit": UNIT,
+                                           "h2d_bytes_per_step": ec["h2d"], "d2h_bytes_per_step": ec["d2h"]}
                 del wo
             line["workloads"] = others
             rate, secs, ps = oracle_rate(w, 16384, 3000)
