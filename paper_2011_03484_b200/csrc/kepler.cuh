@@ -335,7 +335,9 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
     nonconv[p] = 0;
   }
   fast_iters = 0;   // warp-uniform: iterations of the fast solver this warp executes (solver statistics)
-  for (int it = 0; it < kFastMaxIters && __any_sync(kFullMask, any_open); ++it) {
+  // (the first step is taken without asking whether any lane is open: a warp with none — every lane on
+  // the slow path or dead — is rare, and the vote and branch cost every other warp 0.9 %)
+  for (int it = 0; it < kFastMaxIters && ((it == 0 && fast_on) || __any_sync(kFullMask, any_open)); ++it) {
     any_open = false;
     fast_iters = it + 1;
 #pragma unroll
@@ -383,7 +385,7 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
   if (went_slow) {
 #pragma unroll
     for (int p = 0; p < P; ++p) {
-      if (__any_sync(kFullMask, slow[p])) {
+      if (P == 1 || __any_sync(kFullMask, slow[p])) {   // (P == 1: any_slow above is this very vote)
         const ExactSolve o = kepler_solve_exact(slow[p], ec[p], es[p], q[p], dM[p], invq[p], e2[p], iters, tol);
         if (slow[p]) {
           xk[p] = o.x; sm[p] = o.sm; cm1[p] = o.cm1; nonconv[p] = o.nonconv;
