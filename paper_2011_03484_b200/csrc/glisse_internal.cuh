@@ -20,7 +20,7 @@ constexpr int kParticlesPerThread = GL_PPT;  // particles per thread (independen
 constexpr int kParticleWarps = kParticleBlock / 32;
 constexpr int kRingSlots = 2;        // planet-log stages resident in shared memory per WARP
 #ifndef GL_MIN_BLOCKS
-#define GL_MIN_BLOCKS 22
+#define GL_MIN_BLOCKS 20
 #endif
 
 // Doubles per planet-log record (include/glisse.h: glisse_log_stride).

@@ -416,6 +416,101 @@ __device__ __forceinline__ void kepler_drift_warp(const bool (&live_in)[P], doub
   }
 }
 
+// ---- the drift in three pieces, for the particle kernel --------------------------------------------
+// The same arithmetic as kepler_drift_warp (bit for bit, for every body it advances), cut where the
+// particle kernel wants its warp votes: the kernel runs drift_begin, ONE fast-solver step and
+// drift_finish for all 32 lanes without any per-lane predicate, and everything a body can need beyond
+// that (further fast steps, the definition's solver, the unbound / non-convergence flags) in a block it
+// enters on one vote.  A lane that holds no particle of its own runs a copy of a live lane's body there
+// (particles.cu), so no lane needs to be kept finite by selects: an unbound body's NaNs stay in its
+// own lane and send the warp to that block.
+struct DriftVars {
+  double rinv, sqa, rsa, q, ec, es, dM, a, invq, e2;
+};
+
+template <bool REFINE>
+__device__ __forceinline__ void drift_begin(double mu, double two_mu, double inv_mu, double inv_mu_dt, double r2,
+                                            double x, double y, double z, double vx, double vy, double vz,
+                                            DriftVars& k, double& xk, bool& unbound) {
+  const double v2 = fma(vx, vx, fma(vy, vy, vz * vz));
+  const double u = fma(x, vx, fma(y, vy, z * vz));
+  k.rinv = rsqrt_f64(r2);
+  const double r0 = r2 * k.rinv;
+  const double al = fma(two_mu, k.rinv, -v2);  // mu / a
+  unbound = !(hi_word(al) > 0);                 // alpha <= 0 (or below 2^-1042: no such orbit), or NaN
+  k.rsa = rsqrt_f64(al);
+  k.sqa = al * k.rsa;                    // sqrt(alpha) = n a
+  const double inva = k.rsa * k.rsa;     // 1 / alpha
+  k.q = r0 * (al * inv_mu);              // r0 / a = 1 − ec
+  k.ec = 1.0 - k.q;
+  k.es = u * (k.sqa * inv_mu);
+  const double ndt = (al * k.sqa) * inv_mu_dt;                  // n dt
+  k.dM = fma(-rint(ndt * kInvTwoPi), kTwoPi, ndt);              // reading S9
+  k.a = mu * inva;
+  k.invq = k.a * k.rinv;  // a / r0
+  k.e2 = fma(k.ec, k.ec, k.es * k.es);
+  xk = k.dM * k.invq;
+  if (REFINE) {
+    const int e2h = hi_word(k.e2);
+    if (e2h < kHiE2_080 && is_small_angle(xk) && wants_refined_guess(e2h, hi_abs(xk))) {
+      const double yy = xk;
+      const double hq = 0.5 * k.invq;
+      const double b2 = k.es * hq;
+      const double b3 = (k.ec * hq) * (1.0 / 3.0);
+      const double c3 = fma(2.0 * b2, b2, -b3);
+      xk = fma(yy * yy, fma(c3, yy, -b2), yy);
+    }
+  }
+}
+
+// acceptance bound of the fast solver for this eccentricity (high word of the bound on |delta|)
+__device__ __forceinline__ int fast_threshold(int e2h) {
+  return e2h < kHiE2_010 ? kHiThr0 : (e2h < kHiE2_030 ? kHiThr1 : (e2h < kHiE2_050 ? kHiThr2 : kHiThr3));
+}
+
+// one step of the fast solver from xk: the new x, sin x − x and cos x − 1 there, and the Newton update dl
+__device__ __forceinline__ void fast_step(const DriftVars& k, double xk, double& xn, double& smn, double& cmn,
+                                          double& dl) {
+  double smk, cmk;
+  sincosm_small(xk, smk, cmk);
+  const double s = xk + smk;
+  const double c = 1.0 + cmk;
+  const double f = fma(-k.es, cmk, fma(-k.ec, s, xk - k.dM));
+  const double f1 = fma(k.es, s, fma(-k.ec, cmk, k.q));
+  const double f2 = fma(k.ec, s, k.es * c);
+  const double inv = rcp_f64_1(f1);
+  dl = f * inv;                     // Newton update
+  const double h = dl * inv;
+  const double u2 = f2 * h;         // 2 a2 delta
+  const double f3 = 1.0 - f1;
+  const double v6 = (f3 * h) * dl;  // 6 a3 delta^2
+  const double w = fma(u2, fma(0.5, u2, 0.5), v6 * (-1.0 / 6.0));
+  const double d = fma(dl, w, dl);
+  const double hd = 0.5 * d;
+  const double h2 = hd * d;                  // d^2 / 2
+  const double d3 = h2 * (d * (1.0 / 3.0));  // d^3 / 6
+  smn = fma(c, d3, fma(-h2, s, fma(-d, cmk, smk)));
+  cmn = fma(-s, d3, fma(-h2, c, fma(d, s, cmk)));
+  xn = xk - d;
+}
+
+// Gauss f, g (PAPER.md:94 step 4) from the solved x: r += (f−1) r + g v, v += fdot r + (gdot−1) v
+__device__ __forceinline__ void drift_finish(const DriftVars& k, double xk, double sm, double cm1, double& x,
+                                             double& y, double& z, double& vx, double& vy, double& vz) {
+  const double s = xk + sm;
+  const double pr = fma(k.es, s, fma(-k.ec, cm1, k.q));  // r(t)/a
+  const double invp = rcp_f64(pr);
+  const double fm1 = cm1 * k.invq;
+  const double g = (k.dM + sm) * (k.a * k.rsa);  // (dM − x + sin x) / n
+  const double fd = -(s * invp) * (k.sqa * k.rinv);
+  const double gm1 = cm1 * invp;
+  const double tx = fma(g, vx, x), ty = fma(g, vy, y), tz = fma(g, vz, z);
+  vx = fma(fd, x, fma(gm1, vx, vx));
+  vy = fma(fd, y, fma(gm1, vy, vy));
+  vz = fma(fd, z, fma(gm1, vz, vz));
+  x = fma(fm1, x, tx); y = fma(fm1, y, ty); z = fma(fm1, z, tz);
+}
+
 // One body per lane (the planet-history kernel and the primitive test hook).
 template <bool REFINE>
 __device__ __forceinline__ int kepler_drift_one(bool live, double mu, double inv_mu, double inv_mu_dt, int iters,

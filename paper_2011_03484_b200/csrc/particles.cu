@@ -107,19 +107,254 @@ __device__ __forceinline__ void publish_group(const ParticleArgs& a, int lane, i
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
+// ---- shared-memory reads of the staged log by 32-bit shared address (the record pointer is one
+// uniform register that advances by the stride; ordered after the mbarrier wait, both being volatile)
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
+
+// The per-lane state of the step loop.  A lane whose own particle is gone (removed in an earlier launch,
+// past the end of the array, or flagged during this launch) is `dead`: it goes on with a COPY of a live
+// lane's body (its donor), so that it computes exactly what the donor computes — never a NaN, a slow
+// path or a test hit of its own — and the step loop needs no per-lane predicate at all.  Everything a
+// removal needs (flag, removal record, the frozen state written to memory, a new donor for the lane and
+// for every lane that was copying it) happens in blocks entered on one warp vote.
+struct Lane {
+  double x, y, z, vx, vy, vz;
+  int flag;     // of the lane's own particle (0 = still integrating); -1 = the lane never had one
+  int rs;       // record index (within this launch) at which it was flagged
+  bool dead;    // the registers hold a donor's body
+};
+
+__device__ __forceinline__ double shfl_f64(double v, int src) { return __shfl_sync(kFullMask, v, src); }
+
+// the frozen state of a particle flagged during this launch goes to memory at once (O5 / S12)
+__device__ __forceinline__ void freeze(const ParticleArgs& a, long long i, const Lane& L, int flag, int k) {
+  a.st[0][i] = L.x; a.st[1][i] = L.y; a.st[2][i] = L.z;
+  a.st[3][i] = L.vx; a.st[4][i] = L.vy; a.st[5][i] = L.vz;
+  a.flag[i] = flag;
+  a.rstep[i] = a.step0 + k;
+}
+
+// ---- the removal blocks: out of line, entered by the whole warp on one vote, so that neither their
+// registers nor their branches cost the step loop anything.  The lane's numbers travel through a small
+// record in local memory.  Both return true when no lane of the warp has a particle left.
+struct KickRecord {
+  Lane L;
+  double ax, ay, az, r2;
+};
+
+// Exact distance tests of O5 at the record at `rec` (the hot path saw a high-word superset pass in some
+// lane), lowest planet index first (S11); a particle that is hit is frozen WITHOUT this evaluation's kick.
+static __device__ __noinline__ bool removal_at_kick(const ParticleArgs& a, int np, uint32_t rec, int k, long long i,
+                                                    KickRecord* io) {
+  Lane L = io->L;
+  const double r2 = io->r2;
+  int hit = 0;
+  for (int jj = 0; jj < np; ++jj) {
+    const int j = np - 1 - jj;
+    const double qx = lds_f64(rec + 24 * j), qy = lds_f64(rec + 24 * j + 8), qz = lds_f64(rec + 24 * j + 16);
+    const double dx = L.x - qx, dy = L.y - qy, dz = L.z - qz;
+    const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    hit = (d2 < a.rc2[j]) ? (GLISSE_FLAG_PLANET0 + j) : hit;
+  }
+  hit = (r2 > a.rmax2) ? GLISSE_FLAG_RMAX : hit;
+  hit = (r2 < a.rmin2) ? GLISSE_FLAG_RMIN : hit;
+  if (!__any_sync(kFullMask, hit != 0)) return false;
+  if (hit != 0 && !L.dead) {
+    freeze(a, i, L, hit, k);
+    io->L.flag = hit;
+    io->L.rs = k;
+  }
+  const bool dead = L.dead || hit != 0;
+  io->L.dead = dead;
+  const unsigned alive = __ballot_sync(kFullMask, !dead);
+  if (alive == 0u) return true;
+  // every lane that hit — the particle's own lane and the lanes that were copying it — takes a new donor
+  const int donor = __ffs(alive) - 1;
+  const double tx = shfl_f64(L.x, donor), ty = shfl_f64(L.y, donor), tz = shfl_f64(L.z, donor);
+  const double tvx = shfl_f64(L.vx, donor), tvy = shfl_f64(L.vy, donor), tvz = shfl_f64(L.vz, donor);
+  const double tax = shfl_f64(io->ax, donor), tay = shfl_f64(io->ay, donor), taz = shfl_f64(io->az, donor);
+  const double tr2 = shfl_f64(r2, donor);
+  if (hit != 0) {
+    io->L.x = tx; io->L.y = ty; io->L.z = tz; io->L.vx = tvx; io->L.vy = tvy; io->L.vz = tvz;
+    io->ax = tax; io->ay = tay; io->az = taz; io->r2 = tr2;
+  }
+  return false;
+}
+
+// Force evaluation with the tests (O1/O4/O5) at the record at shared address `rec`, then the kick(s):
+// v += acc hdt, and again with hdt2 (hdt for an interior record of KDK — the closing half kick of one step
+// and the opening one of the next — and for DKD's full kick; 0 at record 0).  Returns true when no lane of
+// the warp has a particle left.  r2 = |r|^2 is handed on to the drift.
+template <int NP>
+__device__ __forceinline__ bool kick_with_tests(const ParticleArgs& a, int np, uint32_t rec, int k, long long i,
+                                                double hdt, double hdt2, Lane& L, double& r2) {
+  // The tests compare squared distances (O5).  On the hot path they are taken on the HIGH WORDS in the
+  // integer pipe, as a superset (d2 < R2 implies hi(d2) <= hi(R2) for non-negative doubles); the exact
+  // fp64 comparisons run only in a warp where some lane passes the superset.
+  r2 = fma(L.x, L.x, fma(L.y, L.y, L.z * L.z));
+  double ax = lds_f64(rec + 24 * np), ay = lds_f64(rec + 24 * np + 8), az = lds_f64(rec + 24 * np + 16);  // h0
+  const int r2h = __double2hiint(r2);
+  bool maybe = (r2h >= a.rmax2_hi) || (r2h <= a.rmin2_hi);
+#pragma unroll
+  for (int j = 0; j < np; ++j) {
+    const double qx = lds_f64(rec + 24 * j), qy = lds_f64(rec + 24 * j + 8), qz = lds_f64(rec + 24 * j + 16);
+    const double dx = L.x - qx, dy = L.y - qy, dz = L.z - qz;
+    const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    maybe = maybe || (__double2hiint(d2) <= a.rc2_hi[j]);
+    const double w = gm_over_r3(a.gm[j], d2);
+    ax = fma(-w, dx, ax);
+    ay = fma(-w, dy, ay);
+    az = fma(-w, dz, az);
+  }
+  if (__any_sync(kFullMask, maybe)) {  // rare
+    KickRecord io;
+    io.L = L; io.ax = ax; io.ay = ay; io.az = az; io.r2 = r2;
+    const bool finished = removal_at_kick(a, np, rec, k, i, &io);
+    L = io.L; ax = io.ax; ay = io.ay; az = io.az; r2 = io.r2;
+    if (__any_sync(kFullMask, finished)) return true;   // (the vote tells the compiler that the exit is warp-uniform)
+  }
+  L.vx = fma(ax, hdt, L.vx); L.vy = fma(ay, hdt, L.vy); L.vz = fma(az, hdt, L.vz);
+  L.vx = fma(ax, hdt2, L.vx); L.vy = fma(ay, hdt2, L.vy); L.vz = fma(az, hdt2, L.vz);
+  return false;
+}
+
+struct DriftRecord {
+  Lane L;
+  DriftVars v;
+  double xk, sm, cm1;     // the solver's state: x, sin x − x, cos x − 1
+  int thr;                // acceptance bound of the fast solver for this body
+  bool unbound, open, slow;
+  unsigned iters, went_slow;   // statistics: fast-solver steps taken here, slow path entered
+};
+
+// Everything a drift can need beyond its first fast-solver step: further steps for the bodies that are
+// still `open` (exactly as kepler_drift_warp takes them, starting with step number it0), the definition's
+// solver for the `slow` ones, flags 3 / 4 with the state on entry to the drift frozen, new donors.
+static __device__ __noinline__ bool solve_and_flag(const ParticleArgs& a, int it0, int k, long long i, DriftRecord* io) {
+  const DriftVars v = io->v;
+  double xk = io->xk, sm = io->sm, cm1 = io->cm1;
+  const int thr = io->thr;
+  const bool unbound = io->unbound;
+  bool open = io->open, slow = io->slow;
+  unsigned iters = 0;
+  for (int it = it0; it < kFastMaxIters && __any_sync(kFullMask, open); ++it) {
+    double xn, smn, cmn, dl;
+    fast_step(v, xk, xn, smn, cmn, dl);
+    ++iters;
+    if (open) {
+      sm = smn; cm1 = cmn; xk = xn;
+      const bool done = hi_abs(dl) < thr;
+      const bool lost = !done && !is_small_angle(xk);
+      open = !done && !lost;
+      slow = slow || lost;
+    }
+  }
+  slow = slow || open;   // no convergence in kFastMaxIters steps
+  int nonconv = 0;
+  io->went_slow = 0;
+  if (__any_sync(kFullMask, slow)) {
+    io->went_slow = 1;
+    const ExactSolve o = kepler_solve_exact(slow, v.ec, v.es, v.q, v.dM, v.invq, v.e2, a.iters, a.tol);
+    if (slow) { xk = o.x; sm = o.sm; cm1 = o.cm1; nonconv = o.nonconv; }
+  }
+  io->iters = iters;
+  io->xk = xk; io->sm = sm; io->cm1 = cm1;
+  const bool bad = unbound || nonconv != 0;
+  if (!__any_sync(kFullMask, bad)) return false;
+  const Lane L = io->L;
+  if (bad && !L.dead) {
+    const int why = unbound ? GLISSE_FLAG_UNBOUND : GLISSE_FLAG_NONCONV;
+    freeze(a, i, L, why, k);
+    io->L.flag = why;
+    io->L.rs = k;
+  }
+  const bool dead = L.dead || bad;
+  io->L.dead = dead;
+  const unsigned alive = __ballot_sync(kFullMask, !dead);
+  if (alive == 0u) return true;
+  const int donor = __ffs(alive) - 1;
+  // (one value at a time: the shuffle, then the select)
+#define GL_TAKE(field) { const double t_ = shfl_f64(field, donor); if (bad) io->field = t_; }
+  GL_TAKE(L.x) GL_TAKE(L.y) GL_TAKE(L.z) GL_TAKE(L.vx) GL_TAKE(L.vy) GL_TAKE(L.vz)
+  GL_TAKE(v.rinv) GL_TAKE(v.sqa) GL_TAKE(v.rsa) GL_TAKE(v.q) GL_TAKE(v.ec) GL_TAKE(v.es)
+  GL_TAKE(v.dM) GL_TAKE(v.a) GL_TAKE(v.invq)
+#undef GL_TAKE
+  { const double t_ = shfl_f64(xk, donor); if (bad) io->xk = t_; }
+  { const double t_ = shfl_f64(sm, donor); if (bad) io->sm = t_; }
+  { const double t_ = shfl_f64(cm1, donor); if (bad) io->cm1 = t_; }
+  return false;
+}
+
+// Kepler drift of the warp's 32 bodies (O2): begin, one fast-solver step, finish, with one vote in between
+// that sends the warp to solve_and_flag.  lim_e2 / lim_x are the high words below which a body may use the
+// fast solver (both 0 when the run's kepler_iters / kepler_tol keep it out).  In the REFINE instantiation
+// (planet-crossing populations) a second fast-solver step is common, so it is taken in line before the
+// call.  Returns true when no lane of the warp has a particle left.
+template <bool REFINE, bool STATS>
+__device__ __forceinline__ bool drift_with_flags(const ParticleArgs& a, double two_mu, double inv_mu_dt, int lim_e2,
+                                                 int lim_x, double r2, int k, long long i, Lane& L,
+                                                 unsigned (&stat)[3]) {
+  DriftVars v;
+  double xk, xn, sm, cm1, dl;
+  bool unbound;
+  drift_begin<REFINE>(a.mu, two_mu, a.inv_mu, inv_mu_dt, r2, L.x, L.y, L.z, L.vx, L.vy, L.vz, v, xk, unbound);
+  const int e2h = hi_word(v.e2);
+  const int thr = fast_threshold(e2h);
+  const bool notopen = unbound || !(e2h < lim_e2) || !(hi_abs(xk) < lim_x);
+  fast_step(v, xk, xn, sm, cm1, dl);
+  const bool done = hi_abs(dl) < thr;
+  if (STATS) { stat[0] += 1; stat[1] += lim_x != 0 ? 1 : 0; }
+  if (__any_sync(kFullMask, notopen || !done)) {
+    bool open = !notopen && !done && is_small_angle(xn);
+    bool slow = !unbound && (notopen || (!done && !open));
+    int it0 = 1;
+    bool more = true;
+    if (REFINE) {   // the second step in line
+      if (__any_sync(kFullMask, open)) {
+        double xn2, smn, cmn, dl2;
+        fast_step(v, xn, xn2, smn, cmn, dl2);
+        if (STATS) stat[1] += 1;
+        if (open) {
+          sm = smn; cm1 = cmn; xn = xn2;
+          const bool done2 = hi_abs(dl2) < thr;
+          const bool lost = !done2 && !is_small_angle(xn);
+          open = !done2 && !lost;
+          slow = slow || lost;
+        }
+      }
+      it0 = 2;
+      more = __any_sync(kFullMask, open || slow || unbound);
+    }
+    if (more) {
+      DriftRecord io;
+      io.L = L; io.v = v; io.xk = xn; io.sm = sm; io.cm1 = cm1; io.thr = thr;
+      io.unbound = unbound; io.open = open; io.slow = slow;
+      const bool finished = solve_and_flag(a, it0, k, i, &io);
+      L = io.L; v = io.v; xn = io.xk; sm = io.sm; cm1 = io.cm1;
+      if (STATS) { stat[1] += io.iters; stat[2] += io.went_slow; }
+      if (__any_sync(kFullMask, finished)) return true;
+    }
+  }
+  drift_finish(v, xn, sm, cm1, L.x, L.y, L.z, L.vx, L.vy, L.vz);
+  return false;
+}
+
 // NP > 0: compile-time planet count (fully unrolled kick); NP == 0: run-time count a.np.
-// P = particles per thread (kParticlesPerThread): independent instruction streams, see kepler.cuh.
 // STATS: instrumented instantiation (glisse_test.h: glisse_solver_stats); same arithmetic.
 // DKD: the drift-kick-drift splitting (GLISSE_SCHEME_DKD): per step a half drift, the force evaluation
 // with the tests at the half-step record, a full kick, a half drift; nsteps records are read, not
 // nsteps + 1, and the state between launches is synchronised at the integer steps as in KDK.
 // REFINE: third-order starting point of the Kepler solve (kepler.cuh; include/glisse.h: guess_order).
-template <int NP, int P, bool STATS, bool DKD, bool REFINE>
+template <int NP, bool STATS, bool DKD, bool REFINE>
 __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel(const __grid_constant__ ParticleArgs a) {
   static_assert(kParticleBlock == 32, "one warp per block: the launch chain hands groups of one warp on");
+  static_assert(kParticlesPerThread == 1, "one particle per thread");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31;
-  constexpr int warp = 0;
   const int np = NP > 0 ? NP : a.np;
   const int stride = a.stride;
   const int nsteps = a.nsteps;
@@ -130,41 +365,37 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   pdl_launch_dependents();
   if (grp < 0) return;   // gave up waiting (a.error is set): touch nothing
   const int n = *a.n_slots;
-  // particle p of this thread: consecutive threads hold consecutive particles (coalesced), the P
-  // particles of a thread lie kParticleBlock apart
-  const long long i0 = static_cast<long long>(grp) * (kParticleBlock * P) + threadIdx.x;
+  const long long i = static_cast<long long>(grp) * kParticleBlock + threadIdx.x;  // consecutive lanes, consecutive particles
 
   // ---- a2: load ------------------------------------------------------------------------------
-  double x[P], y[P], z[P], vx[P], vy[P], vz[P];
-  int flag[P];
-  bool was_alive[P], alive[P];
-  int rs[P];   // record index (within this launch) at which the particle was flagged, −1 = not yet
-  bool any_alive_t = false;
-#pragma unroll
-  for (int p = 0; p < P; ++p) {
-    const long long i = i0 + p * kParticleBlock;
-    x[p] = 1.0; y[p] = 0.0; z[p] = 0.0; vx[p] = 0.0; vy[p] = 0.0; vz[p] = 0.0;
-    flag[p] = -1;
-    if (i < n) {  // through L2: the group's previous owner may have run on another SM a launch ago
-      flag[p] = __ldcg(a.flag + i);
-      x[p] = __ldcg(a.st[0] + i); y[p] = __ldcg(a.st[1] + i); z[p] = __ldcg(a.st[2] + i);
-      vx[p] = __ldcg(a.st[3] + i); vy[p] = __ldcg(a.st[4] + i); vz[p] = __ldcg(a.st[5] + i);
-    }
-    was_alive[p] = (flag[p] == 0);
-    alive[p] = was_alive[p];
-    any_alive_t = any_alive_t || alive[p];
-    rs[p] = -1;
+  Lane L;
+  L.x = 1.0; L.y = 0.0; L.z = 0.0; L.vx = 0.0; L.vy = 0.0; L.vz = 0.0;
+  L.flag = -1;
+  L.rs = -1;
+  if (i < n) {  // through L2: the group's previous owner may have run on another SM a launch ago
+    L.flag = __ldcg(a.flag + i);
+    L.x = __ldcg(a.st[0] + i); L.y = __ldcg(a.st[1] + i); L.z = __ldcg(a.st[2] + i);
+    L.vx = __ldcg(a.st[3] + i); L.vy = __ldcg(a.st[4] + i); L.vz = __ldcg(a.st[5] + i);
   }
-  if (!__any_sync(kFullMask, any_alive_t)) {  // nothing to do in this warp: leave before any copy
-    publish_group(a, lane, grp);
-    return;
+  const bool own = (L.flag == 0);   // the lane has a particle to integrate
+  L.dead = !own;
+  {
+    if (!__any_sync(kFullMask, own)) {  // nothing to do in this warp: leave before any copy
+      publish_group(a, lane, grp);
+      return;
+    }
+    const unsigned alive = __ballot_sync(kFullMask, own);
+    const int donor = __ffs(alive) - 1;
+    const double tx = shfl_f64(L.x, donor), ty = shfl_f64(L.y, donor), tz = shfl_f64(L.z, donor);
+    const double tvx = shfl_f64(L.vx, donor), tvy = shfl_f64(L.vy, donor), tvz = shfl_f64(L.vz, donor);
+    if (!own) { L.x = tx; L.y = ty; L.z = tz; L.vx = tvx; L.vy = tvy; L.vz = tvz; }
   }
 
   // ---- warp-private ring ------------------------------------------------------------------------
-  double* ring = reinterpret_cast<double*>(smem_raw) + static_cast<size_t>(warp) * kRingSlots * stage_doubles;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<double*>(smem_raw) +
-                                               static_cast<size_t>(kParticleWarps) * kRingSlots * stage_doubles) +
-                   warp * kRingSlots;
+  double* ring = reinterpret_cast<double*>(smem_raw);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(ring + static_cast<size_t>(kRingSlots) * stage_doubles);
+  const uint32_t ring_addr = smem_u32(ring);
+  const uint32_t rec_bytes = static_cast<uint32_t>(stride) * 8u;
   const int nrec = DKD ? nsteps : nsteps + 1;
   const int nstages = (nrec + R - 1) / R;
   if (lane == 0) {
@@ -181,129 +412,43 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   __syncwarp();
 
   const double hdt = a.hdt;
-  unsigned stat_calls = 0, stat_iters = 0, stat_slow = 0;
-  int k = 0;  // global record index
+  // 2 mu, exactly, by an exponent increment in the integer (uniform) pipe
+  const double two_mu = __longlong_as_double(__double_as_longlong(a.mu) + (1LL << 52));
+  const bool fast_on = a.iters >= kFastMinIters && a.tol >= kFastMinTol;
+  const int lim_e2 = fast_on ? kHiE2_080 : 0;
+  const int lim_x = fast_on ? 0x3fe921fb : 0;   // high word of pi/4 (is_small_angle)
+  const double inv_mu_dt = DKD ? a.inv_mu_hdt : a.inv_mu_dt;
+  unsigned stat[3] = {0u, 0u, 0u};
+  double hdt2 = DKD ? hdt : 0.0;   // the second half kick: none at record 0 of KDK
+  bool finished = false;           // no lane has a particle left
   int st = 0;
   for (; st < nstages; ++st) {
     const int slot = st & (kRingSlots - 1);
     mbar_wait(&bars[slot], (st / kRingSlots) & 1);
-    const double* stage = ring + slot * stage_doubles;
+    uint32_t rec = ring_addr + static_cast<uint32_t>(slot * stage_doubles) * 8u;
     const int recs = min(R, nrec - st * R);
-    bool any_alive = true;
-    for (int kk = 0; kk < recs; ++kk, ++k) {
-      const double* rec = stage + kk * stride;
+    // the steps of this stage; in KDK the very last record of the launch is a kick without a drift
+    const int nfull = (!DKD && st == nstages - 1) ? recs - 1 : recs;
+    int kk = 0;
+    for (; kk < nfull; ++kk, rec += rec_bytes) {
+      const int k = st * R + kk;   // record index within the launch (used by the removal blocks only)
+      double r2;
       if (DKD) {  // ---- first half drift of step k (D1): flags 3 / 4 freeze the state of t_k
-        double r2h[P];
-        int st_h[P], fi;
-        bool ws;
-#pragma unroll
-        for (int p = 0; p < P; ++p) r2h[p] = fma(x[p], x[p], fma(y[p], y[p], z[p] * z[p]));
-        kepler_drift_warp<P, REFINE>(alive, a.mu, a.inv_mu, a.inv_mu_hdt, a.iters, a.tol, r2h, x, y, z, vx, vy, vz, st_h,
-                                     fi, ws);
-        if (STATS) { stat_calls += 1; stat_iters += fi; stat_slow += ws ? 1 : 0; }
-#pragma unroll
-        for (int p = 0; p < P; ++p) {
-          if (st_h[p] != 0) {
-            flag[p] = st_h[p];
-            rs[p] = k;
-            alive[p] = false;
-          }
-        }
+        r2 = fma(L.x, L.x, fma(L.y, L.y, L.z * L.z));
+        if (drift_with_flags<REFINE, STATS>(a, two_mu, inv_mu_dt, lim_e2, lim_x, r2, k, i, L, stat)) { finished = true; break; }
       }
-      // ---- a3/a4: force evaluation with the tests (O1/O4/O5) at time t_{step0+k} ----------------
-      // The tests compare squared distances (O5).  On the hot path they are taken on the HIGH WORDS
-      // in the integer pipe, as a superset (d2 < R2 implies hi(d2) <= hi(R2) for non-negative
-      // doubles); the exact fp64 comparisons run only in a warp where some lane passes the superset.
-      double r2[P], ax[P], ay[P], az[P];
-      bool maybe[P];
-#pragma unroll
-      for (int p = 0; p < P; ++p) {
-        r2[p] = fma(x[p], x[p], fma(y[p], y[p], z[p] * z[p]));
-        ax[p] = rec[3 * np]; ay[p] = rec[3 * np + 1]; az[p] = rec[3 * np + 2];  // h0
-        const int r2h = __double2hiint(r2[p]);
-        maybe[p] = (r2h >= a.rmax2_hi) || (r2h <= a.rmin2_hi);
-      }
-#pragma unroll
-      for (int j = 0; j < np; ++j) {
-        const double qx = rec[3 * j], qy = rec[3 * j + 1], qz = rec[3 * j + 2];
-#pragma unroll
-        for (int p = 0; p < P; ++p) {
-          const double dx = x[p] - qx, dy = y[p] - qy, dz = z[p] - qz;
-          const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
-          maybe[p] = maybe[p] || (__double2hiint(d2) <= a.rc2_hi[j]);
-          const double w = gm_over_r3(a.gm[j], d2);
-          ax[p] = fma(-w, dx, ax[p]);
-          ay[p] = fma(-w, dy, ay[p]);
-          az[p] = fma(-w, dz, az[p]);
-        }
-      }
-      int hit[P];
-      bool any_maybe = false;
-#pragma unroll
-      for (int p = 0; p < P; ++p) {
-        hit[p] = 0;
-        any_maybe = any_maybe || (maybe[p] && alive[p]);
-      }
-      if (__any_sync(kFullMask, any_maybe)) {  // rare: the exact tests, lowest planet index wins (S11)
-        for (int jj = 0; jj < np; ++jj) {
-          const int j = np - 1 - jj;
-          const double qx = rec[3 * j], qy = rec[3 * j + 1], qz = rec[3 * j + 2];
-#pragma unroll
-          for (int p = 0; p < P; ++p) {
-            const double dx = x[p] - qx, dy = y[p] - qy, dz = z[p] - qz;
-            const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
-            hit[p] = (d2 < a.rc2[j]) ? (GLISSE_FLAG_PLANET0 + j) : hit[p];
-          }
-        }
-#pragma unroll
-        for (int p = 0; p < P; ++p) {
-          hit[p] = (r2[p] > a.rmax2) ? GLISSE_FLAG_RMAX : hit[p];
-          hit[p] = (r2[p] < a.rmin2) ? GLISSE_FLAG_RMIN : hit[p];
-        }
-      }
-      bool any_alive_k = false;
-#pragma unroll
-      for (int p = 0; p < P; ++p) {
-        if (alive[p] && hit[p] != 0) {
-          flag[p] = hit[p];
-          rs[p] = k;
-          alive[p] = false;
-        }
-        if (alive[p]) {
-          vx[p] = fma(ax[p], hdt, vx[p]); vy[p] = fma(ay[p], hdt, vy[p]); vz[p] = fma(az[p], hdt, vz[p]);
-          // KDK interior: closing half kick of step k-1 and opening of step k; DKD: the one full kick (D3)
-          if (DKD || (k > 0 && k < nsteps)) {
-            vx[p] = fma(ax[p], hdt, vx[p]); vy[p] = fma(ay[p], hdt, vy[p]); vz[p] = fma(az[p], hdt, vz[p]);
-          }
-        }
-      }
+      // ---- a3/a4: force evaluation with the tests at time t_{step0+k}, kick(s) ------------------------
+      if (kick_with_tests<NP>(a, np, rec, k, i, hdt, hdt2, L, r2)) { finished = true; break; }
       // ---- a5/a6: drift (O2; in DKD the second half drift, D4) ---------------------------------------
-      if (DKD || k < nsteps) {
-        int st_d[P];
-        int fast_iters;
-        bool went_slow;
-        kepler_drift_warp<P, REFINE>(alive, a.mu, a.inv_mu, DKD ? a.inv_mu_hdt : a.inv_mu_dt, a.iters, a.tol, r2, x, y,
-                                     z, vx, vy, vz, st_d, fast_iters, went_slow);
-        if (STATS) {
-          stat_calls += 1;
-          stat_iters += fast_iters;
-          stat_slow += went_slow ? 1 : 0;
-        }
-#pragma unroll
-        for (int p = 0; p < P; ++p) {
-          if (st_d[p] != 0) {
-            flag[p] = st_d[p];
-            rs[p] = k;
-            alive[p] = false;
-          }
-        }
-      }
-#pragma unroll
-      for (int p = 0; p < P; ++p) any_alive_k = any_alive_k || alive[p];
-      any_alive = __any_sync(kFullMask, any_alive_k);
-      if (!any_alive) break;
+      if (DKD) r2 = fma(L.x, L.x, fma(L.y, L.y, L.z * L.z));
+      if (drift_with_flags<REFINE, STATS>(a, two_mu, inv_mu_dt, lim_e2, lim_x, r2, k, i, L, stat)) { finished = true; break; }
+      hdt2 = hdt;
     }
-    if (!any_alive) break;
+    if (finished) break;
+    if (kk < recs) {   // KDK: closing half kick of the launch's last step at record nsteps
+      double r2;
+      if (kick_with_tests<NP>(a, np, rec, st * R + kk, i, hdt, 0.0, L, r2)) { finished = true; break; }
+    }
     __syncwarp();
     if (lane == 0 && st + kRingSlots < nstages) {
       const int nx = st + kRingSlots;
@@ -320,39 +465,27 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
       mbar_wait(&bars[o & (kRingSlots - 1)], (o / kRingSlots) & 1);
   }
 
-  // ---- a7: store --------------------------------------------------------------------------------
-#pragma unroll
-  for (int p = 0; p < P; ++p) {
-    if (was_alive[p]) {  // particles that were already removed at load are untouched
-      const long long i = i0 + p * kParticleBlock;
-      a.st[0][i] = x[p]; a.st[1][i] = y[p]; a.st[2][i] = z[p];
-      a.st[3][i] = vx[p]; a.st[4][i] = vy[p]; a.st[5][i] = vz[p];
-      if (flag[p] != 0) {
-        a.flag[i] = flag[p];
-        a.rstep[i] = a.step0 + rs[p];
-      }
-    }
+  // ---- a7: store (particles flagged during this launch were written when they were flagged) ----------
+  if (own && L.flag == 0) {
+    a.st[0][i] = L.x; a.st[1][i] = L.y; a.st[2][i] = L.z;
+    a.st[3][i] = L.vx; a.st[4][i] = L.vy; a.st[5][i] = L.vz;
   }
-  // steps started by this thread's particles: all nsteps for a survivor; for a particle flagged at
+  // steps started by this thread's particle: all nsteps for a survivor; for a particle flagged at
   // record k, KDK: k if a force-evaluation test caught it and k + 1 if its drift did (flags 3 and 4);
   // DKD: k + 1 whatever caught it (the step had begun with its first half drift)
   unsigned drifts = 0;
-#pragma unroll
-  for (int p = 0; p < P; ++p) {
-    if (was_alive[p])
-      drifts += flag[p] == 0 ? static_cast<unsigned>(nsteps)
-                             : static_cast<unsigned>(rs[p]) +
-                                   ((DKD || flag[p] == GLISSE_FLAG_NONCONV || flag[p] == GLISSE_FLAG_UNBOUND) ? 1u : 0u);
-  }
+  if (own)
+    drifts = L.flag == 0 ? static_cast<unsigned>(nsteps)
+                         : static_cast<unsigned>(L.rs) +
+                               ((DKD || L.flag == GLISSE_FLAG_NONCONV || L.flag == GLISSE_FLAG_UNBOUND) ? 1u : 0u);
   unsigned tot = __reduce_add_sync(kFullMask, drifts);
   if (lane == 0 && tot) atomicAdd(a.pstep_counter, static_cast<unsigned long long>(tot));
   if (STATS && lane == 0) {
-    atomicAdd(a.solver_stats, static_cast<unsigned long long>(stat_calls));
-    atomicAdd(a.solver_stats + 1, static_cast<unsigned long long>(stat_iters));
-    atomicAdd(a.solver_stats + 2, static_cast<unsigned long long>(stat_slow));
+    atomicAdd(a.solver_stats, static_cast<unsigned long long>(stat[0]));
+    atomicAdd(a.solver_stats + 1, static_cast<unsigned long long>(stat[1]));
+    atomicAdd(a.solver_stats + 2, static_cast<unsigned long long>(stat[2]));
   }
-  // (the group index is rebuilt from i0 rather than kept live across the step loop)
-  publish_group(a, lane, static_cast<int>((i0 - threadIdx.x) / (kParticleBlock * P)));
+  publish_group(a, lane, static_cast<int>((i - threadIdx.x) / kParticleBlock));
 }
 
 size_t particle_smem_bytes(const ParticleArgs& a) {
@@ -388,7 +521,7 @@ __global__ void __launch_bounds__(256) count_refine_kernel(const double* x, cons
 
 template <int NP, bool STATS, bool DKD, bool REFINE>
 cudaError_t configure_kernel() {
-  return cudaFuncSetAttribute(particle_kernel<NP, kParticlesPerThread, STATS, DKD, REFINE>,
+  return cudaFuncSetAttribute(particle_kernel<NP, STATS, DKD, REFINE>,
                               cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
 }
 
@@ -415,7 +548,7 @@ cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chai
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = chained ? 1 : 0;
-  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, kParticlesPerThread, STATS, DKD, REFINE>, a);
+  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, STATS, DKD, REFINE>, a);
 }
 
 template <int NP, bool REFINE>
