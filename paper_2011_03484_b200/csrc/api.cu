@@ -853,6 +853,12 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   a.rmax2 = (prm.r_max > 0.0 && std::isfinite(prm.r_max)) ? prm.r_max * prm.r_max
                                                            : std::numeric_limits<double>::infinity();
   a.tol = prm.kepler_tol;
+  a.two_mu = 2.0 * gm_star;
+  {
+    const bool fast_on = fast_solver_allowed(prm.kepler_iters, prm.kepler_tol);
+    a.fast_lim_e2 = fast_on ? fast_solver_e2_limit() : 0;
+    a.fast_lim_x = fast_on ? fast_solver_x_limit() : 0;
+  }
   for (int j = 0; j < kMaxPlanets; ++j) {
     a.gm[j] = (j < np) ? gm_planet[j] : 0.0;
     a.rc2[j] = (j < np && planet_rcrit) ? planet_rcrit[j] * planet_rcrit[j] : 0.0;

@@ -36,6 +36,25 @@ inline int stage_records(int np) {
 
 // ---- arguments of the particle kernel (a2–a7), passed by value as a __grid_constant__ ----------
 struct ParticleArgs {
+  // Read by every step of the kernel, so laid out for 16-byte constant-bank loads: the scalars of the
+  // drift first, then the kick's per-planet constants, each group on a 16-byte boundary.
+  alignas(16) double mu;
+  double inv_mu;
+  double inv_mu_dt;
+  double two_mu;                       // 2 mu
+  double inv_mu_hdt;                   // (dt / 2) / mu: the half drifts of the drift-kick-drift scheme
+  double hdt;
+  alignas(16) double gm[kMaxPlanets];
+  // high words of rc2[], rmin2, rmax2: the hot path's integer superset of the distance tests
+  alignas(16) int rc2_hi[kMaxPlanets];
+  alignas(16) int rmin2_hi;
+  int rmax2_hi;
+  // high words below which a body may use the fast Kepler solver: of e^2 = 0.64 and of |x| = pi/4, both 0
+  // when the run's kepler_iters / kepler_tol keep the fast solver out (kepler.cuh)
+  int fast_lim_e2, fast_lim_x;
+  // ---- the rest is read once per launch or in the removal blocks only
+  double rmin2, rmax2, tol;
+  double rc2[kMaxPlanets];
   double* st[6];                       // x, y, z, vx, vy, vz  (struct of arrays, working order)
   int* flag;                           // 0 = active
   long long* rstep;                    // removal step
@@ -48,13 +67,6 @@ struct ParticleArgs {
   int stage_recs;
   int np;
   int iters;
-  double hdt, mu, inv_mu, inv_mu_dt, rmin2, rmax2, tol;
-  double inv_mu_hdt;                   // (dt / 2) / mu: the half drifts of the drift-kick-drift scheme
-  double gm[kMaxPlanets];
-  double rc2[kMaxPlanets];
-  // high words of rmin2, rmax2, rc2[]: the hot path's integer superset of the distance tests
-  int rmin2_hi, rmax2_hi;
-  int rc2_hi[kMaxPlanets];
   // Launch chaining: a chunk is issued as back-to-back launches of a few hundred steps
   // each, the later ones with programmatic stream serialisation, so that they become resident while
   // the earlier one drains.  A warp of launch j+1 takes the k-th group of 32 particles that launch j
@@ -95,6 +107,10 @@ cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool cha
 cudaError_t launch_count_refine(const double* const st[6], long long n, double mu, double dt, unsigned long long* out,
                                 cudaStream_t s);
 cudaError_t configure_particle_kernels();
+// host side of ParticleArgs::fast_lim_*: whether kepler_iters / kepler_tol admit the fast solver, and its limits
+bool fast_solver_allowed(int kepler_iters, double kepler_tol);
+int fast_solver_e2_limit();
+int fast_solver_x_limit();
 int particles_per_group();
 
 // Planet-history kernel (a1): from the Jacobi state `jin` write nsteps+1 log records and nsteps+1

@@ -115,6 +115,10 @@ __device__ __forceinline__ double lds_f64(uint32_t addr) {
   return v;
 }
 
+__device__ __forceinline__ void lds_f64x2(uint32_t addr, double& v0, double& v1) {
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v0), "=d"(v1) : "r"(addr));
+}
+
 // The per-lane state of the step loop.  A lane whose own particle is gone (removed in an earlier launch,
 // past the end of the array, or flagged during this launch) is `dead`: it goes on with a COPY of a live
 // lane's body (its donor), so that it computes exactly what the donor computes — never a NaN, a slow
@@ -196,19 +200,37 @@ __device__ __forceinline__ bool kick_with_tests(const ParticleArgs& a, int np, u
   // integer pipe, as a superset (d2 < R2 implies hi(d2) <= hi(R2) for non-negative doubles); the exact
   // fp64 comparisons run only in a warp where some lane passes the superset.
   r2 = fma(L.x, L.x, fma(L.y, L.y, L.z * L.z));
-  double ax = lds_f64(rec + 24 * np), ay = lds_f64(rec + 24 * np + 8), az = lds_f64(rec + 24 * np + 16);  // h0
   const int r2h = __double2hiint(r2);
-  bool maybe = (r2h >= a.rmax2_hi) || (r2h <= a.rmin2_hi);
+  bool maybe = (r2h >= a.rmax2_hi) | (r2h <= a.rmin2_hi);   // (| not ||: no short-circuit, no predicated loads)
+  double ax, ay, az;
+  if (NP > 0) {   // the record as 16-byte shared-memory loads (records are 16-byte aligned, stride even)
+    constexpr int kD = 3 * (NP > 0 ? NP : 1) + 3;
+    double rv[kD + 1];
 #pragma unroll
-  for (int j = 0; j < np; ++j) {
-    const double qx = lds_f64(rec + 24 * j), qy = lds_f64(rec + 24 * j + 8), qz = lds_f64(rec + 24 * j + 16);
-    const double dx = L.x - qx, dy = L.y - qy, dz = L.z - qz;
-    const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
-    maybe = maybe || (__double2hiint(d2) <= a.rc2_hi[j]);
-    const double w = gm_over_r3(a.gm[j], d2);
-    ax = fma(-w, dx, ax);
-    ay = fma(-w, dy, ay);
-    az = fma(-w, dz, az);
+    for (int c = 0; c < kD; c += 2) lds_f64x2(rec + 8 * c, rv[c], rv[c + 1]);
+    ax = rv[3 * NP]; ay = rv[3 * NP + 1]; az = rv[3 * NP + 2];  // h0
+#pragma unroll
+    for (int j = 0; j < NP; ++j) {
+      const double dx = L.x - rv[3 * j], dy = L.y - rv[3 * j + 1], dz = L.z - rv[3 * j + 2];
+      const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      maybe = maybe | (__double2hiint(d2) <= a.rc2_hi[j]);
+      const double w = gm_over_r3(a.gm[j], d2);
+      ax = fma(-w, dx, ax);
+      ay = fma(-w, dy, ay);
+      az = fma(-w, dz, az);
+    }
+  } else {
+    ax = lds_f64(rec + 24 * np); ay = lds_f64(rec + 24 * np + 8); az = lds_f64(rec + 24 * np + 16);  // h0
+    for (int j = 0; j < np; ++j) {
+      const double qx = lds_f64(rec + 24 * j), qy = lds_f64(rec + 24 * j + 8), qz = lds_f64(rec + 24 * j + 16);
+      const double dx = L.x - qx, dy = L.y - qy, dz = L.z - qz;
+      const double d2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      maybe = maybe | (__double2hiint(d2) <= a.rc2_hi[j]);
+      const double w = gm_over_r3(a.gm[j], d2);
+      ax = fma(-w, dx, ax);
+      ay = fma(-w, dy, ay);
+      az = fma(-w, dz, az);
+    }
   }
   if (__any_sync(kFullMask, maybe)) {  // rare
     KickRecord io;
@@ -304,7 +326,7 @@ __device__ __forceinline__ bool drift_with_flags(const ParticleArgs& a, double t
   drift_begin<REFINE>(a.mu, two_mu, a.inv_mu, inv_mu_dt, r2, L.x, L.y, L.z, L.vx, L.vy, L.vz, v, xk, unbound);
   const int e2h = hi_word(v.e2);
   const int thr = fast_threshold(e2h);
-  const bool notopen = unbound || !(e2h < lim_e2) || !(hi_abs(xk) < lim_x);
+  const bool notopen = unbound | !(e2h < lim_e2) | !(hi_abs(xk) < lim_x);
   fast_step(v, xk, xn, sm, cm1, dl);
   const bool done = hi_abs(dl) < thr;
   if (STATS) { stat[0] += 1; stat[1] += lim_x != 0 ? 1 : 0; }
@@ -412,11 +434,8 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
   __syncwarp();
 
   const double hdt = a.hdt;
-  // 2 mu, exactly, by an exponent increment in the integer (uniform) pipe
-  const double two_mu = __longlong_as_double(__double_as_longlong(a.mu) + (1LL << 52));
-  const bool fast_on = a.iters >= kFastMinIters && a.tol >= kFastMinTol;
-  const int lim_e2 = fast_on ? kHiE2_080 : 0;
-  const int lim_x = fast_on ? 0x3fe921fb : 0;   // high word of pi/4 (is_small_angle)
+  const double two_mu = a.two_mu;
+  const int lim_e2 = a.fast_lim_e2, lim_x = a.fast_lim_x;
   const double inv_mu_dt = DKD ? a.inv_mu_hdt : a.inv_mu_dt;
   unsigned stat[3] = {0u, 0u, 0u};
   double hdt2 = DKD ? hdt : 0.0;   // the second half kick: none at record 0 of KDK
@@ -583,6 +602,12 @@ cudaError_t launch_count_refine(const double* const st[6], long long n, double m
   count_refine_kernel<<<static_cast<int>((n + 255) / 256), 256, 0, s>>>(st[0], st[1], st[2], st[3], st[4], st[5], n, mu, dt, out);
   return cudaGetLastError();
 }
+
+bool fast_solver_allowed(int kepler_iters, double kepler_tol) {
+  return kepler_iters >= kFastMinIters && kepler_tol >= kFastMinTol;
+}
+int fast_solver_e2_limit() { return kHiE2_080; }
+int fast_solver_x_limit() { return 0x3fe921fb; }   // high word of pi/4 (is_small_angle)
 
 // particles per launch group (one warp's worth): the host sizes grids and completion lists with it
 int particles_per_group() { return kParticleBlock * kParticlesPerThread; }
