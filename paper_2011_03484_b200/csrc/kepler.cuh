@@ -444,8 +444,10 @@ __device__ __forceinline__ void drift_begin(double mu, double two_mu, double inv
   k.q = r0 * (al * inv_mu);              // r0 / a = 1 − ec
   k.ec = 1.0 - k.q;
   k.es = u * (k.sqa * inv_mu);
-  const double ndt = (al * k.sqa) * inv_mu_dt;                  // n dt
-  k.dM = fma(-rint(ndt * kInvTwoPi), kTwoPi, ndt);              // reading S9
+  // n dt.  The reduction of reading S9 (dM = n dt - 2 pi rint(n dt / 2 pi)) changes nothing while
+  // |n dt| <= pi, i.e. while a step spans less than half a revolution: it is left to reduce_mean_motion,
+  // which the caller applies (out of line) to the bodies whose |n dt| is not below kHiPi
+  k.dM = (al * k.sqa) * inv_mu_dt;
   k.a = mu * inva;
   k.invq = k.a * k.rinv;  // a / r0
   k.e2 = fma(k.ec, k.ec, k.es * k.es);
@@ -463,6 +465,12 @@ __device__ __forceinline__ void drift_begin(double mu, double two_mu, double inv
   }
 }
 
+// reading S9 for a body whose step spans half a revolution or more (drift_begin)
+constexpr int kHiPi = 0x400921fb;   // high word of pi = 0x400921fb54442d18: hi_abs(x) < kHiPi implies |x| < pi
+__device__ __forceinline__ double reduce_mean_motion(double ndt) {
+  return fma(-rint(ndt * kInvTwoPi), kTwoPi, ndt);
+}
+
 // Acceptance bound of the fast solver for this eccentricity (high word of the bound on |delta|), for the
 // particle kernel: the same error model as the tiers above — (5 a2^3 + 5 a2 a3 + a4) delta^4 < 2e-17
 // with a_k = e / (k! (1 - e)) — as ONE integer instruction instead of seven: in the high words
@@ -472,6 +480,10 @@ __device__ __forceinline__ void drift_begin(double mu, double two_mu, double inv
 // which saves planet-crossing bodies a second step.
 constexpr int kHiThrLine = kHiE2_080 + kHiThr3 - 0x10000;
 __device__ __forceinline__ int fast_threshold(int e2h) { return min(kHiThr1, kHiThrLine - e2h); }
+// |delta| (high word, sign cleared) is below fast_threshold(e2h): as two compares and an add, no selects
+__device__ __forceinline__ bool fast_accepts(int dl_hi_abs, int e2h) {
+  return (dl_hi_abs < kHiThr1) & (dl_hi_abs + e2h < kHiThrLine);
+}
 
 // one step of the fast solver from xk: the new x, sin x − x and cos x − 1 there, and the Newton update dl
 __device__ __forceinline__ void fast_step(const DriftVars& k, double xk, double& xn, double& smn, double& cmn,

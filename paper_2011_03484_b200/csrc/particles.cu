@@ -257,11 +257,17 @@ struct DriftRecord {
 // still `open` (exactly as kepler_drift_warp takes them, starting with step number it0), the definition's
 // solver for the `slow` ones, flags 3 / 4 with the state on entry to the drift frozen, new donors.
 static __device__ __noinline__ bool solve_and_flag(const ParticleArgs& a, int it0, int k, long long i, DriftRecord* io) {
-  const DriftVars v = io->v;
+  DriftVars v = io->v;
   double xk = io->xk, sm = io->sm, cm1 = io->cm1;
   const int thr = io->thr;
   const bool unbound = io->unbound;
   bool open = io->open, slow = io->slow;
+  // a step of half a revolution or more: dM reduced to (-pi, pi] here (reading S9); the caller counted the
+  // body as not open, so the definition's solver takes it
+  if (!(hi_abs(v.dM) < kHiPi)) {
+    v.dM = reduce_mean_motion(v.dM);
+    io->v.dM = v.dM;
+  }
   unsigned iters = 0;
   for (int it = it0; it < kFastMaxIters && __any_sync(kFullMask, open); ++it) {
     double xn, smn, cmn, dl;
@@ -325,12 +331,17 @@ __device__ __forceinline__ bool drift_with_flags(const ParticleArgs& a, double t
   bool unbound;
   drift_begin<REFINE>(a.mu, two_mu, a.inv_mu, inv_mu_dt, r2, L.x, L.y, L.z, L.vx, L.vy, L.vz, v, xk, unbound);
   const int e2h = hi_word(v.e2);
-  const int thr = fast_threshold(e2h);
-  const bool notopen = unbound | !(e2h < lim_e2) | !(hi_abs(xk) < lim_x);
+  // (an unbound body needs no test of its own here: alpha <= 0 makes e^2 a NaN, a denormal alpha makes it 1,
+  // and either fails e2h < lim_e2)
+  // (nor does a step of half a revolution or more: |x| = |dM| a / r0 >= |dM| (1 - e) / ... is not relied on —
+  // the mean motion has its own test, since dM is not reduced on this path)
+  const bool hard = !(e2h < lim_e2) | !(hi_abs(xk) < lim_x) | !(hi_abs(v.dM) < kHiPi);
   fast_step(v, xk, xn, sm, cm1, dl);
-  const bool done = hi_abs(dl) < thr;
+  const bool done = fast_accepts(hi_abs(dl), e2h);
   if (STATS) { stat[0] += 1; stat[1] += lim_x != 0 ? 1 : 0; }
-  if (__any_sync(kFullMask, notopen || !done)) {
+  if (__any_sync(kFullMask, hard | !done)) {
+    const int thr = fast_threshold(e2h);
+    const bool notopen = unbound | hard;
     bool open = !notopen && !done && is_small_angle(xn);
     bool slow = !unbound && (notopen || (!done && !open));
     int it0 = 1;

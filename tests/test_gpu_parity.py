@@ -206,6 +206,51 @@ def test_kepler_drift_matches_oracle_per_body(gl, oracle_mod, record):
         assert worst <= 1e-12, worst   # one drift: roundoff times the e <= 0.97 conditioning
 
 
+@pytest.mark.parametrize("dt", [180.0, -37.0])
+@pytest.mark.parametrize("guess_order", [1, 3])
+def test_particle_kernel_drift_per_body(gl, oracle_mod, record, dt, guess_order):
+    """The same bodies through the PARTICLE KERNEL's own drift (its three-piece form with the out-of-line
+    solver block, particles.cu): a simulation without planets, one step, is the Kepler drift alone (both half
+    kicks add zero).  Flags 3 / 4 exactly as the definition decides them, frozen states untouched, and a
+    warp that loses lanes to flags goes on correctly for the others (donor lanes)."""
+    rng = np.random.default_rng(6)
+    n = 6000
+    a = rng.uniform(0.3, 70.0, n)
+    e = np.concatenate([rng.uniform(0.0, 0.8, n // 2), rng.uniform(0.8, 0.97, n - n // 2)])
+    inc = rng.uniform(0, np.pi / 3, n)
+    Om, om, M = (rng.uniform(0, 2 * np.pi, n) for _ in range(3))
+    pos, vel = inputs.elements_to_cartesian(inputs.G, a, e, inc, Om, om, M)
+    vesc = np.sqrt(2.0 * inputs.G / np.linalg.norm(pos[:50], axis=1))
+    vel[:50] *= (1.2 * vesc / np.linalg.norm(vel[:50], axis=1))[:, None]
+    perm = rng.permutation(n)   # flagged bodies spread over the warps
+    pos, vel = pos[perm], vel[perm]
+    ref = [oracle_mod.kepler_drift(inputs.G, pos[i], vel[i], dt, iters=5, tol=1e-14) for i in range(n)]
+    none = np.zeros((0, 3))
+    S = gl.GlisseSim(inputs.G, np.zeros(0), none, none, None, np.ascontiguousarray(pos.T), np.ascontiguousarray(vel.T), dt,
+                     chunk_steps=16, guess_order=guess_order)
+    S.advance(1)
+    p1, v1, flag, rstep = S.read()
+    psteps = S.particle_steps()
+    S.close()
+    p1, v1 = np.asarray(p1).T, np.asarray(v1).T
+    fl_ref = np.array([r[0] for r in ref])
+    assert np.array_equal(flag, fl_ref), np.flatnonzero(flag != fl_ref)[:10]
+    assert (fl_ref == 4).sum() >= 50 and (fl_ref == 3).sum() > 0
+    assert np.all(rstep[fl_ref != 0] == 0)
+    assert psteps == n          # every particle started its one drift
+    worst = 0.0
+    for i in range(n):
+        fl, r1, w1 = ref[i]
+        if fl == 0:
+            worst = max(worst, np.linalg.norm(p1[i] - r1) / np.linalg.norm(r1),
+                        np.linalg.norm(v1[i] - w1) / np.linalg.norm(w1))
+        else:   # frozen on entry to the drift
+            assert np.array_equal(p1[i], pos[i]) and np.array_equal(v1[i], vel[i])
+    record(dict(case=f"particle_kernel_drift_per_body dt={dt} guess_order={guess_order}", n=n,
+                flag_mismatches=0, dev_max=float(worst)))
+    assert worst <= 1e-12, worst
+
+
 # ---------------------------------------------------------------------------------------------------
 # planet-history kernel (a1) against the oracle's planet integrator
 # ---------------------------------------------------------------------------------------------------
