@@ -62,14 +62,14 @@ FLOPS_PER_PLANET = 25.0
 # from that workload's own ncu capture (2 DFMA + DMUL + DADD thread-instructions / thread-steps;
 # dram__bytes_read.sum + dram__bytes_write.sum): (flops, bytes per launch, profile it was read from).
 #   flops per thread-step = (2 DFMA + DMUL + DADD of a launch) / (grid x 32 threads x 128 steps of the launch):
-#   1m_x4 3.657e10 / (31670 x 32 x 128), c2 4.575e9 / (3961 x ...), c3 9.455e9 / (8192 x ...),
-#   c4 5.064e10 / (32492 x ...), c5 1.486e11 / (116553 x ...)
+#   1m_x4 3.594e10 / (31670 x 32 x 128), c2 4.497e9 / (3961 x ...), c3 9.291e9 / (8192 x ...),
+#   c4 4.973e10 / (32492 x ...), c5 1.450e11 / (116554 x ...)
 NCU = {
-    "1m_x4": (281.9, 5.41e7, "profiles/r02_particle_kernel_1m_x4.md"),
-    "c2": (282.0, 6.65e6, "profiles/r02_particle_kernel_c2.md"),
-    "c3": (281.8, 1.37e7, "profiles/r02_particle_kernel_c3.md"),
-    "c4": (380.5, 5.60e7, "profiles/r02_particle_kernel_c4.md"),
-    "c5": (311.3, 3.20e8, "profiles/r02_particle_kernel_c5.md"),
+    "1m_x4": (277.1, 5.51e7, "profiles/r02b_particle_kernel_1m_x4.md"),
+    "c2": (277.2, 6.68e6, "profiles/r02b_particle_kernel_c2.md"),
+    "c3": (276.9, 1.37e7, "profiles/r02b_particle_kernel_c3.md"),
+    "c4": (373.6, 5.54e7, "profiles/r02b_particle_kernel_c4.md"),
+    "c5": (303.8, 3.37e8, "profiles/r02b_particle_kernel_c5.md"),
 }
 # FP64 peak: ncu reports sm__sass_thread_inst_executed_op_dfma_pred_on.sum.peak_sustained = 64 per SM
 # per cycle; x 148 SMs x 2 flops x 1.965 GHz (clocks.max.sm of B200_PROFILING.md)

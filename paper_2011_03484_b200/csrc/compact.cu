@@ -27,7 +27,7 @@ constexpr unsigned kFull = 0xffffffffu;
 // Hardness bin of an orbit for the particle kernel's Kepler solver (kepler.cuh): 0 = one quartic step
 // is accepted at every phase of the orbit, 1 = some phases need more, 2 = some phase leaves the fast
 // solver (e >= 0.8, |x0| > pi/4, unbound).  The fast solver starts from x0 = dM/q, q = 1 - e cos E0,
-// and accepts once the Newton update delta = f(x0)/f'(x0) is below an eccentricity-tiered bound;
+// and accepts once the Newton update delta = f(x0)/f'(x0) is below an eccentricity-dependent bound;
 // here delta is evaluated at 12 phases E0 of the orbit with a safety factor of 2, from the starting
 // point the run's instantiation would use (first order, or the third-order reversion where the body
 // qualifies for it: kepler.cuh).  A heuristic: it decides only which particles share a warp.
@@ -46,7 +46,7 @@ __device__ int hardness_bin(double mu, double dt, bool refine, double x, double 
   double dM = alpha * sqrt(alpha) * dt / mu;
   dM = fabs(dM - kTwoPi * rint(dM / kTwoPi));
   if (dM >= 0.78539816 * (1.0 - e)) return 2;
-  const double thr = 0.5 * (e2 < 0.01 ? 1e-4 : (e2 < 0.09 ? 9e-5 : (e2 < 0.25 ? 5.5e-5 : 2e-5)));
+  const double thr = 0.5 * fmin(9e-5, 1.9e-5 * 0.64 / e2);   // kepler.cuh: fast_threshold, with the safety factor
   double worst = 0.0;
   for (int k = 0; k < 12; ++k) {
     double s0, c0;
