@@ -29,7 +29,7 @@ HORIZON = 1000       # steps
 # Planet log over the horizon, per planet system: a 1-ulp roundoff per step in a
 # planet's energy random-walks into an along-track error of about 1.5 (n dt) 1.1e-16 s^1.5 / sqrt(3)
 # = 1e-12 at s = 1000 for n dt = 0.29; the oracle and the kernel each carry their own.  Tolerance =
-# 3 x the deviation measured on B200 (profiles/r02_parity_stats.md), keyed by (config, N_p).
+# 3 x the deviation measured on B200 (profiles/r02b_parity_stats.md), keyed by (config, N_p).
 PLANET_TOL = {(1, 4): 4.1e-12,    # measured 1.35e-12 (SURVEY.md §7 step 4 hoped for 1e-12)
               (4, 8): 3.3e-12,    # measured 1.08e-12
               (1, 1): 1.7e-11,    # measured 5.42e-12: Jupiter alone, exact Kepler orbit, pure drift roundoff
