@@ -143,6 +143,7 @@ struct glisse_sim {
   int chain_groups = 0;
   bool stats_on = false;
   bool refine = false;            // particle-kernel instantiation with the third-order Kepler starting point
+  bool definition_only = false;   // ... with the definition's Kepler solver alone (kepler_iters / kepler_tol)
   unsigned long long* d_stats = nullptr;  // [3]
 
   // snapshot staging (glisse_snapshot): a copy in original order that stream r ships to the caller
@@ -323,7 +324,7 @@ int launch_particles(glisse_sim* s, const double* log, int nsteps) {
     a.log = log + static_cast<size_t>(off) * s->stride;
     a.step0 = s->step + off;
     a.nsteps = m;
-    CKS(s, launch_particle_kernel(a, groups, !first, s->stats_on, s->dkd, s->refine, s->q));
+    CKS(s, launch_particle_kernel(a, groups, !first, s->stats_on, s->dkd, s->refine, s->definition_only, s->q));
     s->launches += 1;
     s->chain_len += 1;
   }
@@ -854,11 +855,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
                                                            : std::numeric_limits<double>::infinity();
   a.tol = prm.kepler_tol;
   a.two_mu = 2.0 * gm_star;
-  {
-    const bool fast_on = fast_solver_allowed(prm.kepler_iters, prm.kepler_tol);
-    a.fast_lim_e2 = fast_on ? fast_solver_e2_limit() : 0;
-    a.fast_lim_x = fast_on ? fast_solver_x_limit() : 0;
-  }
+  s->definition_only = !fast_solver_allowed(prm.kepler_iters, prm.kepler_tol);
   for (int j = 0; j < kMaxPlanets; ++j) {
     a.gm[j] = (j < np) ? gm_planet[j] : 0.0;
     a.rc2[j] = (j < np && planet_rcrit) ? planet_rcrit[j] * planet_rcrit[j] : 0.0;

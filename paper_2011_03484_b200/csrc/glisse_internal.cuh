@@ -49,9 +49,6 @@ struct ParticleArgs {
   alignas(16) int rc2_hi[kMaxPlanets];
   alignas(16) int rmin2_hi;
   int rmax2_hi;
-  // high words below which a body may use the fast Kepler solver: of e^2 = 0.64 and of |x| = pi/4, both 0
-  // when the run's kepler_iters / kepler_tol keep the fast solver out (kepler.cuh)
-  int fast_lim_e2, fast_lim_x;
   // ---- the rest is read once per launch or in the removal blocks only
   double rmin2, rmax2, tol;
   double rc2[kMaxPlanets];
@@ -101,16 +98,16 @@ inline int jstate_stride(int np) { return 6 * np; }
 // stats: the instrumented instantiation (glisse_test.h: glisse_solver_stats)
 // dkd: the drift-kick-drift instantiation (include/glisse.h: GLISSE_SCHEME_DKD)
 // refine: the instantiation with the third-order starting point of the Kepler solve (guess_order 3)
+// definition_only: the instantiation without the fast solver (see fast_solver_allowed)
 cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd, bool refine,
-                                   cudaStream_t s);
+                                   bool definition_only, cudaStream_t s);
 // *out += number of the n bodies that would take the third-order starting point at this instant
 cudaError_t launch_count_refine(const double* const st[6], long long n, double mu, double dt, unsigned long long* out,
                                 cudaStream_t s);
 cudaError_t configure_particle_kernels();
-// host side of ParticleArgs::fast_lim_*: whether kepler_iters / kepler_tol admit the fast solver, and its limits
+// whether kepler_iters / kepler_tol admit the fast solver (kepler.cuh: kFastMinIters, kFastMinTol); if not,
+// the simulation uses the particle-kernel instantiation that carries the definition's solver alone
 bool fast_solver_allowed(int kepler_iters, double kepler_tol);
-int fast_solver_e2_limit();
-int fast_solver_x_limit();
 int particles_per_group();
 
 // Planet-history kernel (a1): from the Jacobi state `jin` write nsteps+1 log records and nsteps+1

@@ -250,6 +250,7 @@ struct DriftRecord {
   double xk, sm, cm1;     // the solver's state: x, sin x − x, cos x − 1
   int thr;                // acceptance bound of the fast solver for this body
   bool unbound, open, slow;
+  int nonconv;            // the body has been through the definition's solver already and did not converge
   unsigned iters, went_slow;   // statistics: fast-solver steps taken here, slow path entered
 };
 
@@ -282,7 +283,7 @@ static __device__ __noinline__ bool solve_and_flag(const ParticleArgs& a, int it
     }
   }
   slow = slow || open;   // no convergence in kFastMaxIters steps
-  int nonconv = 0;
+  int nonconv = io->nonconv;
   io->went_slow = 0;
   if (__any_sync(kFullMask, slow)) {
     io->went_slow = 1;
@@ -317,28 +318,50 @@ static __device__ __noinline__ bool solve_and_flag(const ParticleArgs& a, int it
   return false;
 }
 
+// Which Kepler solver an instantiation of the kernel carries (chosen once per simulation, api.cu):
+// the fast solver from the first-order starting point, the same from the third-order one (REFINE in
+// kepler.cuh; include/glisse.h: guess_order), or the definition's solver alone for a run whose kepler_iters /
+// kepler_tol keep the fast one out (kepler.cuh: kFastMinIters, kFastMinTol).
+enum : int { kSolverFast = 0, kSolverFastRefined = 1, kSolverDefinition = 2 };
+
 // Kepler drift of the warp's 32 bodies (O2): begin, one fast-solver step, finish, with one vote in between
-// that sends the warp to solve_and_flag.  lim_e2 / lim_x are the high words below which a body may use the
-// fast solver (both 0 when the run's kepler_iters / kepler_tol keep it out).  In the REFINE instantiation
-// (planet-crossing populations) a second fast-solver step is common, so it is taken in line before the
-// call.  Returns true when no lane of the warp has a particle left.
-template <bool REFINE, bool STATS>
-__device__ __forceinline__ bool drift_with_flags(const ParticleArgs& a, double two_mu, double inv_mu_dt, int lim_e2,
-                                                 int lim_x, double r2, int k, long long i, Lane& L,
-                                                 unsigned (&stat)[3]) {
+// that sends the warp to solve_and_flag.  In the kSolverFastRefined instantiation (planet-crossing
+// populations) a second fast-solver step is common, so it is taken in line before the call; in the
+// kSolverDefinition one every body goes straight to kepler_solve_exact and only a flag goes out of line.
+// Returns true when no lane of the warp has a particle left.
+template <int SOLVER, bool STATS>
+__device__ __forceinline__ bool drift_with_flags(const ParticleArgs& a, double two_mu, double inv_mu_dt, double r2, int k,
+                                                 long long i, Lane& L, unsigned (&stat)[3]) {
+  constexpr bool REFINE = SOLVER == kSolverFastRefined;
   DriftVars v;
   double xk, xn, sm, cm1, dl;
   bool unbound;
   drift_begin<REFINE>(a.mu, two_mu, a.inv_mu, inv_mu_dt, r2, L.x, L.y, L.z, L.vx, L.vy, L.vz, v, xk, unbound);
+  if (SOLVER == kSolverDefinition) {
+    if (!(hi_abs(v.dM) < kHiPi)) v.dM = reduce_mean_motion(v.dM);
+    const ExactSolve o = kepler_solve_exact(!unbound, v.ec, v.es, v.q, v.dM, v.invq, v.e2, a.iters, a.tol);
+    xn = o.x; sm = o.sm; cm1 = o.cm1;
+    const int nonconv = unbound ? 0 : o.nonconv;
+    if (STATS) { stat[0] += 1; stat[2] += 1; }
+    if (__any_sync(kFullMask, unbound || nonconv != 0)) {
+      DriftRecord io;
+      io.L = L; io.v = v; io.xk = xn; io.sm = sm; io.cm1 = cm1; io.thr = 0;
+      io.unbound = unbound; io.open = false; io.slow = false; io.nonconv = nonconv;
+      const bool finished = solve_and_flag(a, kFastMaxIters, k, i, &io);
+      L = io.L; v = io.v; xn = io.xk; sm = io.sm; cm1 = io.cm1;
+      if (__any_sync(kFullMask, finished)) return true;
+    }
+    drift_finish(v, xn, sm, cm1, L.x, L.y, L.z, L.vx, L.vy, L.vz);
+    return false;
+  }
   const int e2h = hi_word(v.e2);
   // (an unbound body needs no test of its own here: alpha <= 0 makes e^2 a NaN, a denormal alpha makes it 1,
-  // and either fails e2h < lim_e2)
-  // (nor does a step of half a revolution or more: |x| = |dM| a / r0 >= |dM| (1 - e) / ... is not relied on —
-  // the mean motion has its own test, since dM is not reduced on this path)
-  const bool hard = !(e2h < lim_e2) | !(hi_abs(xk) < lim_x) | !(hi_abs(v.dM) < kHiPi);
+  // and either fails e2h < kHiE2_080; a step of half a revolution or more has one, since dM is not reduced
+  // on this path)
+  const bool hard = !(e2h < kHiE2_080) | !is_small_angle(xk) | !(hi_abs(v.dM) < kHiPi);
   fast_step(v, xk, xn, sm, cm1, dl);
   const bool done = fast_accepts(hi_abs(dl), e2h);
-  if (STATS) { stat[0] += 1; stat[1] += lim_x != 0 ? 1 : 0; }
+  if (STATS) { stat[0] += 1; stat[1] += 1; }
   if (__any_sync(kFullMask, hard | !done)) {
     const int thr = fast_threshold(e2h);
     const bool notopen = unbound | hard;
@@ -365,7 +388,7 @@ __device__ __forceinline__ bool drift_with_flags(const ParticleArgs& a, double t
     if (more) {
       DriftRecord io;
       io.L = L; io.v = v; io.xk = xn; io.sm = sm; io.cm1 = cm1; io.thr = thr;
-      io.unbound = unbound; io.open = open; io.slow = slow;
+      io.unbound = unbound; io.open = open; io.slow = slow; io.nonconv = 0;
       const bool finished = solve_and_flag(a, it0, k, i, &io);
       L = io.L; v = io.v; xn = io.xk; sm = io.sm; cm1 = io.cm1;
       if (STATS) { stat[1] += io.iters; stat[2] += io.went_slow; }
@@ -381,8 +404,8 @@ __device__ __forceinline__ bool drift_with_flags(const ParticleArgs& a, double t
 // DKD: the drift-kick-drift splitting (GLISSE_SCHEME_DKD): per step a half drift, the force evaluation
 // with the tests at the half-step record, a full kick, a half drift; nsteps records are read, not
 // nsteps + 1, and the state between launches is synchronised at the integer steps as in KDK.
-// REFINE: third-order starting point of the Kepler solve (kepler.cuh; include/glisse.h: guess_order).
-template <int NP, bool STATS, bool DKD, bool REFINE>
+// SOLVER: kSolverFast / kSolverFastRefined / kSolverDefinition (above).
+template <int NP, bool STATS, bool DKD, int SOLVER>
 __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel(const __grid_constant__ ParticleArgs a) {
   static_assert(kParticleBlock == 32, "one warp per block: the launch chain hands groups of one warp on");
   static_assert(kParticlesPerThread == 1, "one particle per thread");
@@ -446,7 +469,6 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
 
   const double hdt = a.hdt;
   const double two_mu = a.two_mu;
-  const int lim_e2 = a.fast_lim_e2, lim_x = a.fast_lim_x;
   const double inv_mu_dt = DKD ? a.inv_mu_hdt : a.inv_mu_dt;
   unsigned stat[3] = {0u, 0u, 0u};
   double hdt2 = DKD ? hdt : 0.0;   // the second half kick: none at record 0 of KDK
@@ -465,13 +487,13 @@ __global__ void __launch_bounds__(kParticleBlock, GL_MIN_BLOCKS) particle_kernel
       double r2;
       if (DKD) {  // ---- first half drift of step k (D1): flags 3 / 4 freeze the state of t_k
         r2 = fma(L.x, L.x, fma(L.y, L.y, L.z * L.z));
-        if (drift_with_flags<REFINE, STATS>(a, two_mu, inv_mu_dt, lim_e2, lim_x, r2, k, i, L, stat)) { finished = true; break; }
+        if (drift_with_flags<SOLVER, STATS>(a, two_mu, inv_mu_dt, r2, k, i, L, stat)) { finished = true; break; }
       }
       // ---- a3/a4: force evaluation with the tests at time t_{step0+k}, kick(s) ------------------------
       if (kick_with_tests<NP>(a, np, rec, k, i, hdt, hdt2, L, r2)) { finished = true; break; }
       // ---- a5/a6: drift (O2; in DKD the second half drift, D4) ---------------------------------------
       if (DKD) r2 = fma(L.x, L.x, fma(L.y, L.y, L.z * L.z));
-      if (drift_with_flags<REFINE, STATS>(a, two_mu, inv_mu_dt, lim_e2, lim_x, r2, k, i, L, stat)) { finished = true; break; }
+      if (drift_with_flags<SOLVER, STATS>(a, two_mu, inv_mu_dt, r2, k, i, L, stat)) { finished = true; break; }
       hdt2 = hdt;
     }
     if (finished) break;
@@ -549,24 +571,27 @@ __global__ void __launch_bounds__(256) count_refine_kernel(const double* x, cons
   if (threadIdx.x == 0 && c) atomicAdd(out, static_cast<unsigned long long>(c));
 }
 
-template <int NP, bool STATS, bool DKD, bool REFINE>
+template <int NP, bool STATS, bool DKD, int SOLVER>
 cudaError_t configure_kernel() {
-  return cudaFuncSetAttribute(particle_kernel<NP, STATS, DKD, REFINE>,
+  return cudaFuncSetAttribute(particle_kernel<NP, STATS, DKD, SOLVER>,
                               cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
 }
 
+// the instantiations that exist: {plain, DKD} x three solvers, and the instrumented plain one for the two fast solvers
 template <int NP>
 cudaError_t configure_one() {
   cudaError_t e;
-  if ((e = configure_kernel<NP, false, false, false>())) return e;
-  if ((e = configure_kernel<NP, false, false, true>())) return e;
-  if ((e = configure_kernel<NP, false, true, false>())) return e;
-  if ((e = configure_kernel<NP, false, true, true>())) return e;
-  if ((e = configure_kernel<NP, true, false, false>())) return e;
-  return configure_kernel<NP, true, false, true>();
+  if ((e = configure_kernel<NP, false, false, kSolverFast>())) return e;
+  if ((e = configure_kernel<NP, false, false, kSolverFastRefined>())) return e;
+  if ((e = configure_kernel<NP, false, false, kSolverDefinition>())) return e;
+  if ((e = configure_kernel<NP, false, true, kSolverFast>())) return e;
+  if ((e = configure_kernel<NP, false, true, kSolverFastRefined>())) return e;
+  if ((e = configure_kernel<NP, false, true, kSolverDefinition>())) return e;
+  if ((e = configure_kernel<NP, true, false, kSolverFast>())) return e;
+  return configure_kernel<NP, true, false, kSolverFastRefined>();
 }
 
-template <int NP, bool STATS, bool DKD, bool REFINE>
+template <int NP, bool STATS, bool DKD, int SOLVER>
 cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chained, cudaStream_t s) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(static_cast<unsigned>(blocks));
@@ -578,14 +603,24 @@ cudaError_t launch_one(const ParticleArgs& a, int blocks, size_t smem, bool chai
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = chained ? 1 : 0;
-  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, STATS, DKD, REFINE>, a);
+  return cudaLaunchKernelEx(&cfg, particle_kernel<NP, STATS, DKD, SOLVER>, a);
 }
 
-template <int NP, bool REFINE>
-cudaError_t launch_np(const ParticleArgs& a, int n_groups, size_t smem, bool chained, bool stats, bool dkd, cudaStream_t s) {
-  if (dkd) return launch_one<NP, false, true, REFINE>(a, n_groups, smem, chained, s);   // (no instrumented DKD instantiation)
-  return stats ? launch_one<NP, true, false, REFINE>(a, n_groups, smem, chained, s)
-               : launch_one<NP, false, false, REFINE>(a, n_groups, smem, chained, s);
+template <int NP>
+cudaError_t launch_np(const ParticleArgs& a, int n_groups, size_t smem, bool chained, bool stats, bool dkd, int solver,
+                      cudaStream_t s) {
+  // (no instrumented instantiation for DKD or for the definition's solver: their statistics stay zero)
+  if (solver == kSolverDefinition)
+    return dkd ? launch_one<NP, false, true, kSolverDefinition>(a, n_groups, smem, chained, s)
+               : launch_one<NP, false, false, kSolverDefinition>(a, n_groups, smem, chained, s);
+  if (solver == kSolverFastRefined) {
+    if (dkd) return launch_one<NP, false, true, kSolverFastRefined>(a, n_groups, smem, chained, s);
+    return stats ? launch_one<NP, true, false, kSolverFastRefined>(a, n_groups, smem, chained, s)
+                 : launch_one<NP, false, false, kSolverFastRefined>(a, n_groups, smem, chained, s);
+  }
+  if (dkd) return launch_one<NP, false, true, kSolverFast>(a, n_groups, smem, chained, s);
+  return stats ? launch_one<NP, true, false, kSolverFast>(a, n_groups, smem, chained, s)
+               : launch_one<NP, false, false, kSolverFast>(a, n_groups, smem, chained, s);
 }
 
 }  // namespace
@@ -598,13 +633,14 @@ cudaError_t configure_particle_kernels() {
 }
 
 cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd, bool refine,
-                                   cudaStream_t s) {
+                                   bool definition_only, cudaStream_t s) {
   if (n_groups < 1) n_groups = 1;
   const size_t smem = particle_smem_bytes(a);
+  const int solver = definition_only ? kSolverDefinition : (refine ? kSolverFastRefined : kSolverFast);
   cudaError_t e;
-  if (a.np == 4) e = refine ? launch_np<4, true>(a, n_groups, smem, chained, stats, dkd, s) : launch_np<4, false>(a, n_groups, smem, chained, stats, dkd, s);
-  else if (a.np == 8) e = refine ? launch_np<8, true>(a, n_groups, smem, chained, stats, dkd, s) : launch_np<8, false>(a, n_groups, smem, chained, stats, dkd, s);
-  else e = refine ? launch_np<0, true>(a, n_groups, smem, chained, stats, dkd, s) : launch_np<0, false>(a, n_groups, smem, chained, stats, dkd, s);
+  if (a.np == 4) e = launch_np<4>(a, n_groups, smem, chained, stats, dkd, solver, s);
+  else if (a.np == 8) e = launch_np<8>(a, n_groups, smem, chained, stats, dkd, solver, s);
+  else e = launch_np<0>(a, n_groups, smem, chained, stats, dkd, solver, s);
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
@@ -617,8 +653,6 @@ cudaError_t launch_count_refine(const double* const st[6], long long n, double m
 bool fast_solver_allowed(int kepler_iters, double kepler_tol) {
   return kepler_iters >= kFastMinIters && kepler_tol >= kFastMinTol;
 }
-int fast_solver_e2_limit() { return kHiE2_080; }
-int fast_solver_x_limit() { return 0x3fe921fb; }   // high word of pi/4 (is_small_angle)
 
 // particles per launch group (one warp's worth): the host sizes grids and completion lists with it
 int particles_per_group() { return kParticleBlock * kParticlesPerThread; }
