@@ -784,6 +784,49 @@ def test_crafted_removals_match_oracle(gl, oracle_mod):
     assert np.array_equal(p, pos) and np.array_equal(v, vel)
 
 
+def test_warps_that_lose_their_lanes_one_by_one(gl, oracle_mod):
+    """Donor lanes (particles.cu): a lane whose particle is gone runs a copy of a live lane's body.  Three
+    warps: in the first every particle leaves through r_max at a time of its own, spread over many launches; in
+    the second all but one do; the third keeps (nearly) all of its own.  Flags and removal steps exact, states within tolerance,
+    and nothing depends on how the run is cut into launches or on compaction (the dead lanes then persist
+    for the whole run, or are repacked with live ones)."""
+    import dataclasses
+    w = inputs.config(1)
+    rng = np.random.default_rng(11)
+    n_out = 63
+    a = np.full(n_out, 30.0)
+    e = rng.uniform(0.45, 0.6, n_out)                       # apocentres 43.5 .. 48 AU, beyond r_max = 42
+    M = rng.uniform(0.25 * np.pi, 0.95 * np.pi, n_out)      # on their way out, at different phases
+    inc = rng.uniform(0.3, 0.6, n_out)                      # out of the planets' plane
+    Om, om = rng.uniform(0, 2 * np.pi, n_out), rng.uniform(0, 2 * np.pi, n_out)
+    po, vo = inputs.elements_to_cartesian(inputs.G, a, e, inc, Om, om, M)
+    pos = w.pos[:, :96].copy()
+    vel = w.vel[:, :96].copy()
+    pos[:, :32] = po[:32].T; vel[:, :32] = vo[:32].T         # warp 0: all leave
+    pos[:, 33:64] = po[32:].T; vel[:, 33:64] = vo[32:].T     # warp 1: lane 0 (particle 32) stays
+    w2 = dataclasses.replace(w, pos=pos, vel=vel, r_max=42.0)
+    steps = 300
+    (p0, v0, f0, r0), ps0 = _oracle_run(oracle_mod, w2, steps)
+    gone = f0 != 0
+    assert gone[:32].all() and gone[33:64].all() and not gone[32] and gone[64:].sum() <= 2
+    assert len(set(r0[:64][gone[:64]].tolist())) >= 20       # at least twenty distinct removal steps
+    ref = None
+    for kw in (dict(chunk_steps=32, segment_steps=8, resync_chunks=0), dict(chunk_steps=32, segment_steps=8, resync_chunks=1),
+               dict(chunk_steps=300, segment_steps=0, resync_chunks=0), dict(chunk_steps=7, segment_steps=3, resync_chunks=2)):
+        S = gl.GlisseSim.from_workload(w2, **kw)
+        S.advance(steps)
+        p, v, f, r = S.read()
+        ps = S.particle_steps()
+        S.close()
+        assert np.array_equal(f, f0) and np.array_equal(r, r0), kw
+        assert ps == ps0, kw
+        assert max(_dev(p, p0).max(), _dev(v, v0).max()) <= TOL, kw
+        if ref is None:
+            ref = (p.copy(), v.copy())
+        else:
+            assert np.array_equal(p, ref[0]) and np.array_equal(v, ref[1]), kw
+
+
 @pytest.mark.parametrize("e", [0.8, 0.95])
 def test_nonconvergence_flag(gl, oracle_mod, e):
     """Too few Newton updates near pericentre cannot converge: flag 3 at the oracle's step
