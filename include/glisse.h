@@ -77,7 +77,11 @@ typedef struct {
   double r_max;         /* heliocentric outer removal radius; +inf (or <= 0) disables the test */
   int    kepler_iters;  /* maximum number of Newton updates per Kepler solve, default 5        */
   double kepler_tol;    /* |residual of Kepler's equation| above which a particle is flagged
-                           GLISSE_FLAG_NONCONV, default 1e-14                   */
+                           GLISSE_FLAG_NONCONV, default 1e-14.  With kepler_iters >= 5
+                           and kepler_tol >= 4e-15 bodies with e < 0.8 are solved by a faster method
+                           that reaches the same root to roundoff and leaves a residual below 2e-15;
+                           otherwise every body goes through the Newton loop these two describe
+                           (a slower kernel, chosen at create)                                  */
   int    chunk_steps;   /* K: steps per planet-log chunk = per particle-kernel launch,
                            default 1024, 1..16384; performance only, results do not depend on it */
   int    resync_chunks; /* R: survivor compaction every R chunks, 0 = never, default 1;
