@@ -169,11 +169,18 @@ __global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* 
   const int stride = log_stride(L.np);
   const double hdt = 0.5 * dt;
   const double inv_mu_dt = L.inv_mu * dt;
+  const double two_mu = 2.0 * L.mu;
   // Idle lanes (lane >= np) carry a stand-in: a circular orbit with n dt = 0.01, never kicked, never
   // written.  It takes the same path through the drift as the planets (one quartic step), so the
   // warp does not diverge there; a lane that is merely masked off would.
+  // Each idle lane sits at its own phase of that circle: two lanes at the same point would meet at distance
+  // zero in the all-pairs exchange, and the NaN of that (discarded) term would reach the lane's velocity
+  // through 0 x NaN, and from there send the whole warp through the definition's solver at every step.
   const double r_idle = cbrt(L.gm0 * dt * dt * 1e4);
-  double rx = r_idle, ry = 0.0, rz = 0.0, vx = 0.0, vy = sqrt(L.gm0 / r_idle), vz = 0.0;
+  double s_idle, c_idle;
+  sincospi(L.lane * (1.0 / 16.0), &s_idle, &c_idle);
+  const double v_idle = sqrt(L.gm0 / r_idle);
+  double rx = r_idle * c_idle, ry = r_idle * s_idle, rz = 0.0, vx = -v_idle * s_idle, vy = v_idle * c_idle, vz = 0.0;
   if (L.live) {
     rx = jin[3 * L.lane]; ry = jin[3 * L.lane + 1]; rz = jin[3 * L.lane + 2];
     vx = jin[3 * L.np + 3 * L.lane]; vy = jin[3 * L.np + 3 * L.lane + 1]; vz = jin[3 * L.np + 3 * L.lane + 2];
@@ -187,8 +194,28 @@ __global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* 
     vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
     const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
     // third-order starting point (kepler.cuh): Jupiter at dt = 180 d needs one quartic step instead of two
-    const int st = kepler_drift_one<true>(true, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2,
-                                          rx, ry, rz, vx, vy, vz);
+    // The drift in the particle kernel's three pieces (kepler.cuh), with no per-lane predicate: begin, ONE
+    // fast-solver step, finish.  If any lane (planet or stand-in) is not served by that — not accepted, e >= 0.8,
+    // |x| > pi/4, a step of half a revolution or more, unbound — the whole warp takes the general routine
+    // instead, from the untouched state; for the lanes the short form does serve, the two are the same
+    // arithmetic, bit for bit.
+    int st = 0;
+    {
+      DriftVars dv;
+      double xk, xn, sm, cm1, dl;
+      bool unbound;
+      drift_begin<true>(L.mu, two_mu, L.inv_mu, inv_mu_dt, r2, rx, ry, rz, vx, vy, vz, dv, xk, unbound);
+      const int e2h = hi_word(dv.e2);
+      const int thr = e2h < kHiE2_010 ? kHiThr0 : (e2h < kHiE2_030 ? kHiThr1 : (e2h < kHiE2_050 ? kHiThr2 : kHiThr3));
+      const bool hard = !(e2h < kHiE2_080) | !is_small_angle(xk) | !(hi_abs(dv.dM) < kHiPi);
+      fast_step(dv, xk, xn, sm, cm1, dl);
+      if (__any_sync(kFullMask, hard | !(hi_abs(dl) < thr))) {
+        st = kepler_drift_one<true>(true, L.mu, L.inv_mu, inv_mu_dt, kPlanetKeplerIters, kPlanetKeplerTol, r2, rx, ry,
+                                    rz, vx, vy, vz);
+      } else {
+        drift_finish(dv, xn, sm, cm1, rx, ry, rz, vx, vy, vz);
+      }
+    }
     const unsigned failed = __ballot_sync(kFullMask, st != 0 && L.live);
     if (failed && bad < 0) bad = s;
     jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
