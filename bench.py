@@ -488,6 +488,32 @@ def run_ablations(binding, torch, device, flush):
     return out
 
 
+def run_full_configs(binding, device):
+    """BASELINE.json's five configurations AS STATED — every particle, every step (10^4, 10^5, 10^5, 2 x 10^4,
+    5 x 10^4), K = 1,024, compaction every chunk — in one glisse_advance each: wall time, particle-steps
+    (sum over steps of the active count), how many particles each removal flag took, surviving fraction."""
+    out = {}
+    for c in (1, 2, 3, 4, 5):
+        w = inputs.config(c)
+        t0 = time.perf_counter()
+        sim = binding.GlisseSim.from_workload(w, chunk_steps=CHUNK, resync_chunks=1, device=device.index)
+        t1 = time.perf_counter()
+        sim.advance(w.steps)
+        sim.sync()
+        t2 = time.perf_counter()
+        _, _, flag, rstep = sim.read()
+        ps = sim.particle_steps()
+        sim.close()
+        n = int(flag.shape[0])
+        flags = {str(int(k)): int(v) for k, v in zip(*np.unique(flag, return_counts=True))}
+        out[f"c{c}"] = {"n_particles": n, "n_planets": w.n_planets, "steps": int(w.steps), "dt_days": float(w.dt),
+                        "create_s": t1 - t0, "advance_s": t2 - t1, "particle_steps": int(ps),
+                        "value": ps / (t2 - t1), "nominal_particle_steps": n * int(w.steps),
+                        "surviving_fraction": float((flag == 0).mean()), "flags": flags,
+                        "median_removal_step": float(np.median(rstep[flag != 0])) if (flag != 0).any() else None}
+    return out
+
+
 def rank_main(argv):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -498,6 +524,8 @@ def rank_main(argv):
     ap.add_argument("--no-extras", action="store_true",
                     help="skip e2e, the other workloads, the long-advance line and the cpu baselines")
     ap.add_argument("--ablations", action="store_true", help="run the SURVEY.md 8(d) ablations instead")
+    ap.add_argument("--full-configs", action="store_true",
+                    help="run BASELINE.json's five configurations as stated (all particles, all steps) instead")
     args = ap.parse_args(argv)
     if args.warmup < 3:
         args.warmup = 3
@@ -520,6 +548,12 @@ def rank_main(argv):
         dist.init_process_group("nccl", device_id=device)
     binding.lib()
 
+    if args.full_configs:
+        if rank == 0:
+            print(json.dumps({"full_configs": run_full_configs(binding, device)}))
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=device)
     if args.ablations:
         if rank == 0:
