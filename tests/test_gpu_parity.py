@@ -827,6 +827,27 @@ def test_warps_that_lose_their_lanes_one_by_one(gl, oracle_mod):
             assert np.array_equal(p, ref[0]) and np.array_equal(v, ref[1]), kw
 
 
+def test_a_particle_does_not_depend_on_the_population(gl):
+    """Particles never interact: a particle's result must be the same bit for bit whether it
+    runs among 150 000 others (removals, compaction, donor lanes, launch chain all at work) or among 1 000."""
+    import dataclasses
+    w = inputs.config(5, 150_000)
+    S = gl.GlisseSim.from_workload(w, chunk_steps=256, resync_chunks=1)
+    S.advance(1500)
+    p, v, f, r = S.read()
+    S.close()
+    assert (f != 0).mean() > 0.03
+    for lo in (0, 77_777, 149_000):
+        sub = dataclasses.replace(w, pos=np.ascontiguousarray(w.pos[:, lo:lo + 1000]),
+                                  vel=np.ascontiguousarray(w.vel[:, lo:lo + 1000]))
+        T = gl.GlisseSim.from_workload(sub, chunk_steps=256, resync_chunks=1, guess_order=3)
+        T.advance(1500)
+        p2, v2, f2, r2 = T.read()
+        T.close()
+        assert np.array_equal(f[lo:lo + 1000], f2) and np.array_equal(r[lo:lo + 1000], r2)
+        assert np.array_equal(p[:, lo:lo + 1000], p2) and np.array_equal(v[:, lo:lo + 1000], v2)
+
+
 @pytest.mark.parametrize("e", [0.8, 0.95])
 def test_nonconvergence_flag(gl, oracle_mod, e):
     """Too few Newton updates near pericentre cannot converge: flag 3 at the oracle's step
