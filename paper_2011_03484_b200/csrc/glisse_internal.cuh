@@ -16,7 +16,7 @@ constexpr int kMaxPlanets = GLISSE_MAX_PLANETS;
 #define GL_PPT 1
 #endif
 constexpr int kParticleBlock = GL_BLOCK;     // threads per particle-kernel block
-constexpr int kParticlesPerThread = GL_PPT;  // particles per thread (independent instruction streams)
+constexpr int kParticlesPerThread = GL_PPT;  // particles per thread: the kernel as built supports 1 only
 constexpr int kParticleWarps = kParticleBlock / 32;
 constexpr int kRingSlots = 2;        // planet-log stages resident in shared memory per WARP
 #ifndef GL_MIN_BLOCKS

@@ -10,7 +10,7 @@
 // on its warp-mates, so results are bit-identical under compaction and re-chunking.
 // Then the Gauss f, g functions advance (r, v).
 //
-// The FP64 pipe is the roofline of the whole path (DESIGN.md §6), so every primitive here is
+// The FP64 pipe is the roofline of the whole path (DESIGN.md §7), so every primitive here is
 // written to a counted number of FP64-pipe instructions:
 //   rsqrt_f64   MUFU.RSQ64H seed + one cubic step          (2 DMUL + 3 DFMA)
 //   rcp_f64     MUFU.RCP64H seed + two quadratic steps     (4 DFMA)

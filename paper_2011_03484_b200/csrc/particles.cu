@@ -12,6 +12,12 @@
 // the opening half kick of step s+1 use the same acceleration: it is evaluated once and applied
 // as two half kicks, so that a chunk boundary (where the state is stored between them) leaves no
 // trace in the bits: results do not depend on K or on how advance() calls are split.
+//
+// The step loop is the same straight code for all 32 lanes, with no per-lane predicate: a lane whose
+// particle is gone runs a copy of a live lane's body (struct Lane below), and everything a removal or a
+// hard Kepler solve needs runs in two out-of-line functions entered on one warp vote each
+// (removal_at_kick, solve_and_flag).  The FP64 pipe is the roofline; what this layout saves is the
+// integer work that existed only because lanes can be dead (DESIGN.md sections 7 and 12).
 #include "glisse_internal.cuh"
 #include "kepler.cuh"
 

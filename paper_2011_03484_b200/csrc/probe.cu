@@ -1,5 +1,5 @@
 // probe.cu — (i) the FP64-FMA peak probe that gives the roofline denominator of this ALU-bound path
-// (MEASURED_PEAKS.json has no FP64 figure; DESIGN.md §6) and (ii) a test hook that evaluates the
+// (MEASURED_PEAKS.json has no FP64 figure; DESIGN.md §7) and (ii) a test hook that evaluates the
 // device primitives of kepler.cuh on arrays, so the tests can check them one by one.
 #include "glisse_internal.cuh"
 #include "kepler.cuh"
