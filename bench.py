@@ -63,13 +63,13 @@ FLOPS_PER_PLANET = 25.0
 # dram__bytes_read.sum + dram__bytes_write.sum): (flops, bytes per launch, profile it was read from).
 #   flops per thread-step = (2 DFMA + DMUL + DADD of a launch) / (grid x 32 threads x 128 steps of the launch):
 #   1m_x4 3.594e10 / (31670 x 32 x 128), c2 4.497e9 / (3961 x ...), c3 9.291e9 / (8192 x ...),
-#   c4 4.973e10 / (32492 x ...), c5 1.450e11 / (116554 x ...)
+#   c4 4.973e10 / (32492 x ...), c5 1.385e11 / (116554 x ...) (iteration binning on: the default there)
 NCU = {
     "1m_x4": (277.1, 5.51e7, "profiles/r02b_particle_kernel_1m_x4.md"),
     "c2": (277.2, 6.68e6, "profiles/r02b_particle_kernel_c2.md"),
     "c3": (276.9, 1.37e7, "profiles/r02b_particle_kernel_c3.md"),
     "c4": (373.6, 5.54e7, "profiles/r02b_particle_kernel_c4.md"),
-    "c5": (303.8, 3.37e8, "profiles/r02b_particle_kernel_c5.md"),
+    "c5": (290.2, 3.36e8, "profiles/r02b_particle_kernel_c5.md"),
 }
 # FP64 peak: ncu reports sm__sass_thread_inst_executed_op_dfma_pred_on.sum.peak_sustained = 64 per SM
 # per cycle; x 148 SMs x 2 flops x 1.965 GHz (clocks.max.sm of B200_PROFILING.md)
@@ -405,8 +405,8 @@ def run_ablations(binding, torch, device, flush):
     # config 5: resync on / off, binning on / off, after 8 warm-up chunks (about 20 % removed)
     _, c5 = make_workload("c5")
     out["config5"] = {
-        "resync_every_chunk": rate(c5, steps=4, warmup=8),
-        "resync_off": rate(c5, steps=4, warmup=8, resync_chunks=0),
+        "resync_every_chunk": rate(c5, steps=4, warmup=8, bin_iterations=0),
+        "resync_off": rate(c5, steps=4, warmup=8, resync_chunks=0, bin_iterations=0),
         "resync_every_chunk_binned": rate(c5, steps=4, warmup=8, bin_iterations=1),
     }
     # mean fast-solver iterations per warp-step with and without binning (instrumented kernel)

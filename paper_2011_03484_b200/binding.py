@@ -168,7 +168,7 @@ class GlisseSim:
 
     def __init__(self, gm_star, gm_planet, planet_pos, planet_vel, planet_rcrit, pos, vel, dt, *, r_min=0.0,
                  r_max=float("inf"), kepler_iters=5, kepler_tol=1e-14, chunk_steps=1024, resync_chunks=1,
-                 device=0, stream=None, snapshot_chunks=0, resonance_chunks=0, bin_iterations=0,
+                 device=0, stream=None, snapshot_chunks=0, resonance_chunks=0, bin_iterations=2,
                  segment_steps=None, scheme="kdk", guess_order=0):
         L = lib()
         gm_planet = np.ascontiguousarray(gm_planet, dtype=np.float64).reshape(-1)

@@ -144,6 +144,7 @@ struct glisse_sim {
   bool stats_on = false;
   bool refine = false;            // particle-kernel instantiation with the third-order Kepler starting point
   bool definition_only = false;   // ... with the definition's Kepler solver alone (kepler_iters / kepler_tol)
+  bool binning = false;           // survivors ordered by Kepler-solver hardness at every resync (bin_iterations)
   unsigned long long* d_stats = nullptr;  // [3]
 
   // snapshot staging (glisse_snapshot): a copy in original order that stream r ships to the caller
@@ -354,7 +355,7 @@ int run_compaction(glisse_sim* s) {
   c.n_out_host = s->h_nslots;
   c.block_counts = s->d_block_counts;
   c.bin = s->d_bin;
-  c.bins = s->prm.bin_iterations ? kCompactBins : 1;
+  c.bins = s->binning ? kCompactBins : 1;
   c.mu = s->gm0;
   c.dt = s->dkd ? 0.5 * s->dt : s->dt;
   c.refine = s->refine ? 1 : 0;
@@ -597,7 +598,7 @@ void glisse_default_params(glisse_params* p) {
   p->stream = nullptr;
   p->snapshot_chunks = 0;
   p->resonance_chunks = 0;
-  p->bin_iterations = 0;
+  p->bin_iterations = 2;
   p->scheme = GLISSE_SCHEME_KDK;
   p->guess_order = 0;
   p->segment_steps = 128;
@@ -644,7 +645,8 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
       prm.resync_chunks < 0 || prm.device < 0 || std::isnan(prm.r_min) || std::isnan(prm.r_max) ||
       prm.snapshot_chunks < 0 || prm.resonance_chunks < 0 || prm.segment_steps < 0 ||
       (prm.scheme != GLISSE_SCHEME_KDK && prm.scheme != GLISSE_SCHEME_DKD) ||
-      (prm.guess_order != 0 && prm.guess_order != 1 && prm.guess_order != 3))
+      (prm.guess_order != 0 && prm.guess_order != 1 && prm.guess_order != 3) || prm.bin_iterations < 0 ||
+      prm.bin_iterations > 2)
     return GLISSE_EINVAL;
 
   int ndev = 0;
@@ -864,7 +866,9 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   a.rmin2_hi = high_word(a.rmin2);
   a.rmax2_hi = high_word(a.rmax2);
   // iteration-count binning: the initial order is binned too (nothing is removed by it)
-  if (prm.bin_iterations && run_compaction(s) != GLISSE_OK) {
+  // (2 = automatic: on for the populations that were given the third-order starting point, the hard ones)
+  s->binning = prm.bin_iterations == 1 || (prm.bin_iterations == 2 && s->refine);
+  if (s->binning && run_compaction(s) != GLISSE_OK) {
     const int st = s->status;
     free_sim(s);
     return st;

@@ -59,7 +59,7 @@ def test_host_only_entry_points(libpath):
     L.glisse_default_params(ctypes.byref(p))
     assert (p.kepler_iters, p.kepler_tol, p.chunk_steps, p.resync_chunks) == (5, 1e-14, 1024, 1)
     assert (p.snapshot_chunks, p.resonance_chunks, p.bin_iterations, p.scheme, p.guess_order, p.segment_steps) == (
-        0, 0, 0, 0, 0, 128)
+        0, 0, 2, 0, 0, 128)
     assert p.r_min == 0.0 and p.r_max == float("inf")
 
 
