@@ -409,6 +409,21 @@ def run_ablations(binding, torch, device, flush):
         "resync_off": rate(c5, steps=4, warmup=8, resync_chunks=0, bin_iterations=0),
         "resync_every_chunk_binned": rate(c5, steps=4, warmup=8, bin_iterations=1),
     }
+    # a quiet population with a few planet-crossing bodies mixed in: without the ordering every warp that
+    # holds one of them pays for it at every step
+    import dataclasses
+    _, w1 = make_workload("1m_x4")
+    rng = np.random.default_rng(5)
+    pick = rng.uniform(size=w1.pos.shape[1])
+    out["mixed_population_1m_x4"] = {}
+    for frac in (0.0, 0.01, 0.03):
+        pos, vel = w1.pos.copy(), w1.vel.copy()
+        m = pick < frac
+        pos[:, m], vel[:, m] = c5.pos[:, :pos.shape[1]][:, m], c5.vel[:, :pos.shape[1]][:, m]
+        wm = dataclasses.replace(w1, pos=pos, vel=vel)
+        out["mixed_population_1m_x4"][f"{frac:.2f}"] = {
+            "particle_id_order": rate(wm, steps=4, warmup=3, bin_iterations=0)["value"],
+            "ordered_by_hardness": rate(wm, steps=4, warmup=3, bin_iterations=1)["value"]}
     # mean fast-solver iterations per warp-step with and without binning (instrumented kernel)
     for binned in (0, 1):
         sim = binding.GlisseSim.from_workload(c5, chunk_steps=CHUNK, bin_iterations=binned, device=device.index)

@@ -100,10 +100,12 @@ typedef struct {
                            number of Kepler-solver iterations their orbit can need, hardest group
                            first, particle-ID order within a group ("sort the
                            particles by the expected number of iterations ... the most eccentric
-                           group would be launched first"); 0: particle-ID order;
-                           2 (default): 1 if the population was given the third-order starting
-                           point (guess_order), else 0.  Performance only: results are
-                           bit-identical.                                                       */
+                           group would be launched first"): a few eccentric bodies then slow down
+                           a few warps instead of every warp they are scattered over; 0:
+                           particle-ID order; 2 (default): 1 if at create at least
+                           one body in a thousand has an orbit the solver finds hard, else 0.
+                           Performance only: results are bit-identical, and glisse_read returns
+                           the caller's order either way.                                       */
   int    scheme;           /* GLISSE_SCHEME_KDK (default) or GLISSE_SCHEME_DKD                          */
   int    guess_order;      /* starting point of the Kepler solve ("a judicious initial guess",
                            PAPER.md:123): 1 = dE = dM a/r for every body; 3 = the series reversion

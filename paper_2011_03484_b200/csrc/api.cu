@@ -145,6 +145,7 @@ struct glisse_sim {
   bool refine = false;            // particle-kernel instantiation with the third-order Kepler starting point
   bool definition_only = false;   // ... with the definition's Kepler solver alone (kepler_iters / kepler_tol)
   bool binning = false;           // survivors ordered by Kepler-solver hardness at every resync (bin_iterations)
+  unsigned long long hard_at_create = 0;   // bodies that wanted the third-order starting point at create
   unsigned long long* d_stats = nullptr;  // [3]
 
   // snapshot staging (glisse_snapshot): a copy in original order that stream r ships to the caller
@@ -818,7 +819,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     }
     // guess_order = 0: the Kepler starting point is chosen here, once, from the initial conditions
     // (deterministic: the same inputs always give the same instantiation, whatever K, R or the schedule)
-    if (prm.guess_order == 0) {
+    if (prm.guess_order == 0 || prm.bin_iterations == 2) {   // (the same count decides automatic binning)
       CKF(launch_count_refine(s->work[0], N, gm_star, (s->dkd ? 0.5 : 1.0) * dt, s->d_counters + 2, s->q));
       s->launches += 1;
     }
@@ -830,6 +831,7 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
       return GLISSE_EINVAL;
     }
     s->refine = prm.guess_order == 3 || (prm.guess_order == 0 && 20 * cnt[1] > static_cast<unsigned long long>(N));
+    s->hard_at_create = cnt[1];
   }
   CKF(launch_init_ids(s->id[0], s->flag[0], s->rstep[0], s->fin_flag, s->fin_rstep, static_cast<int>(N), s->q));
   s->launches += 1;
@@ -866,8 +868,9 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
   a.rmin2_hi = high_word(a.rmin2);
   a.rmax2_hi = high_word(a.rmax2);
   // iteration-count binning: the initial order is binned too (nothing is removed by it)
-  // (2 = automatic: on for the populations that were given the third-order starting point, the hard ones)
-  s->binning = prm.bin_iterations == 1 || (prm.bin_iterations == 2 && s->refine);
+  // 2 = automatic: on if at least one body in a thousand is a hard one at create (the count of bodies that
+  // want the third-order starting point), or if the population was given that starting point
+  s->binning = prm.bin_iterations == 1 || (prm.bin_iterations == 2 && (s->refine || s->hard_at_create * 1000ULL >= static_cast<unsigned long long>(N)));
   if (s->binning && run_compaction(s) != GLISSE_OK) {
     const int st = s->status;
     free_sim(s);

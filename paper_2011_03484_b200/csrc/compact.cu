@@ -27,10 +27,16 @@ constexpr unsigned kFull = 0xffffffffu;
 // Hardness bin of an orbit for the particle kernel's Kepler solver (kepler.cuh): 0 = one quartic step
 // is accepted at every phase of the orbit, 1 = some phases need more, 2 = some phase leaves the fast
 // solver (e >= 0.8, |x0| > pi/4, unbound).  The fast solver starts from x0 = dM/q, q = 1 - e cos E0,
-// and accepts once the Newton update delta = f(x0)/f'(x0) is below an eccentricity-dependent bound;
-// here delta is evaluated at 12 phases E0 of the orbit with a safety factor of 2, from the starting
-// point the run's instantiation would use (first order, or the third-order reversion where the body
-// qualifies for it: kepler.cuh).  A heuristic: it decides only which particles share a warp.
+// and accepts once the Newton update delta = f(x0)/f'(x0) is below an eccentricity-dependent bound.
+// With Kepler's equation as  q x + (es/2) x^2 + (ec/6) x^3 - (es/24) x^4 ... = dM  the update left by the
+// first-order starting point is ~ [(es/2) x0^2 + (ec/6) x0^3] / q, and by the third-order reversion
+// (where the body qualifies for it: kepler.cuh) ~ |5 b2^3 - 5 b2 b3 + b4| y^4 with b2 = es/2q, b3 = ec/6q,
+// b4 = -es/24q, y = dM/q.  First a bound: the largest these can be over the phase E0 — every e sin, e cos
+// replaced by e, every q by 1 - e — with a safety factor of 2: closed form, a few dozen operations, and it
+// clears every body of a quiet population.  A body it does not clear is then looked at phase by phase:
+// delta at 12 phases E0, from the starting point the run's instantiation would use.  The key is evaluated
+// for every survivor at every resync.  A heuristic: it decides only which particles share a warp,
+// never a result.
 __device__ int hardness_bin(double mu, double dt, bool refine, double x, double y, double z, double vx, double vy,
                             double vz) {
   const double r = sqrt(x * x + y * y + z * z);
@@ -45,17 +51,24 @@ __device__ int hardness_bin(double mu, double dt, bool refine, double x, double 
   const double kTwoPi = 6.283185307179586;
   double dM = alpha * sqrt(alpha) * dt / mu;
   dM = fabs(dM - kTwoPi * rint(dM / kTwoPi));
-  if (dM >= 0.78539816 * (1.0 - e)) return 2;
+  const double q = 1.0 - e;                       // smallest q of the orbit
+  if (dM >= 0.78539816 * q) return 2;
   const double thr = 0.5 * fmin(9e-5, 1.9e-5 * 0.64 / e2);   // kepler.cuh: fast_threshold, with the safety factor
-  double worst = 0.0;
+  const double y0 = dM / q;                       // largest starting point of the orbit
+  const double b2 = 0.5 * e / q, b3 = e / (6.0 * q), b4 = e / (24.0 * q);
+  double worst = (b2 + b3 * y0) * y0 * y0;       // first-order starting point
+  if (refine && wants_refined_guess(hi_word(e2), hi_abs(y0)))
+    worst = (5.0 * b2 * b2 * b2 + 5.0 * b2 * b3 + b4) * (y0 * y0) * (y0 * y0);
+  if (worst < thr) return 0;
+  worst = 0.0;
   for (int k = 0; k < 12; ++k) {
     double s0, c0;
     sincos(kTwoPi * k / 12.0, &s0, &c0);
-    const double q = 1.0 - e * c0, es = e * s0;
-    double x0 = dM / q;
+    const double qk = 1.0 - e * c0, es = e * s0;
+    double x0 = dM / qk;
     if (refine && wants_refined_guess(hi_word(e2), hi_abs(x0))) {
-      const double b2 = 0.5 * es / q, b3 = e * c0 / (6.0 * q);
-      x0 = x0 + x0 * x0 * (-b2 + (2.0 * b2 * b2 - b3) * x0);
+      const double c2 = 0.5 * es / qk, c3 = e * c0 / (6.0 * qk);
+      x0 = x0 + x0 * x0 * (-c2 + (2.0 * c2 * c2 - c3) * x0);
     }
     double sx, cx;
     sincos(x0, &sx, &cx);
