@@ -424,6 +424,8 @@ def run_ablations(binding, torch, device, flush):
         out["mixed_population_1m_x4"][f"{frac:.2f}"] = {
             "particle_id_order": rate(wm, steps=4, warmup=3, bin_iterations=0)["value"],
             "ordered_by_hardness": rate(wm, steps=4, warmup=3, bin_iterations=1)["value"]}
+    # the drift-kick-drift splitting (BASELINE.json's wording; two half drifts per step) against kick-drift-kick
+    out["scheme_1m_x4"] = {"kdk": rate(w1, steps=4, warmup=3)["value"], "dkd": rate(w1, steps=4, warmup=3, scheme="dkd")["value"]}
     # mean fast-solver iterations per warp-step with and without binning (instrumented kernel)
     for binned in (0, 1):
         sim = binding.GlisseSim.from_workload(c5, chunk_steps=CHUNK, bin_iterations=binned, device=device.index)
