@@ -848,6 +848,65 @@ def test_a_particle_does_not_depend_on_the_population(gl):
         assert np.array_equal(p[:, lo:lo + 1000], p2) and np.array_equal(v[:, lo:lo + 1000], v2)
 
 
+def test_random_small_systems(gl, oracle_mod, record):
+    """Differential test over 150 seeded random problems: 0 to 6 planets of random mass, spacing and
+    encounter radius, 1 to 200 particles with a from 0.5 to 63 AU and e up to 0.985 (3 % of them pushed to
+    hyperbolic speed), dt from 1 to 400 d of either sign, random r_min / r_max, both splittings, every
+    starting point, binning setting, chunk length, launch-segment length and resync interval.  Flags and
+    removal steps must equal the oracle's wherever the oracle's own 1-ulp twins agree with it, states must stay
+    within max(1e-10, 100 sigma), and the particle-step count must match whenever the flags do."""
+    G = inputs.G
+    rng = np.random.default_rng(1)
+    ang = lambda k: rng.uniform(0, 2 * np.pi, k)
+    n_mis = n_excused = n_bodies = 0
+    worst_ratio = 0.0
+    for case in range(150):
+        npl = int(rng.integers(0, 7))
+        n = int(rng.integers(1, 200))
+        pa = np.sort(rng.uniform(0.5, 30.0, npl)) * (1 + 0.4 * np.arange(npl))
+        pm = 10.0 ** rng.uniform(-7, -3, npl)
+        if npl:
+            ppos, pvel = inputs.elements_to_cartesian(G * (1 + pm), pa, rng.uniform(0, 0.1, npl), rng.uniform(0, 0.05, npl),
+                                                      ang(npl), ang(npl), ang(npl))
+            rc = inputs.hill_radius(pa, pm) * rng.uniform(0.5, 3.0)
+        else:
+            ppos, pvel, rc = np.zeros((0, 3)), np.zeros((0, 3)), np.zeros(0)
+        a = 10.0 ** rng.uniform(-0.3, 1.8, n)
+        e = np.minimum(rng.uniform(0, 1.0, n) ** rng.choice([0.5, 1, 3]), 0.985)
+        pos, vel = inputs.elements_to_cartesian(G, a, e, rng.uniform(0, 1.0, n), ang(n), ang(n), ang(n))
+        vel[rng.uniform(size=n) < 0.03] *= 1.5
+        dt = float(10.0 ** rng.uniform(0, 2.6)) * (1 if rng.uniform() < 0.8 else -1)
+        steps = int(rng.integers(1, 160))
+        w = inputs.Workload("random", G, G * pm, ppos, pvel, rc, np.ascontiguousarray(pos.T), np.ascontiguousarray(vel.T),
+                            dt, steps, float(rng.choice([0.0, 0.3, 1.0])), float(rng.choice([np.inf, 80.0, 1000.0])))
+        kw = dict(chunk_steps=int(rng.integers(1, 70)), resync_chunks=int(rng.integers(0, 3)),
+                  segment_steps=int(rng.choice([0, 3, 16, 128])), scheme=str(rng.choice(["kdk", "kdk", "dkd"])),
+                  guess_order=int(rng.choice([0, 1, 3])), bin_iterations=int(rng.choice([0, 1, 2])))
+        okw = dict(scheme=kw["scheme"])
+        (po, vo, fo, ro), ps_o = _oracle_run(oracle_mod, w, steps, **okw)
+        sigma, agree = _sensitivity(oracle_mod, w, steps, po, vo, fo, ro, **okw)
+        S = gl.GlisseSim.from_workload(w, **kw)
+        S.advance(steps)
+        p, v, f, r = S.read()
+        ps_g = S.particle_steps()
+        S.close()
+        same = (f == fo) & (r == ro)
+        n_bodies += n
+        n_mis += int((~same & agree).sum())
+        n_excused += int((~same & ~agree).sum())
+        assert (same | ~agree).all(), (case, kw, np.flatnonzero(~same & agree)[:5])
+        if same.all():
+            assert ps_g == ps_o, (case, kw)
+        ok = same & agree
+        dev = np.maximum(_dev(p, po), _dev(v, vo))
+        bound = np.maximum(TOL, TWIN_FACTOR * sigma)
+        if ok.any():
+            worst_ratio = max(worst_ratio, float((dev[ok] / bound[ok]).max()))
+            assert np.all(dev[ok] <= bound[ok]), (case, kw, float((dev[ok] / bound[ok]).max()))
+    record(dict(case="random_small_systems_150", n=n_bodies, flag_mismatches=n_mis + n_excused,
+                flag_mismatches_where_twins_agree=n_mis, max_dev_over_bound=worst_ratio))
+
+
 @pytest.mark.parametrize("e", [0.8, 0.95])
 def test_nonconvergence_flag(gl, oracle_mod, e):
     """Too few Newton updates near pericentre cannot converge: flag 3 at the oracle's step
