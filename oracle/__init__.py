@@ -51,6 +51,9 @@ def lib():
             getattr(L, name).restype = c_int
         L.oracle_planet_log.argtypes = [c_void_p, c_longlong, c_void_p]
         L.oracle_planet_log.restype = c_int
+        L.oracle_interpolate_log.argtypes = [c_int, c_void_p, c_longlong, c_void_p, c_void_p, c_void_p, c_double,
+                                             c_double, c_longlong, c_void_p]
+        L.oracle_interpolate_log.restype = c_int
         L.oracle_advance_with_log.argtypes = [c_void_p, c_longlong, c_void_p]
         L.oracle_advance_with_log.restype = c_int
         L.oracle_read.argtypes = [c_void_p, P3, P3, c_void_p, c_void_p]
@@ -226,6 +229,23 @@ def libration_summary(phi, window):
     d = dict(seen0=out[:, 0] != 0, seen180=out[:, 1] != 0, phi_min=out[:, 2], phi_max=out[:, 3],
              amp_mean=out[:, 4], amp_max=out[:, 5], n_amp=out[:, 6].astype(np.int64))
     return {k: v[0] for k, v in d.items()} if one else d
+
+
+def interpolate_log(gm_planet, sample_time, sample_pos, sample_vel, t_first, dt_record, n_records):
+    """Planet log [n_records, stride] by cubic Hermite interpolation of a sparse history:
+    sample_time [M], sample_pos / sample_vel [M, Np, 3] heliocentric."""
+    gm = _f64(gm_planet).reshape(-1)
+    npl = gm.shape[0]
+    t = _f64(sample_time).reshape(-1)
+    q = _f64(sample_pos).reshape(t.shape[0], npl, 3)
+    v = _f64(sample_vel).reshape(t.shape[0], npl, 3)
+    stride = lib().oracle_log_stride(npl)
+    out = np.zeros((int(n_records), stride), dtype=np.float64)
+    st = lib().oracle_interpolate_log(npl, _p(gm), t.shape[0], _p(t), _p(q), _p(v), float(t_first), float(dt_record),
+                                      int(n_records), _p(out))
+    if st != 0:
+        raise ValueError(f"oracle_interpolate_log refused its arguments (status {st})")
+    return out
 
 
 def kepler_drift(mu, r, v, dt, iters=5, tol=1e-14):

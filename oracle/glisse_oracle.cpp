@@ -17,7 +17,8 @@
  * high-order direct integration (T6), the paper's 5-iteration / 1e-14 claim (T7),
  * removal logic on crafted inputs (T8), osculating elements against the textbook perifocal
  * construction (T9), resonant argument against its formula and constant at exact commensurability
- * (T10), libration summary against constructed librators and hand-worked series (T11).
+ * (T10), libration summary against constructed librators and hand-worked series (T11), the interpolated
+ * planet log against exactness on cubics, the Hermite error bound on a circular orbit and h0's formula (T12).
  * Parity unpinned: none of the functions below; the
  * paper's application-level numbers (10.8 % librators …) are unpinned because the authors'
  * initial conditions are not available.
@@ -472,6 +473,49 @@ int oracle_planet_log(oracle_sim* sim, long long n_steps, double* log) {
       const int bad = planet_step(S.np, S.gm0, S.gm.data(), q.data(), qd.data(), S.dt);
       if (bad) return -4;
     }
+  }
+  return 0;
+}
+
+/* Planet log from a SPARSE history by interpolation ("these planetary positions could be
+ * supplied using any method, such as interpolation from a history file"; reading S24): the
+ * history holds n_samples instants t_m (strictly increasing) with the heliocentric positions q_j(t_m) and
+ * velocities qd_j(t_m) of the np planets, [n_samples][np][3] each.  Record r = 0 .. n_records-1 of the log
+ * is taken at t = t_first + r dt_record by cubic Hermite interpolation on the interval [t_m, t_m+1] that
+ * holds t (the last interval includes its right end), component by component:
+ *   tau = (t - t_m)/D,  D = t_m+1 - t_m
+ *   q(t) = h00 q_m + h10 D qd_m + h01 q_m+1 + h11 D qd_m+1
+ *   h00 = 2 tau^3 - 3 tau^2 + 1, h10 = tau^3 - 2 tau^2 + tau, h01 = -2 tau^3 + 3 tau^2, h11 = tau^3 - tau^2
+ * and h0 = -sum_j mu_j q_j/|q_j|^3 of the interpolated positions.  Layout of a record as in
+ * oracle_planet_log.  Returns -1 for bad arguments or a time outside the history. */
+int oracle_interpolate_log(int np, const double* gm, long long n_samples, const double* sample_time,
+                           const double* sample_pos, const double* sample_vel, double t_first, double dt_record,
+                           long long n_records, double* log) {
+  if (np < 0 || np > kMaxPlanets || n_samples < 2 || n_records < 0 || !sample_time || !log) return -1;
+  if (np > 0 && (!gm || !sample_pos || !sample_vel)) return -1;
+  for (long long m = 0; m + 1 < n_samples; ++m)
+    if (!(sample_time[m + 1] > sample_time[m])) return -1;
+  const int st = log_stride(np);
+  for (long long r = 0; r < n_records; ++r) {
+    const double t = t_first + static_cast<double>(r) * dt_record;
+    if (!(t >= sample_time[0]) || !(t <= sample_time[n_samples - 1])) return -1;
+    long long m = 0;
+    while (m + 2 < n_samples && t >= sample_time[m + 1]) ++m;
+    const double D = sample_time[m + 1] - sample_time[m];
+    const double tau = (t - sample_time[m]) / D;
+    const double tau2 = tau * tau, tau3 = tau2 * tau;
+    const double h00 = 2.0 * tau3 - 3.0 * tau2 + 1.0;
+    const double h10 = tau3 - 2.0 * tau2 + tau;
+    const double h01 = -2.0 * tau3 + 3.0 * tau2;
+    const double h11 = tau3 - tau2;
+    double* rec = log + r * st;
+    for (int i = 0; i < st; ++i) rec[i] = 0.0;
+    for (int i = 0; i < 3 * np; ++i) {
+      const double q0 = sample_pos[m * 3 * np + i], q1 = sample_pos[(m + 1) * 3 * np + i];
+      const double v0 = sample_vel[m * 3 * np + i], v1 = sample_vel[(m + 1) * 3 * np + i];
+      rec[i] = h00 * q0 + h10 * D * v0 + h01 * q1 + h11 * D * v1;
+    }
+    common_term_h0(np, gm, rec, rec + 3 * np);
   }
   return 0;
 }

@@ -623,3 +623,57 @@ def test_T11_libration_summary_on_constructed_series(oracle_mod):
     assert r["seen180"] and not r["seen0"]
     r = oracle_mod.libration_summary(np.array([2 * np.pi - 0.1]), 0.25)
     assert r["seen0"]
+
+
+# ---------------------------------------------------------------------------------------------------
+# T12  planet log interpolated from a sparse history (reading S24):
+#      exact on cubics, the Hermite error bound on a circular orbit, the samples themselves, h0's formula
+# ---------------------------------------------------------------------------------------------------
+def test_T12_interpolated_planet_log(oracle_mod):
+    rng = np.random.default_rng(12)
+    npl = 3
+    gm = np.array([3e-7, 1e-6, 2.5e-7])
+    stride = 3 * (npl + 1) + ((3 * (npl + 1)) & 1)
+
+    def h0_of(q):   # PAPER.md:111, typed out
+        return -sum(gm[j] * q[j] / np.linalg.norm(q[j]) ** 3 for j in range(npl))
+
+    # (a) cubic Hermite interpolation reproduces any cubic exactly: q_j(t) = c0 + c1 t + c2 t^2 + c3 t^3
+    c = rng.uniform(-1.0, 1.0, (4, npl, 3)) + np.array([3.0, 0.0, 0.0, 0.0])[:, None, None]
+    ts = np.array([0.0, 0.7, 1.1, 2.5, 2.9, 4.0])          # unequal spacing
+    poly = lambda t: c[0] + c[1] * t + c[2] * t ** 2 + c[3] * t ** 3
+    dpoly = lambda t: c[1] + 2 * c[2] * t + 3 * c[3] * t ** 2
+    q = np.array([poly(t) for t in ts]); v = np.array([dpoly(t) for t in ts])
+    t_first, dtr, n = 0.05, 0.0393, 100
+    log = oracle_mod.interpolate_log(gm, ts, q, v, t_first, dtr, n)
+    assert log.shape == (n, stride)
+    for r in range(n):
+        t = t_first + r * dtr
+        want = poly(t)
+        assert np.max(np.abs(log[r, :3 * npl].reshape(npl, 3) - want)) <= 2e-14 * np.max(np.abs(want))
+        assert np.allclose(log[r, 3 * npl:3 * npl + 3], h0_of(log[r, :3 * npl].reshape(npl, 3)), rtol=1e-14, atol=0)
+        assert np.all(log[r, 3 * npl + 3:] == 0.0)
+    # (b) at the sample instants it returns the samples (both ends of the history included)
+    log = oracle_mod.interpolate_log(gm, ts[[0, 3, 5]], q[[0, 3, 5]], v[[0, 3, 5]], 0.0, 2.5, 2)
+    assert np.array_equal(log[0, :3 * npl], q[0].ravel()) and np.allclose(log[1, :3 * npl], q[3].ravel(), rtol=1e-15)
+    log = oracle_mod.interpolate_log(gm, ts, q, v, 4.0, 1.0, 1)
+    assert np.allclose(log[0, :3 * npl], q[5].ravel(), rtol=1e-15)
+    # (c) a circular orbit of radius a and mean motion w sampled every D: the error of cubic Hermite
+    # interpolation is bounded by D^4 max|q''''| / 384 = a (w D)^4 / 384, and is not far below it
+    a, w = 5.2, 2 * np.pi / 4332.6
+    for D in (120.0, 240.0, 480.0):
+        ts = np.arange(0.0, 4000.0, D)
+        circ = lambda t: np.array([[a * np.cos(w * t), a * np.sin(w * t), 0.0]])
+        dcirc = lambda t: np.array([[-a * w * np.sin(w * t), a * w * np.cos(w * t), 0.0]])
+        q = np.array([circ(t) for t in ts]); v = np.array([dcirc(t) for t in ts])
+        tt = np.arange(0.0, ts[-1], 7.3)
+        log = oracle_mod.interpolate_log(gm[:1], ts, q, v, 0.0, 7.3, len(tt))
+        err = max(np.linalg.norm(log[r, :3] - circ(t)[0]) for r, t in enumerate(tt))
+        bound = a * (w * D) ** 4 / 384.0
+        assert 0.3 * bound <= err <= 1.0001 * bound * np.sqrt(2.0), (D, err, bound)   # two components, each bounded
+    # (d) refusals: a time outside the history, samples out of order
+    for bad in (dict(t_first=-0.1), dict(t_first=3999.0, n=200)):
+        with pytest.raises(ValueError):
+            oracle_mod.interpolate_log(gm[:1], ts, q, v, bad.get("t_first", 0.0), 7.3, bad.get("n", 3))
+    with pytest.raises(ValueError):
+        oracle_mod.interpolate_log(gm[:1], ts[::-1], q, v, 0.0, 7.3, 3)
