@@ -186,6 +186,24 @@ int glisse_set_planets(glisse_sim* sim, const double* planet_pos, const double* 
 int glisse_log_stride(int n_planets);
 
 /*
+ * A planet log from a SPARSE history by interpolation ("these planetary positions could
+ * be supplied using any method, such as interpolation from a history file"; reading S24).
+ * The history holds n_samples >= 2 instants sample_time[m] (strictly increasing, in the unit of dt) with
+ * the heliocentric positions sample_pos and velocities sample_vel of the sim's planets at them,
+ * [n_samples][n_planets][3] each, in the planet order of glisse_create; host or device.  Record
+ * r = 0 .. n_records-1 is taken at t_first + r dt_record by cubic Hermite interpolation of positions and
+ * velocities on the interval that holds that instant, h0 from the interpolated positions, and written to
+ * log (host or device, n_records x glisse_log_stride(n_planets) doubles, layout above) — ready for
+ * glisse_advance_with_log (kick-drift-kick: n_steps+1 records from the current time with dt_record = dt;
+ * drift-kick-drift: the same count from half a step later, the last one unused).  The simulation is not
+ * changed.
+ * GLISSE_EINVAL if the instants are not increasing or a record falls outside them.  Synchronises.
+ */
+int glisse_interpolate_log(glisse_sim* sim, long long n_samples, const double* sample_time,
+                           const double* sample_pos, const double* sample_vel, double t_first,
+                           double dt_record, long long n_records, double* log);
+
+/*
  * Write the planet log the library itself would generate for the next n_steps steps
  * (n_steps+1 records, layout above) into log (host or device) WITHOUT changing the simulation.
  * Used to check the planet-history kernel (a1) against the oracle.  Synchronises.

@@ -23,7 +23,7 @@ FLAG_ACTIVE, FLAG_RMIN, FLAG_RMAX, FLAG_NONCONV, FLAG_UNBOUND, FLAG_PLANET0 = 0,
 #: every symbol include/glisse.h declares (tests check that the library exports each one) ...
 EXPORTS = (
     "glisse_default_params", "glisse_create", "glisse_advance", "glisse_advance_with_log", "glisse_set_planets",
-    "glisse_log_stride", "glisse_planet_log", "glisse_read", "glisse_read_planets",
+    "glisse_log_stride", "glisse_planet_log", "glisse_interpolate_log", "glisse_read", "glisse_read_planets",
     "glisse_snapshot", "glisse_snapshot_wait", "glisse_snapshot_ring", "glisse_snapshots_emitted",
     "glisse_resonance_begin", "glisse_resonance_sample", "glisse_resonance_read", "glisse_libration_read",
     "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_sync", "glisse_destroy",
@@ -88,6 +88,9 @@ def lib():
         L.glisse_log_stride.restype = c_int
         L.glisse_planet_log.argtypes = [c_void_p, c_longlong, c_void_p]
         L.glisse_planet_log.restype = c_int
+        L.glisse_interpolate_log.argtypes = [c_void_p, c_longlong, c_void_p, c_void_p, c_void_p, c_double, c_double,
+                                             c_longlong, c_void_p]
+        L.glisse_interpolate_log.restype = c_int
         L.glisse_read.argtypes = [c_void_p, P3, P3, c_void_p, c_void_p]
         L.glisse_read.restype = c_int
         L.glisse_snapshot.argtypes = [c_void_p, c_int, POINTER(c_void_p), c_void_p, c_void_p]
@@ -225,6 +228,22 @@ class GlisseSim:
     def planet_log(self, n_steps):
         out = np.zeros((int(n_steps) + 1, log_stride(self.n_planets)), dtype=np.float64)
         _check(lib().glisse_planet_log(self._h, int(n_steps), _ptr(out)), "glisse_planet_log")
+        return out
+
+    def interpolate_log(self, sample_time, sample_pos, sample_vel, t_first, dt_record, n_records, out=None):
+        """Planet log [n_records, stride] interpolated from a sparse history: sample_time [M], sample_pos /
+        sample_vel [M, Np, 3] (numpy or torch CUDA float64); out: optional numpy / torch CUDA buffer."""
+        if out is None:
+            out = np.empty((int(n_records), log_stride(self.n_planets)), dtype=np.float64)
+        keep = []
+        def as_arg(t):
+            if _is_torch(t):
+                t = t.contiguous(); keep.append(t); return t
+            t = np.ascontiguousarray(t, dtype=np.float64); keep.append(t); return t
+        st, sq, sv = as_arg(sample_time), as_arg(sample_pos), as_arg(sample_vel)
+        n_samples = int(st.shape[0])
+        _check(lib().glisse_interpolate_log(self._h, n_samples, _ptr(st), _ptr(sq), _ptr(sv), float(t_first),
+                                            float(dt_record), int(n_records), _ptr(out)), "glisse_interpolate_log")
         return out
 
     def read(self, out=None):

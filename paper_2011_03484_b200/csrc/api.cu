@@ -1050,6 +1050,49 @@ int glisse_planet_log(glisse_sim* s, long long n_steps, double* log) {
   return fail < s->step + n_steps ? GLISSE_EPLANET : GLISSE_OK;   // not sticky: the sim itself is intact
 }
 
+int glisse_interpolate_log(glisse_sim* s, long long n_samples, const double* sample_time, const double* sample_pos,
+                           const double* sample_vel, double t_first, double dt_record, long long n_records,
+                           double* log) {
+  if (!s || n_samples < 2 || n_samples > (1LL << 24) || n_records < 0 || n_records > (1LL << 26) || !sample_time || !log ||
+      !std::isfinite(t_first) || !std::isfinite(dt_record))
+    return GLISSE_EINVAL;
+  const int np = s->np;
+  if (np > 0 && (!sample_pos || !sample_vel)) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (n_records == 0) return GLISSE_OK;
+  CKS(s, cudaSetDevice(s->device));
+  break_chain(s);
+  // the instants come to the host once (they may live on the device): increasing, and covering the records
+  std::vector<double> t(static_cast<size_t>(n_samples));
+  CKS(s, cudaMemcpyAsync(t.data(), sample_time, sizeof(double) * n_samples, cudaMemcpyDefault, s->q));
+  CKS(s, cudaStreamSynchronize(s->q));
+  for (long long m = 0; m + 1 < n_samples; ++m)
+    if (!(t[m + 1] > t[m])) return GLISSE_EINVAL;
+  const double t_last = t_first + static_cast<double>(n_records - 1) * dt_record;
+  if (!(std::min(t_first, t_last) >= t[0]) || !(std::max(t_first, t_last) <= t[n_samples - 1])) return GLISSE_EINVAL;
+  const size_t n_state = static_cast<size_t>(n_samples) * 3 * np;
+  const size_t count = static_cast<size_t>(n_records) * s->stride;
+  double *d_t = nullptr, *d_q = nullptr, *d_v = nullptr, *d_log = nullptr;
+  cudaError_t e = dmalloc(&d_t, static_cast<size_t>(n_samples));
+  if (e == cudaSuccess) e = dmalloc(&d_q, n_state ? n_state : 1);
+  if (e == cudaSuccess) e = dmalloc(&d_v, n_state ? n_state : 1);
+  if (e == cudaSuccess) e = dmalloc(&d_log, count);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_t, t.data(), sizeof(double) * n_samples, cudaMemcpyHostToDevice, s->q);
+  if (e == cudaSuccess && n_state) e = cudaMemcpyAsync(d_q, sample_pos, sizeof(double) * n_state, cudaMemcpyDefault, s->q);
+  if (e == cudaSuccess && n_state) e = cudaMemcpyAsync(d_v, sample_vel, sizeof(double) * n_state, cudaMemcpyDefault, s->q);
+  if (e == cudaSuccess)
+    e = launch_interpolate_log(s->d_sys, n_samples, d_t, d_q, d_v, t_first, dt_record, n_records, d_log, s->q);
+  s->launches += 1;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(log, d_log, count * sizeof(double), cudaMemcpyDefault, s->q);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->q);
+  cudaFree(d_t);
+  cudaFree(d_q);
+  cudaFree(d_v);
+  cudaFree(d_log);
+  CKS(s, e);
+  return GLISSE_OK;
+}
+
 int glisse_read(glisse_sim* s, double* const pos[3], double* const vel[3], int* flag, long long* removal_step) {
   if (!s) return GLISSE_EINVAL;
   if (s->status != GLISSE_OK) return s->status;

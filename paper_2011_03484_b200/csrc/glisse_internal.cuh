@@ -126,6 +126,11 @@ cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const d
 cudaError_t launch_planet_read(const PlanetSystem* sys, const double* jstate, double* q, double* qd,
                                cudaStream_t s);
 
+// planet log records by cubic Hermite interpolation of a sparse history (all pointers device)
+cudaError_t launch_interpolate_log(const PlanetSystem* sys, long long n_samples, const double* sample_time,
+                                   const double* sample_pos, const double* sample_vel, double t_first, double dt_record,
+                                   long long n_records, double* log, cudaStream_t s);
+
 struct CompactArgs {
   const double* src[6];
   double* dst[6];

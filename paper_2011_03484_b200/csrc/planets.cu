@@ -263,6 +263,52 @@ __global__ void __launch_bounds__(32) planet_read_kernel(const PlanetSystem* sys
   }
 }
 
+
+// Planet log from a sparse history ("interpolation from a history file"; DESIGN.md reading
+// S24): one thread per record.  The cubic that matches positions and velocities at both ends of the interval
+// [t_m, t_m+1] that holds t, in powers of tau = (t - t_m)/D:
+//   q(t) = q_m + tau { D qd_m + tau [ 3 d - D (2 qd_m + qd_m+1) + tau ( -2 d + D (qd_m + qd_m+1) ) ] },  d = q_m+1 - q_m
+// then h0 = -sum_j gm_j q_j/|q_j|^3 of the interpolated positions.  The interval is found by bisection.
+__global__ void __launch_bounds__(128) interpolate_log_kernel(const PlanetSystem* sys, long long n_samples,
+                                                              const double* __restrict__ st,
+                                                              const double* __restrict__ sq,
+                                                              const double* __restrict__ sv, double t_first,
+                                                              double dt_record, long long n_records,
+                                                              double* __restrict__ log) {
+  const long long r = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (r >= n_records) return;
+  const int np = sys->np;
+  const int stride = log_stride(np);
+  const double t = t_first + static_cast<double>(r) * dt_record;
+  long long lo = 0, hi = n_samples - 1;   // invariant: st[lo] <= t (<= st[hi]); ends with hi = lo + 1
+  while (hi - lo > 1) {
+    const long long mid = (lo + hi) >> 1;
+    if (t >= st[mid]) lo = mid; else hi = mid;
+  }
+  const double D = st[lo + 1] - st[lo];
+  const double tau = (t - st[lo]) / D;
+  double* rec = log + r * stride;
+  double hx = 0.0, hy = 0.0, hz = 0.0;
+  for (int j = 0; j < np; ++j) {
+    double q[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const long long i0 = (lo * np + j) * 3 + c, i1 = ((lo + 1) * np + j) * 3 + c;
+      const double q0 = sq[i0], d = sq[i1] - q0;
+      const double v0 = D * sv[i0], v1 = D * sv[i1];
+      const double c2 = 3.0 * d - (2.0 * v0 + v1);
+      const double c3 = (v0 + v1) - 2.0 * d;
+      q[c] = q0 + tau * (v0 + tau * (c2 + tau * c3));
+      rec[3 * j + c] = q[c];
+    }
+    const double r2 = q[0] * q[0] + q[1] * q[1] + q[2] * q[2];
+    const double w = sys->gm[j] / (r2 * sqrt(r2));
+    hx -= w * q[0]; hy -= w * q[1]; hz -= w * q[2];
+  }
+  rec[3 * np] = hx; rec[3 * np + 1] = hy; rec[3 * np + 2] = hz;
+  for (int c = 3 * np + 3; c < stride; ++c) rec[c] = 0.0;
+}
+
 }  // namespace
 
 cudaError_t launch_planet_kernel(const PlanetSystem* sys, int np, const double* jin, double* log, double* jlog,
@@ -302,6 +348,15 @@ cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const d
 cudaError_t launch_planet_read(const PlanetSystem* sys, const double* jstate, double* q, double* qd,
                                cudaStream_t s) {
   planet_read_kernel<<<1, 32, 0, s>>>(sys, jstate, q, qd);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_interpolate_log(const PlanetSystem* sys, long long n_samples, const double* sample_time,
+                                   const double* sample_pos, const double* sample_vel, double t_first, double dt_record,
+                                   long long n_records, double* log, cudaStream_t s) {
+  if (n_records <= 0) return cudaSuccess;
+  interpolate_log_kernel<<<static_cast<unsigned>((n_records + 127) / 128), 128, 0, s>>>(
+      sys, n_samples, sample_time, sample_pos, sample_vel, t_first, dt_record, n_records, log);
   return cudaGetLastError();
 }
 

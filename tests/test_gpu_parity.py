@@ -447,6 +447,56 @@ def test_external_log_is_streamed_and_the_planet_clock_can_be_reseeded(gl, oracl
         assert dev <= 1e-12     # heliocentric -> Jacobi -> heliocentric round trip of the planets
 
 
+def test_planet_log_interpolated_from_a_sparse_history(gl, oracle_mod, record):
+    """PAPER.md:109 "interpolation from a history file" (reading S24): a planet history sampled every third
+    step (positions and velocities, from the oracle's planet integration) is interpolated into a log by
+    glisse_interpolate_log — element by element against the oracle's interpolation, host and device inputs —
+    and the particles advanced with it end where the oracle's particles end with the oracle's log; both
+    splittings.  Refusals: a record outside the history, instants out of order."""
+    import torch
+    w = inputs.config(1, 700)
+    steps, every = 240, 3
+    O = oracle_mod.OracleSim.from_workload(w)
+    ts, qs, vs = [], [], []
+    for m in range(steps // every + 2):
+        q, v = O.read_planets()
+        ts.append(m * every * w.dt); qs.append(q.copy()); vs.append(v.copy())
+        O.advance(every)
+    O.close()
+    ts, qs, vs = np.array(ts), np.array(qs), np.array(vs)
+    for scheme, t_first, nrec in (("kdk", 0.0, steps + 1), ("dkd", 0.5 * w.dt, steps + 1)):
+        ref = oracle_mod.interpolate_log(w.gm_planet, ts, qs, vs, t_first, w.dt, nrec)
+        S = gl.GlisseSim.from_workload(w, chunk_steps=64, scheme=scheme)
+        log = S.interpolate_log(ts, qs, vs, t_first, w.dt, nrec)
+        dev = np.abs(log - ref).max() / np.abs(ref).max()
+        log_d = S.interpolate_log(torch.from_numpy(ts).cuda(), torch.from_numpy(qs).cuda(), torch.from_numpy(vs).cuda(),
+                                  t_first, w.dt, nrec, out=torch.empty(ref.shape, dtype=torch.float64, device="cuda"))
+        assert np.array_equal(log_d.cpu().numpy(), log)       # device inputs and output: the same bits
+        assert dev <= 1e-14, dev
+        npl = w.n_planets
+        h0 = -sum(w.gm_planet[j] * log[:, 3 * j:3 * j + 3] / np.linalg.norm(log[:, 3 * j:3 * j + 3], axis=1)[:, None] ** 3
+                  for j in range(npl))                           # PAPER.md:111, typed out
+        assert np.abs(log[:, 3 * npl:3 * npl + 3] - h0).max() <= 1e-13 * np.abs(h0).max()
+        S.advance_with_log(steps, log)
+        p, v, f, r = S.read()
+        S.close()
+        Oo = oracle_mod.OracleSim.from_workload(w, scheme=scheme)
+        Oo.advance_with_log(steps, ref)
+        po, vo, fo, ro = Oo.read()
+        Oo.close()
+        assert np.array_equal(f, fo) and np.array_equal(r, ro)
+        d = max(_dev(p, po).max(), _dev(v, vo).max())
+        record(dict(case=f"interpolated_log_{scheme}", n=w.n_particles, log_dev_max=float(dev), dev_max=float(d)))
+        assert d <= TOL, d
+    S = gl.GlisseSim.from_workload(w, chunk_steps=64)
+    for bad in (lambda: S.interpolate_log(ts, qs, vs, -1.0, w.dt, 5), lambda: S.interpolate_log(ts, qs, vs, 0.0, w.dt, 10 ** 6),
+                lambda: S.interpolate_log(ts[::-1].copy(), qs, vs, 0.0, w.dt, 5)):
+        with pytest.raises(gl.GlisseError):
+            bad()
+    S.advance(10)     # refused arguments leave the simulation usable
+    S.close()
+
+
 def test_periodic_output_ring(gl):
     """params.snapshot_chunks ("copied back to the CPU after a user-configurable number of
     planetary chunk calculations"): ONE glisse_advance of 10 chunks emits a snapshot every 2 chunks
