@@ -23,9 +23,10 @@
  *  - Ownership: inputs are copied during glisse_create (the caller keeps its buffers); outputs
  *    are caller-allocated.  The library owns its internal device state until glisse_destroy.
  *  - Threading: a glisse_sim must be used by one host thread at a time; different sims may be used
- *    from different threads.  Process-wide state is limited to two caches behind one mutex: a
- *    stream-ordered memory pool per device (a sim's arena comes from it and goes back to it) and
- *    one pinned page of mailbox words for survivor counts.
+ *    from different threads.  Process-wide state is limited to three caches behind one mutex: a
+ *    stream-ordered memory pool per device (a sim's arena comes from it and goes back to it), up to
+ *    eight idle streams of each priority per device (a sim's streams come from them and go back,
+ *    synchronised, at glisse_destroy) and one pinned page of mailbox words for survivor counts.
  *  - Measurement and test hooks (launch counter, kernel timer, FP64 probe, primitive evaluator,
  *    solver statistics) are NOT part of this interface: include/glisse_test.h.
  */
