@@ -765,10 +765,10 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     need(&s->d_nslots, 2);
     need(&s->d_block_counts, static_cast<size_t>(kCompactBins) * ((N + 255) / 256 + 1) + 1);
     need(&s->d_bin, N);
-    need(&s->d_counters, 3);
-    need(&s->d_ticket, 2);
+    need(&s->d_counters, 3);   // d_counters, d_error, d_stats: consecutive, cleared by ONE memset at create
     need(&s->d_error, 1);
     need(&s->d_stats, 3);
+    need(&s->d_ticket, 2);
     need(&s->d_ring_steps, kRingStepWords);
     need(&s->d_fail, 2);
     need(&s->d_sys, 1);
@@ -845,20 +845,16 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     CKF(cudaMemcpyAsync(s->work[0][k], pos[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
     CKF(cudaMemcpyAsync(s->work[0][3 + k], vel[k], sizeof(double) * N, cudaMemcpyDefault, s->q));
   }
-  CKF(cudaMemsetAsync(s->d_counters, 0, 3 * sizeof(unsigned long long), s->q));
-  CKF(cudaMemsetAsync(s->d_error, 0, sizeof(int), s->q));
-  CKF(cudaMemsetAsync(s->d_stats, 0, 3 * sizeof(unsigned long long), s->q));
+  CKF(cudaMemsetAsync(s->d_counters, 0,
+                      reinterpret_cast<char*>(s->d_stats + 3) - reinterpret_cast<char*>(s->d_counters), s->q));
   {
-    for (int k = 0; k < 6; ++k) {
-      CKF(launch_count_nonfinite(s->work[0][k], N, s->d_counters + 1, s->q));
-      s->launches += 1;
-    }
-    // guess_order = 0: the Kepler starting point is chosen here, once, from the initial conditions
-    // (deterministic: the same inputs always give the same instantiation, whatever K, R or the schedule)
-    if (prm.guess_order == 0 || prm.bin_iterations == 2) {   // (the same count decides automatic binning)
-      CKF(launch_count_refine(s->work[0], N, gm_star, (s->dkd ? 0.5 : 1.0) * dt, s->d_counters + 2, s->q));
-      s->launches += 1;
-    }
+    // One pass: identity order and cleared flags, the count of non-finite inputs, and the count of bodies that
+    // want the third-order Kepler starting point.  guess_order = 0: the starting point is chosen here, once,
+    // from the initial conditions (deterministic: the same inputs always give the same instantiation, whatever
+    // K, R or the schedule); the same count decides automatic binning.
+    CKF(launch_create_pass(s->work[0], N, gm_star, (s->dkd ? 0.5 : 1.0) * dt, s->d_counters + 1, s->id[0], s->flag[0],
+                           s->rstep[0], s->fin_flag, s->fin_rstep, s->q));
+    s->launches += 1;
     unsigned long long cnt[2] = {0, 0};   // non-finite inputs, bodies wanting the third-order starting point
     CKF(cudaMemcpyAsync(cnt, s->d_counters + 1, sizeof(cnt), cudaMemcpyDeviceToHost, s->q));
     CKF(cudaStreamSynchronize(s->q));
@@ -869,8 +865,6 @@ int glisse_create(glisse_sim** out, double gm_star, int n_planets, const double*
     s->refine = prm.guess_order == 3 || (prm.guess_order == 0 && 20 * cnt[1] > static_cast<unsigned long long>(N));
     s->hard_at_create = cnt[1];
   }
-  CKF(launch_init_ids(s->id[0], s->flag[0], s->rstep[0], s->fin_flag, s->fin_rstep, static_cast<int>(N), s->q));
-  s->launches += 1;
   const int nsl[2] = {static_cast<int>(N), 0};
   CKF(cudaMemcpyAsync(s->d_nslots, nsl, sizeof(nsl), cudaMemcpyHostToDevice, s->q));
   s->nslots_upper = static_cast<int>(N);

@@ -205,27 +205,6 @@ __global__ void __launch_bounds__(kBlock) count_active_kernel(const int* __restr
   if (threadIdx.x == 0 && c) atomicAdd(out, static_cast<unsigned long long>(c));
 }
 
-__global__ void __launch_bounds__(kBlock) init_ids_kernel(int* id, int* flag, long long* rstep, int* fin_flag,
-                                                           long long* fin_rstep, int n) {
-  const int i = blockIdx.x * kBlock + threadIdx.x;
-  if (i >= n) return;
-  id[i] = i;
-  flag[i] = 0;
-  rstep[i] = -1;
-  fin_flag[i] = 0;
-  fin_rstep[i] = -1;
-}
-
-__global__ void __launch_bounds__(kBlock) count_nonfinite_kernel(const double* __restrict__ p, long long n,
-                                                                  unsigned long long* __restrict__ out) {
-  long long bad = 0;
-  for (long long i = static_cast<long long>(blockIdx.x) * kBlock + threadIdx.x; i < n;
-       i += static_cast<long long>(gridDim.x) * kBlock)
-    bad += !isfinite(p[i]);
-  const int c = __syncthreads_count(bad != 0);
-  if (threadIdx.x == 0 && c) atomicAdd(out, static_cast<unsigned long long>(c));
-}
-
 }  // namespace
 
 cudaError_t launch_compaction(const CompactArgs& a, int n_slots_upper, cudaStream_t s, long long* launches) {
@@ -248,20 +227,6 @@ cudaError_t launch_count_active(const int* flag, const int* n_slots, int n_slots
                                 cudaStream_t s) {
   if (n_slots_upper < 1) n_slots_upper = 1;
   count_active_kernel<<<(n_slots_upper + kBlock - 1) / kBlock, kBlock, 0, s>>>(flag, n_slots, out);
-  return cudaGetLastError();
-}
-
-cudaError_t launch_init_ids(int* id, int* flag, long long* rstep, int* fin_flag, long long* fin_rstep, int n,
-                            cudaStream_t s) {
-  init_ids_kernel<<<(n + kBlock - 1) / kBlock, kBlock, 0, s>>>(id, flag, rstep, fin_flag, fin_rstep, n);
-  return cudaGetLastError();
-}
-
-cudaError_t launch_count_nonfinite(const double* p, long long n, unsigned long long* out, cudaStream_t s) {
-  long long nb = (n + kBlock - 1) / kBlock;
-  if (nb > 148 * 16) nb = 148 * 16;
-  if (nb < 1) nb = 1;
-  count_nonfinite_kernel<<<static_cast<int>(nb), kBlock, 0, s>>>(p, n, out);
   return cudaGetLastError();
 }
 

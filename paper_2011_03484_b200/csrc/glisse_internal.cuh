@@ -101,9 +101,12 @@ inline int jstate_stride(int np) { return 6 * np; }
 // definition_only: the instantiation without the fast solver (see fast_solver_allowed)
 cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool chained, bool stats, bool dkd, bool refine,
                                    bool definition_only, cudaStream_t s);
-// *out += number of the n bodies that would take the third-order starting point at this instant
-cudaError_t launch_count_refine(const double* const st[6], long long n, double mu, double dt, unsigned long long* out,
-                                cudaStream_t s);
+// the one pass over the particles at create: identity order, cleared flags and removal steps (working and
+// original order); counts[0] += non-finite bodies, counts[1] += bodies that would take the third-order
+// starting point at this instant
+cudaError_t launch_create_pass(const double* const st[6], long long n, double mu, double dt, unsigned long long* counts,
+                               int* id, int* flag, long long* rstep, int* fin_flag, long long* fin_rstep,
+                               cudaStream_t s);
 cudaError_t configure_particle_kernels();
 // whether kepler_iters / kepler_tol admit the fast solver (kepler.cuh: kFastMinIters, kFastMinTol); if not,
 // the simulation uses the particle-kernel instantiation that carries the definition's solver alone
@@ -163,9 +166,6 @@ struct ScatterArgs {
 cudaError_t launch_scatter_to_original(const ScatterArgs& a, int n_slots_upper, cudaStream_t s);
 cudaError_t launch_count_active(const int* flag, const int* n_slots, int n_slots_upper,
                                 unsigned long long* out, cudaStream_t s);
-cudaError_t launch_init_ids(int* id, int* flag, long long* rstep, int* fin_flag, long long* fin_rstep, int n,
-                            cudaStream_t s);
-cudaError_t launch_count_nonfinite(const double* p, long long n, unsigned long long* out, cudaStream_t s);
 
 // snapshot.cu: ONE pass over the original-order arrays that serves the snapshot (staging copy,
 // Cartesian or osculating elements) and the resonant-argument reduction of the same instant: the

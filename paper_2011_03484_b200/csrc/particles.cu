@@ -551,15 +551,24 @@ size_t particle_smem_bytes(const ParticleArgs& a) {
          static_cast<size_t>(kParticleWarps) * kRingSlots * 8;
 }
 
-// Bodies that would take the third-order starting point at this instant (guess_order = 0 chooses the
-// instantiation from their share at create).  Plain arithmetic: off the hot path.
-__global__ void __launch_bounds__(256) count_refine_kernel(const double* x, const double* y, const double* z,
-                                                            const double* vx, const double* vy, const double* vz,
-                                                            long long n, double mu, double dt,
-                                                            unsigned long long* out) {
+// The one pass over the particles at create: identity order, flags and removal steps (working and original
+// order), the count of non-finite inputs (counts[0]: create refuses them), and the count of bodies that would
+// take the third-order starting point at this instant (counts[1]: guess_order = 0 chooses the instantiation
+// from their share, bin_iterations = 2 the binning).  Plain arithmetic: off the hot path.
+__global__ void __launch_bounds__(256) create_pass_kernel(const double* x, const double* y, const double* z,
+                                                           const double* vx, const double* vy, const double* vz,
+                                                           long long n, double mu, double dt,
+                                                           unsigned long long* counts, int* id, int* flag,
+                                                           long long* rstep, int* fin_flag, long long* fin_rstep) {
   const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
-  bool want = false;
+  bool want = false, bad = false;
   if (i < n) {
+    id[i] = static_cast<int>(i);
+    flag[i] = 0;
+    rstep[i] = -1;
+    fin_flag[i] = 0;
+    fin_rstep[i] = -1;
+    bad = !isfinite(x[i]) | !isfinite(y[i]) | !isfinite(z[i]) | !isfinite(vx[i]) | !isfinite(vy[i]) | !isfinite(vz[i]);
     const double r0 = sqrt(x[i] * x[i] + y[i] * y[i] + z[i] * z[i]);
     const double v2 = vx[i] * vx[i] + vy[i] * vy[i] + vz[i] * vz[i];
     const double u = x[i] * vx[i] + y[i] * vy[i] + z[i] * vz[i];
@@ -573,8 +582,10 @@ __global__ void __launch_bounds__(256) count_refine_kernel(const double* x, cons
       want = hi_word(e2) < kHiE2_080 && is_small_angle(xk) && wants_refined_guess(hi_word(e2), hi_abs(xk));
     }
   }
-  const int c = __syncthreads_count(want);
-  if (threadIdx.x == 0 && c) atomicAdd(out, static_cast<unsigned long long>(c));
+  const int cb = __syncthreads_count(bad);
+  const int cw = __syncthreads_count(want);
+  if (threadIdx.x == 0 && cb) atomicAdd(counts, static_cast<unsigned long long>(cb));
+  if (threadIdx.x == 0 && cw) atomicAdd(counts + 1, static_cast<unsigned long long>(cw));
 }
 
 template <int NP, bool STATS, bool DKD, int SOLVER>
@@ -650,9 +661,11 @@ cudaError_t launch_particle_kernel(const ParticleArgs& a, int n_groups, bool cha
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-cudaError_t launch_count_refine(const double* const st[6], long long n, double mu, double dt, unsigned long long* out,
-                                cudaStream_t s) {
-  count_refine_kernel<<<static_cast<int>((n + 255) / 256), 256, 0, s>>>(st[0], st[1], st[2], st[3], st[4], st[5], n, mu, dt, out);
+cudaError_t launch_create_pass(const double* const st[6], long long n, double mu, double dt, unsigned long long* counts,
+                               int* id, int* flag, long long* rstep, int* fin_flag, long long* fin_rstep,
+                               cudaStream_t s) {
+  create_pass_kernel<<<static_cast<int>((n + 255) / 256), 256, 0, s>>>(st[0], st[1], st[2], st[3], st[4], st[5], n, mu, dt,
+                                                                        counts, id, flag, rstep, fin_flag, fin_rstep);
   return cudaGetLastError();
 }
 
