@@ -428,13 +428,15 @@ struct DriftVars {
   double rinv, sqa, rsa, q, ec, es, dM, a, invq, e2;
 };
 
+// rinv = rsqrt_f64(r2): a caller whose positions are known long before its velocities (the planet-history
+// kernel: the kick changes the velocities only) takes it off the dependent chain by computing it early
 template <bool REFINE>
-__device__ __forceinline__ void drift_begin(double mu, double two_mu, double inv_mu, double inv_mu_dt, double r2,
-                                            double x, double y, double z, double vx, double vy, double vz,
-                                            DriftVars& k, double& xk, bool& unbound) {
+__device__ __forceinline__ void drift_begin_rinv(double mu, double two_mu, double inv_mu, double inv_mu_dt, double r2,
+                                                 double rinv, double x, double y, double z, double vx, double vy,
+                                                 double vz, DriftVars& k, double& xk, bool& unbound) {
   const double v2 = fma(vx, vx, fma(vy, vy, vz * vz));
   const double u = fma(x, vx, fma(y, vy, z * vz));
-  k.rinv = rsqrt_f64(r2);
+  k.rinv = rinv;
   const double r0 = r2 * k.rinv;
   const double al = fma(two_mu, k.rinv, -v2);  // mu / a
   unbound = !(hi_word(al) > 0);                 // alpha <= 0 (or below 2^-1042: no such orbit), or NaN
@@ -463,6 +465,13 @@ __device__ __forceinline__ void drift_begin(double mu, double two_mu, double inv
       xk = fma(yy * yy, fma(c3, yy, -b2), yy);
     }
   }
+}
+
+template <bool REFINE>
+__device__ __forceinline__ void drift_begin(double mu, double two_mu, double inv_mu, double inv_mu_dt, double r2,
+                                            double x, double y, double z, double vx, double vy, double vz,
+                                            DriftVars& k, double& xk, bool& unbound) {
+  drift_begin_rinv<REFINE>(mu, two_mu, inv_mu, inv_mu_dt, r2, rsqrt_f64(r2), x, y, z, vx, vy, vz, k, xk, unbound);
 }
 
 // reading S9 for a body whose step spans half a revolution or more (drift_begin)

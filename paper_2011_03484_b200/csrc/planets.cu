@@ -48,6 +48,16 @@ __device__ __forceinline__ int partner(const Lane& L, int jj) {
   return j >= np ? j - np : j;   // lanes >= np (idle) read some live lane; their results are discarded
 }
 
+// s += take ? t : 0, the one-sided sums of the Jacobi maps.  Up to four planets the condition (a function of
+// lane and round only) is kept as a weight 1.0 / 0.0 in a register over the step loop and the sum is ONE fma:
+// fma(1, t, s) = t + s and fma(0, t, s) = s to the bit (36 selects fewer per step at N_p = 4; measured slower
+// from N_p = 8 on, where the weights no longer fit the registers).
+template <int NP>
+__device__ __forceinline__ void add_if(bool take, double t, double& s) {
+  if constexpr (NP > 0 && NP <= 4) s = fma(take ? 1.0 : 0.0, t, s);
+  else s += take ? t : 0.0;
+}
+
 // q from r' (Jacobi -> heliocentric): q_k = r'_k + sum_{i<k} (gm_i/eta_i) r'_i; the same linear map
 // serves velocities
 template <int NP>
@@ -60,8 +70,7 @@ __device__ __forceinline__ void jacobi_to_helio(const Lane& L, double rx, double
   for (int jj = 0; jj + 1 < np; ++jj) {
     const int j = partner<NP>(L, jj);
     const double tx = shfl(cx, j), ty = shfl(cy, j), tz = shfl(cz, j);
-    const bool below = j < L.lane;
-    sx += below ? tx : 0.0; sy += below ? ty : 0.0; sz += below ? tz : 0.0;
+    add_if<NP>(j < L.lane, tx, sx); add_if<NP>(j < L.lane, ty, sy); add_if<NP>(j < L.lane, tz, sz);
   }
   qx = rx + sx; qy = ry + sy; qz = rz + sz;
 }
@@ -77,8 +86,7 @@ __device__ __forceinline__ void helio_to_jacobi(const Lane& L, double qx, double
   for (int jj = 0; jj + 1 < np; ++jj) {
     const int j = partner<NP>(L, jj);
     const double tx = shfl(cx, j), ty = shfl(cy, j), tz = shfl(cz, j);
-    const bool below = j < L.lane;
-    sx += below ? tx : 0.0; sy += below ? ty : 0.0; sz += below ? tz : 0.0;
+    add_if<NP>(j < L.lane, tx, sx); add_if<NP>(j < L.lane, ty, sy); add_if<NP>(j < L.lane, tz, sz);
   }
   rx = qx - sx * L.inv_eta_prev; ry = qy - sy * L.inv_eta_prev; rz = qz - sz * L.inv_eta_prev;
 }
@@ -86,8 +94,8 @@ __device__ __forceinline__ void helio_to_jacobi(const Lane& L, double qx, double
 // Jacobi acceleration of this lane's planet, and h0 (valid on lane 0, which writes it)
 template <int NP>
 __device__ __forceinline__ void kick_accel(const Lane& L, double qx, double qy, double qz, double rx, double ry,
-                                           double rz, double& ax, double& ay, double& az, double& hx, double& hy,
-                                           double& hz) {
+                                           double rz, double r2, double& ax, double& ay, double& az, double& hx,
+                                           double& hy, double& hz) {
   const int np = count<NP>(L);
   // star term of A_i and this planet's contribution to h0
   const double q2 = fma(qx, qx, fma(qy, qy, qz * qz));
@@ -95,8 +103,7 @@ __device__ __forceinline__ void kick_accel(const Lane& L, double qx, double qy, 
   double Ax = -(L.gm0 * qi3) * qx, Ay = -(L.gm0 * qi3) * qy, Az = -(L.gm0 * qi3) * qz;
   const double tx = (L.gm * qi3) * qx, ty = (L.gm * qi3) * qy, tz = (L.gm * qi3) * qz;
   // the Jacobi two-body term, independent of the sums below
-  const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
-  const double w0 = gm_over_r3(L.gm0, r2);
+  const double w0 = gm_over_r3(L.gm0, r2);   // r2 = |r'|^2
   hx = -tx; hy = -ty; hz = -tz;   // lane 0: t_0, then t_1, t_2, ... in the rounds below
 #pragma unroll
   for (int jj = 0; jj + 1 < np; ++jj) {
@@ -116,8 +123,7 @@ __device__ __forceinline__ void kick_accel(const Lane& L, double qx, double qy, 
   for (int jj = 0; jj + 1 < np; ++jj) {
     const int j = partner<NP>(L, jj);
     const double ux = shfl(mx, j), uy = shfl(my, j), uz = shfl(mz, j);
-    const bool above = j > L.lane;
-    Tx += above ? ux : 0.0; Ty += above ? uy : 0.0; Tz += above ? uz : 0.0;
+    add_if<NP>(j > L.lane, ux, Tx); add_if<NP>(j > L.lane, uy, Ty); add_if<NP>(j > L.lane, uz, Tz);
   }
   // idle lanes get a zero kick: their stand-in orbit stays the circle it started as
   const double sc = L.live ? L.sc : 0.0;
@@ -144,19 +150,21 @@ __device__ __forceinline__ Lane make_lane(const PlanetSystem* sys) {
   return L;
 }
 
+template <int NP>
 __device__ __forceinline__ void write_record(const Lane& L, double* log, double* jlog, int rec, int stride,
                                              double qx, double qy, double qz, double hx, double hy, double hz,
                                              double rx, double ry, double rz, double vx, double vy, double vz) {
+  const int np = count<NP>(L);
   double* r = log + static_cast<size_t>(rec) * stride;
   if (L.live) {
     r[3 * L.lane] = qx; r[3 * L.lane + 1] = qy; r[3 * L.lane + 2] = qz;
-    double* js = jlog + static_cast<size_t>(rec) * 6 * L.np;
+    double* js = jlog + static_cast<size_t>(rec) * 6 * np;
     js[3 * L.lane] = rx; js[3 * L.lane + 1] = ry; js[3 * L.lane + 2] = rz;
-    js[3 * L.np + 3 * L.lane] = vx; js[3 * L.np + 3 * L.lane + 1] = vy; js[3 * L.np + 3 * L.lane + 2] = vz;
+    js[3 * np + 3 * L.lane] = vx; js[3 * np + 3 * L.lane + 1] = vy; js[3 * np + 3 * L.lane + 2] = vz;
   }
   if (L.lane == 0) {
-    r[3 * L.np] = hx; r[3 * L.np + 1] = hy; r[3 * L.np + 2] = hz;
-    for (int c = 3 * L.np + 3; c < stride; ++c) r[c] = 0.0;
+    r[3 * np] = hx; r[3 * np + 1] = hy; r[3 * np + 2] = hz;
+    if ((3 * np + 3) & 1) r[3 * np + 3] = 0.0;   // the one padding word of an odd record (log_stride)
   }
 }
 
@@ -166,7 +174,7 @@ __global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* 
                                                              int nsteps, double dt, long long step0,
                                                              long long* fail_step) {
   const Lane L = make_lane(sys);
-  const int stride = log_stride(L.np);
+  const int stride = log_stride(count<NP>(L));
   const double hdt = 0.5 * dt;
   const double inv_mu_dt = L.inv_mu * dt;
   const double two_mu = 2.0 * L.mu;
@@ -186,13 +194,16 @@ __global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* 
     vx = jin[3 * L.np + 3 * L.lane]; vy = jin[3 * L.np + 3 * L.lane + 1]; vz = jin[3 * L.np + 3 * L.lane + 2];
   }
   double qx, qy, qz, ax, ay, az, hx, hy, hz;
+  // |r'|^2 and its inverse root for the NEXT drift: the kick leaves the positions alone, so both are known
+  // as soon as the drift ends and are computed beside the kick, off the dependent chain of the step
+  double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
+  double rinv = rsqrt_f64(r2);
   jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
-  kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
-  write_record(L, log, jlog, 0, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
+  kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, r2, ax, ay, az, hx, hy, hz);
+  write_record<NP>(L, log, jlog, 0, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
   int bad = -1;   // first step (within this launch) whose drift failed
   for (int s = 0; s < nsteps; ++s) {
     vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
-    const double r2 = fma(rx, rx, fma(ry, ry, rz * rz));
     // third-order starting point (kepler.cuh): Jupiter at dt = 180 d needs one quartic step instead of two
     // The drift in the particle kernel's three pieces (kepler.cuh), with no per-lane predicate: begin, ONE
     // fast-solver step, finish.  If any lane (planet or stand-in) is not served by that — not accepted, e >= 0.8,
@@ -204,7 +215,7 @@ __global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* 
       DriftVars dv;
       double xk, xn, sm, cm1, dl;
       bool unbound;
-      drift_begin<true>(L.mu, two_mu, L.inv_mu, inv_mu_dt, r2, rx, ry, rz, vx, vy, vz, dv, xk, unbound);
+      drift_begin_rinv<true>(L.mu, two_mu, L.inv_mu, inv_mu_dt, r2, rinv, rx, ry, rz, vx, vy, vz, dv, xk, unbound);
       const int e2h = hi_word(dv.e2);
       const int thr = e2h < kHiE2_010 ? kHiThr0 : (e2h < kHiE2_030 ? kHiThr1 : (e2h < kHiE2_050 ? kHiThr2 : kHiThr3));
       const bool hard = !(e2h < kHiE2_080) | !is_small_angle(xk) | !(hi_abs(dv.dM) < kHiPi);
@@ -218,10 +229,12 @@ __global__ void __launch_bounds__(32) planet_history_kernel(const PlanetSystem* 
     }
     const unsigned failed = __ballot_sync(kFullMask, st != 0 && L.live);
     if (failed && bad < 0) bad = s;
+    r2 = fma(rx, rx, fma(ry, ry, rz * rz));
+    rinv = rsqrt_f64(r2);
     jacobi_to_helio<NP>(L, rx, ry, rz, qx, qy, qz);
-    kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, ax, ay, az, hx, hy, hz);
+    kick_accel<NP>(L, qx, qy, qz, rx, ry, rz, r2, ax, ay, az, hx, hy, hz);
     vx = fma(ax, hdt, vx); vy = fma(ay, hdt, vy); vz = fma(az, hdt, vz);
-    write_record(L, log, jlog, s + 1, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
+    write_record<NP>(L, log, jlog, s + 1, stride, qx, qy, qz, hx, hy, hz, rx, ry, rz, vx, vy, vz);
   }
   // records up to and including step0 + bad are valid (glisse_internal.cuh: kNoPlanetFailure)
   if (bad >= 0 && L.lane == 0) atomicMin(fail_step, step0 + bad);
