@@ -413,11 +413,15 @@ int run_compaction(glisse_sim* s) {
 // (re-)seeded is cut into pieces of 64, 64, 128, 256, ... steps (summing to K): the planet-history
 // kernel is serial in time, so a full first chunk would keep the particles waiting for K x 1 us before
 // their first step; after the ramp the planets stay one buffer ahead.  Results do not depend on the
-// cut.
+// cut.  From kNoRampParticles particles on the first chunk is NOT cut: the pieces are
+// separate launch chains (an event wait between two launches ends the programmatic chaining), each with
+// a tail of its own that costs more than one wave of particles waiting once — 1.0 ms of the first
+// chunk at 2^20 particles, where the upload alone outlasts the planet kernel's K steps.
+constexpr long long kNoRampParticles = 1LL << 18;
 int buffer_len(const glisse_sim* s, long long start) {
   const int K = s->K;
   const long long rel = start - s->origin;
-  if (K < 256 || rel >= K) return K;
+  if (K < 256 || rel >= K || s->n >= kNoRampParticles) return K;
   if (rel == 0) return 64;
   return static_cast<int>(std::min<long long>(rel, K - rel));
 }
