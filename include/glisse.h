@@ -326,6 +326,29 @@ int glisse_sync(glisse_sim* sim);
 
 void glisse_destroy(glisse_sim* sim);
 
+/*
+ * One-shot run: glisse_create + glisse_advance(n_steps) + glisse_read + glisse_destroy over caller arrays
+ * (host or device; pinned host arrays for the copies to overlap), PIPELINED over n_parts contiguous slices
+ * of the particles.  Test particles never interact and the paper's own scaling strategy is
+ * particles partitioned, planets replicated; here the partition is over time slots of one
+ * GPU: each part is a simulation of its own (own planet-history kernel, same planets), part i+1 is
+ * uploaded and part i read back while the kernels of the other parts run, so all but about one part's
+ * share of the host<->device copies hides behind the integration.
+ *   n_parts: 1 .. 64, or 0 = automatic (parts of about 2^17 particles, at most 8; one part below 2^18).
+ *            Cuts fall on multiples of 256 particles.
+ *   out_pos / out_vel / flag / removal_step: as glisse_read (each may be NULL), original particle order.
+ *   particle_steps: if not NULL, receives the particle-steps integrated (sum over the parts).
+ * The result of every particle is what a single simulation over all of them returns, bit for bit, when
+ * params fixes guess_order (1 or 3); with guess_order = 0 each part chooses its Kepler starting point from
+ * its own particles, as every rank of a multi-GPU run does (a roundoff-level difference).  Arguments and
+ * statuses otherwise as glisse_create.  Synchronous.
+ */
+int glisse_run(double gm_star, int n_planets, const double* gm_planet, const double* planet_pos,
+               const double* planet_vel, const double* planet_rcrit, long long n_particles,
+               const double* const pos[3], const double* const vel[3], double dt, const glisse_params* params,
+               long long n_steps, int n_parts, double* const out_pos[3], double* const out_vel[3], int* flag,
+               long long* removal_step, long long* particle_steps);
+
 /* Static string for a status code. */
 const char* glisse_strerror(int status);
 

@@ -26,7 +26,7 @@ EXPORTS = (
     "glisse_log_stride", "glisse_planet_log", "glisse_interpolate_log", "glisse_read", "glisse_read_planets",
     "glisse_snapshot", "glisse_snapshot_wait", "glisse_snapshot_ring", "glisse_snapshots_emitted",
     "glisse_resonance_begin", "glisse_resonance_sample", "glisse_resonance_read", "glisse_libration_read",
-    "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_sync", "glisse_destroy",
+    "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_sync", "glisse_destroy", "glisse_run",
     "glisse_strerror",
 )
 #: ... and the measurement / test hooks of include/glisse_test.h
@@ -118,6 +118,10 @@ def lib():
         L.glisse_test_primitive.restype = c_int
         L.glisse_destroy.argtypes = [c_void_p]
         L.glisse_destroy.restype = None
+        L.glisse_run.argtypes = [c_double, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_longlong, P3, P3, c_double,
+                                 POINTER(GlisseParams), c_longlong, c_int, P3, P3, c_void_p, c_void_p,
+                                 POINTER(c_longlong)]
+        L.glisse_run.restype = c_int
         L.glisse_strerror.argtypes = [c_int]
         L.glisse_strerror.restype = ctypes.c_char_p
         _lib = L
@@ -166,6 +170,55 @@ def _p3(rows):
     return (c_void_p * 3)(*[(r.data_ptr() if _is_torch(r) else r.ctypes.data) for r in rows])
 
 
+def _params(*, r_min=0.0, r_max=float("inf"), kepler_iters=5, kepler_tol=1e-14, chunk_steps=1024, resync_chunks=1,
+            device=0, stream=None, snapshot_chunks=0, resonance_chunks=0, bin_iterations=2, segment_steps=None,
+            scheme="kdk", guess_order=0):
+    """glisse_params from keywords (defaults = glisse_default_params)."""
+    prm = GlisseParams()
+    lib().glisse_default_params(byref(prm))
+    prm.r_min, prm.r_max = float(r_min), float(r_max)
+    prm.kepler_iters, prm.kepler_tol = int(kepler_iters), float(kepler_tol)
+    prm.chunk_steps, prm.resync_chunks = int(chunk_steps), int(resync_chunks)
+    prm.device = int(device)
+    prm.stream = None if stream is None else c_void_p(int(stream))
+    prm.snapshot_chunks, prm.resonance_chunks = int(snapshot_chunks), int(resonance_chunks)
+    prm.bin_iterations = int(bin_iterations)
+    prm.scheme = {"kdk": 0, "dkd": 1}[scheme]
+    prm.guess_order = int(guess_order)
+    if segment_steps is not None:
+        prm.segment_steps = int(segment_steps)
+    return prm
+
+
+def run(w, n_steps, n_parts=0, out=None, **kw):
+    """glisse_run on a workload (inputs.Workload fields): create + advance(n_steps) + read + destroy, pipelined
+    over n_parts slices of the particles (0 = automatic).  w.pos / w.vel: [3, N] numpy arrays (pinned for the
+    copies to overlap) or torch CUDA tensors; out = (pos[3,N], vel[3,N], flag[N] int32, removal_step[N] int64)
+    or None (allocated, pageable).  Returns (pos, vel, flag, removal_step, particle_steps)."""
+    kw.setdefault("chunk_steps", w.chunk_steps)
+    prm = _params(r_min=w.r_min, r_max=w.r_max, **kw)
+    gm_planet = np.ascontiguousarray(w.gm_planet, dtype=np.float64).reshape(-1)
+    npl = int(gm_planet.shape[0])
+    ppos = np.ascontiguousarray(w.planet_pos, dtype=np.float64).reshape(npl, 3)
+    pvel = np.ascontiguousarray(w.planet_vel, dtype=np.float64).reshape(npl, 3)
+    rcrit = None if w.planet_rcrit is None else np.ascontiguousarray(w.planet_rcrit, dtype=np.float64).reshape(npl)
+    keep_p, prow = _rows(w.pos, 3)
+    keep_v, vrow = _rows(w.vel, 3)
+    n = int(prow[0].shape[0])
+    if out is None:
+        out = (np.empty((3, n), dtype=np.float64), np.empty((3, n), dtype=np.float64),
+               np.empty(n, dtype=np.int32), np.empty(n, dtype=np.int64))
+    pos, vel, flag, rstep = out
+    ps = c_longlong(0)
+    st = lib().glisse_run(float(w.gm_star), npl, _ptr(gm_planet), _ptr(ppos), _ptr(pvel), _ptr(rcrit), n, _p3(prow),
+                          _p3(vrow), float(w.dt), byref(prm), int(n_steps), int(n_parts),
+                          None if pos is None else _p3([pos[k] for k in range(3)]),
+                          None if vel is None else _p3([vel[k] for k in range(3)]), _ptr(flag), _ptr(rstep),
+                          byref(ps))
+    _check(st, "glisse_run")
+    return pos, vel, flag, rstep, int(ps.value)
+
+
 class GlisseSim:
     """glisse_create / glisse_advance / glisse_read with the C ABI's argument order."""
 
@@ -184,19 +237,11 @@ class GlisseSim:
         keep_v, vrow = _rows(vel, 3)
         self.n = int(prow[0].shape[0])
         self.device = int(device)
-        prm = GlisseParams()
-        L.glisse_default_params(byref(prm))
-        prm.r_min, prm.r_max = float(r_min), float(r_max)
-        prm.kepler_iters, prm.kepler_tol = int(kepler_iters), float(kepler_tol)
-        prm.chunk_steps, prm.resync_chunks = int(chunk_steps), int(resync_chunks)
-        prm.device = self.device
-        prm.stream = None if stream is None else c_void_p(int(stream))
-        prm.snapshot_chunks, prm.resonance_chunks = int(snapshot_chunks), int(resonance_chunks)
-        prm.bin_iterations = int(bin_iterations)
-        prm.scheme = {"kdk": 0, "dkd": 1}[scheme]
-        prm.guess_order = int(guess_order)
-        if segment_steps is not None:
-            prm.segment_steps = int(segment_steps)
+        prm = _params(r_min=r_min, r_max=r_max, kepler_iters=kepler_iters, kepler_tol=kepler_tol,
+                      chunk_steps=chunk_steps, resync_chunks=resync_chunks, device=device, stream=stream,
+                      snapshot_chunks=snapshot_chunks, resonance_chunks=resonance_chunks,
+                      bin_iterations=bin_iterations, segment_steps=segment_steps, scheme=scheme,
+                      guess_order=guess_order)
         h = c_void_p()
         st = L.glisse_create(byref(h), float(gm_star), self.n_planets, _ptr(gm_planet), _ptr(planet_pos),
                              _ptr(planet_vel), _ptr(rcrit), self.n, _p3(prow), _p3(vrow), float(dt), byref(prm))

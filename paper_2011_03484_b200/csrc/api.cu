@@ -1362,4 +1362,59 @@ int glisse_test_primitive(int which, long long n, const double* in, double* out)
 
 void glisse_destroy(glisse_sim* s) { free_sim(s); }
 
+// One-shot run over host (or device) arrays, pipelined over parts (include/glisse.h).  Each part is a sim
+// of its own on a contiguous slice of the particles: they never interact, so this is the
+// paper's own partition of the particles with the planets replicated — here over time slots of one GPU
+// instead of over GPUs.  Part i+1 is created (its upload) and part i read back (its download) while the
+// kernels of the other parts run.
+int glisse_run(double gm_star, int n_planets, const double* gm_planet, const double* planet_pos,
+               const double* planet_vel, const double* planet_rcrit, long long n_particles,
+               const double* const pos[3], const double* const vel[3], double dt, const glisse_params* params,
+               long long n_steps, int n_parts, double* const out_pos[3], double* const out_vel[3], int* flag,
+               long long* removal_step, long long* particle_steps) {
+  constexpr int kMaxParts = 64;
+  constexpr long long kAutoPart = 1LL << 17;   // automatic: parts of about 2^17 particles, at most 8
+  if (n_particles < 1 || n_steps < 0 || n_parts < 0 || n_parts > kMaxParts || !pos || !vel) return GLISSE_EINVAL;
+  for (int k = 0; k < 3; ++k)
+    if (!pos[k] || !vel[k]) return GLISSE_EINVAL;
+  if (n_parts == 0) n_parts = static_cast<int>(std::max<long long>(1, std::min<long long>(8, n_particles / kAutoPart)));
+  // cuts at multiples of 256 particles (whole warps, 2 KiB-aligned rows); no part is empty
+  long long cut[kMaxParts + 1];
+  int parts = 0;
+  cut[0] = 0;
+  for (int i = 1; i <= n_parts; ++i) {
+    long long c = (i == n_parts) ? n_particles : (n_particles * i / n_parts) / 256 * 256;
+    if (c > cut[parts]) cut[++parts] = c;
+  }
+  glisse_sim* sims[kMaxParts] = {};
+  int st = GLISSE_OK;
+  for (int i = 0; i < parts && st == GLISSE_OK; ++i) {
+    const long long lo = cut[i];
+    const double* p[3] = {pos[0] + lo, pos[1] + lo, pos[2] + lo};
+    const double* v[3] = {vel[0] + lo, vel[1] + lo, vel[2] + lo};
+    st = glisse_create(&sims[i], gm_star, n_planets, gm_planet, planet_pos, planet_vel, planet_rcrit, cut[i + 1] - lo, p,
+                       v, dt, params);
+    if (st == GLISSE_OK) st = glisse_advance(sims[i], n_steps);
+  }
+  long long psteps = 0;
+  for (int i = 0; i < parts && st == GLISSE_OK; ++i) {
+    const long long lo = cut[i];
+    double* p[3] = {nullptr, nullptr, nullptr};
+    double* v[3] = {nullptr, nullptr, nullptr};
+    for (int k = 0; k < 3; ++k) {
+      if (out_pos && out_pos[k]) p[k] = out_pos[k] + lo;
+      if (out_vel && out_vel[k]) v[k] = out_vel[k] + lo;
+    }
+    st = glisse_read(sims[i], p, v, flag ? flag + lo : nullptr, removal_step ? removal_step + lo : nullptr);
+    if (st == GLISSE_OK && particle_steps) {
+      const long long c = glisse_particle_steps(sims[i]);
+      if (c < 0) st = static_cast<int>(c);
+      else psteps += c;
+    }
+  }
+  for (int i = 0; i < parts; ++i) free_sim(sims[i]);
+  if (st == GLISSE_OK && particle_steps) *particle_steps = psteps;
+  return st;
+}
+
 }  // extern "C"

@@ -497,6 +497,48 @@ def test_planet_log_interpolated_from_a_sparse_history(gl, oracle_mod, record):
     S.close()
 
 
+def test_one_shot_run_pipelined_over_parts(gl, oracle_mod, record):
+    """glisse_run (include/glisse.h): create + advance + read + destroy over slices of the particles, each slice a
+    simulation of its own.  With a fixed Kepler starting point the result does not depend on
+    the number of parts, bit for bit, and equals the single simulation's; with everything automatic it holds
+    the oracle's tolerance.  Host arrays and device tensors; refused arguments."""
+    import dataclasses
+    import torch
+    w = inputs.config(5, 9000)
+    steps = 300
+    S = gl.GlisseSim.from_workload(w, chunk_steps=128, guess_order=1)
+    S.advance(steps)
+    p0, v0, f0, r0 = S.read()
+    ps0 = S.particle_steps()
+    S.close()
+    assert (f0 != 0).sum() > 50                       # removals happen in every part
+    for parts in (1, 2, 5, 64):
+        p, v, f, r, ps = gl.run(w, steps, parts, chunk_steps=128, guess_order=1)
+        assert np.array_equal(p, p0) and np.array_equal(v, v0) and np.array_equal(f, f0) and np.array_equal(r, r0)
+        assert ps == ps0
+    wd = dataclasses.replace(w, pos=torch.from_numpy(w.pos).cuda(), vel=torch.from_numpy(w.vel).cuda())
+    out = (torch.empty((3, w.n_particles), dtype=torch.float64, device="cuda"),
+           torch.empty((3, w.n_particles), dtype=torch.float64, device="cuda"),
+           torch.empty(w.n_particles, dtype=torch.int32, device="cuda"),
+           torch.empty(w.n_particles, dtype=torch.int64, device="cuda"))
+    p, v, f, r, ps = gl.run(wd, steps, 3, out=out, chunk_steps=128, guess_order=1)
+    assert np.array_equal(p.cpu().numpy(), p0) and np.array_equal(r.cpu().numpy(), r0) and ps == ps0
+    # everything automatic (parts, starting point, binning) against the oracle, under the module's rule
+    (po, vo, fo, ro), ps_o = _oracle_run(oracle_mod, w, steps)
+    sigma, twin_agrees = _sensitivity(oracle_mod, w, steps, po, vo, fo, ro)
+    p, v, f, r, ps = gl.run(w, steps, 0, chunk_steps=128)
+    dev = np.maximum(_dev(p, po), _dev(v, vo))
+    _judge(record, "one_shot_run_auto", dev, sigma, twin_agrees, f, r, fo, ro, False, 0.5)
+    # only the flags / steps asked for
+    _, _, f, r, _ = gl.run(w, steps, 2, out=(None, None, np.empty(w.n_particles, np.int32), np.empty(w.n_particles, np.int64)),
+                           chunk_steps=128, guess_order=1)
+    assert np.array_equal(f, f0) and np.array_equal(r, r0)
+    for bad in (lambda: gl.run(w, -1, 1), lambda: gl.run(w, steps, 65), lambda: gl.run(w, steps, -1),
+                lambda: gl.run(w, steps, 2, kepler_iters=-3)):
+        with pytest.raises(gl.GlisseError):
+            bad()
+
+
 def test_periodic_output_ring(gl):
     """params.snapshot_chunks ("copied back to the CPU after a user-configurable number of
     planetary chunk calculations"): ONE glisse_advance of 10 chunks emits a snapshot every 2 chunks
