@@ -45,6 +45,8 @@ extern "C" {
 #define GLISSE_ENOMEM  (-3)  /* host or device allocation failed                              */
 #define GLISSE_EPLANET (-4)  /* a planet's Kepler drift failed (unbound / not converged): the
                                 paper requires encounter-free planets           */
+#define GLISSE_ELIMIT  (-5)  /* a size beyond the fixed capacity of an entry point that may not
+                                allocate (glisse_planet_log_static)                           */
 
 /* ---- per-particle flag values ("a flag that records which planet") ------------ */
 #define GLISSE_FLAG_ACTIVE    0
@@ -210,6 +212,31 @@ int glisse_interpolate_log(glisse_sim* sim, long long n_samples, const double* s
  * Used to check the planet-history kernel (a1) against the oracle.  Synchronises.
  */
 int glisse_planet_log(glisse_sim* sim, long long n_steps, double* log);
+
+/*
+ * glisse_planet_log for callers that may not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same planet-history kernel, the same records, but NO
+ * cudaMalloc / cudaFree / allocating routine anywhere in the call.  glisse_planet_log allocates two
+ * buffers per call (a staging copy of the log, and the kernel's scratch: the Jacobi state it writes at
+ * every record); here the kernel writes the log straight into the caller's buffer and its scratch is a
+ * fixed array in device memory that the library holds on every GPU that loads it (2 MiB, until the
+ * process exits).
+ *   log: DEVICE memory of this sim's device, 16-byte aligned, (n_steps+1) x glisse_log_stride(n_planets)
+ *        doubles (GLISSE_EINVAL for a host pointer: the kernel writes it directly).
+ *   Limit: (n_steps + 1) x 6 n_planets doubles of scratch must fit 2^18 doubles, i.e. n_steps <=
+ *        glisse_planet_log_static_limit(n_planets) (10 921 steps at 4 planets, 5 460 at 8, 1 364 at 32);
+ *        beyond it GLISSE_ELIMIT, nothing launched, nothing changed.
+ *   Sharing: every call on a device uses the same scratch array, which keeps the last call's contents.
+ *        Nothing in it has to start at zero (the kernel writes each record before anything reads it), but
+ *        two calls that OVERLAP on the GPU — different sims on different streams, or different host
+ *        threads — race on it; this call synchronises before it returns, so calls made one after the other
+ *        from one thread never overlap.
+ * The simulation is not changed.  Synchronises.  Statuses otherwise as glisse_planet_log.
+ */
+int glisse_planet_log_static(glisse_sim* sim, long long n_steps, double* log);
+
+/* Largest n_steps glisse_planet_log_static accepts for n_planets planets; < 0 if n_planets is out of range. */
+long long glisse_planet_log_static_limit(int n_planets);
 
 /*
  * Read the particle state in ORIGINAL particle order (compaction is invisible).

@@ -17,13 +17,14 @@ import numpy as np
 
 from . import build as _build
 
-OK, EINVAL, ECUDA, ENOMEM, EPLANET = 0, -1, -2, -3, -4
+OK, EINVAL, ECUDA, ENOMEM, EPLANET, ELIMIT = 0, -1, -2, -3, -4, -5
 FLAG_ACTIVE, FLAG_RMIN, FLAG_RMAX, FLAG_NONCONV, FLAG_UNBOUND, FLAG_PLANET0 = 0, 1, 2, 3, 4, 16
 
 #: every symbol include/glisse.h declares (tests check that the library exports each one) ...
 EXPORTS = (
     "glisse_default_params", "glisse_create", "glisse_advance", "glisse_advance_with_log", "glisse_set_planets",
-    "glisse_log_stride", "glisse_planet_log", "glisse_interpolate_log", "glisse_read", "glisse_read_planets",
+    "glisse_log_stride", "glisse_planet_log", "glisse_planet_log_static", "glisse_planet_log_static_limit",
+    "glisse_interpolate_log", "glisse_read", "glisse_read_planets",
     "glisse_snapshot", "glisse_snapshot_wait", "glisse_snapshot_ring", "glisse_snapshots_emitted",
     "glisse_resonance_begin", "glisse_resonance_sample", "glisse_resonance_read", "glisse_libration_read",
     "glisse_active_count", "glisse_step", "glisse_particle_steps", "glisse_sync", "glisse_destroy", "glisse_run",
@@ -88,6 +89,10 @@ def lib():
         L.glisse_log_stride.restype = c_int
         L.glisse_planet_log.argtypes = [c_void_p, c_longlong, c_void_p]
         L.glisse_planet_log.restype = c_int
+        L.glisse_planet_log_static.argtypes = [c_void_p, c_longlong, c_void_p]
+        L.glisse_planet_log_static.restype = c_int
+        L.glisse_planet_log_static_limit.argtypes = [c_int]
+        L.glisse_planet_log_static_limit.restype = c_longlong
         L.glisse_interpolate_log.argtypes = [c_void_p, c_longlong, c_void_p, c_void_p, c_void_p, c_double, c_double,
                                              c_longlong, c_void_p]
         L.glisse_interpolate_log.restype = c_int
@@ -130,6 +135,10 @@ def lib():
 
 def strerror(status: int) -> str:
     return lib().glisse_strerror(int(status)).decode()
+
+
+def planet_log_static_limit(n_planets: int) -> int:
+    return int(lib().glisse_planet_log_static_limit(int(n_planets)))
 
 
 def log_stride(n_planets: int) -> int:
@@ -273,6 +282,12 @@ class GlisseSim:
     def planet_log(self, n_steps):
         out = np.zeros((int(n_steps) + 1, log_stride(self.n_planets)), dtype=np.float64)
         _check(lib().glisse_planet_log(self._h, int(n_steps), _ptr(out)), "glisse_planet_log")
+        return out
+
+    def planet_log_static(self, n_steps, out):
+        """glisse_planet_log_static: the same log written straight into `out`, a torch CUDA float64 tensor
+        [n_steps + 1, stride] the caller allocated; the library allocates nothing."""
+        _check(lib().glisse_planet_log_static(self._h, int(n_steps), _ptr(out)), "glisse_planet_log_static")
         return out
 
     def interpolate_log(self, sample_time, sample_pos, sample_vel, t_first, dt_record, n_records, out=None):

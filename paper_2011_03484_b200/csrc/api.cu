@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstddef>
+#include <cstdint>
 #include <cstring>
 #include <limits>
 #include <mutex>
@@ -658,6 +659,7 @@ const char* glisse_strerror(int status) {
     case GLISSE_ECUDA: return "CUDA failure";
     case GLISSE_ENOMEM: return "out of memory";
     case GLISSE_EPLANET: return "a planet's Kepler drift failed (planets must be encounter-free and bound)";
+    case GLISSE_ELIMIT: return "size beyond the fixed capacity of a non-allocating entry point";
     default: return "unknown status";
   }
 }
@@ -1079,6 +1081,46 @@ int glisse_planet_log(glisse_sim* s, long long n_steps, double* log) {
   cudaFree(d_log);
   cudaFree(d_jlog);
   CKS(s, e);
+  const int st = sync_all(s);
+  if (st != GLISSE_OK) return st;
+  return fail < s->step + n_steps ? GLISSE_EPLANET : GLISSE_OK;   // not sticky: the sim itself is intact
+}
+
+long long glisse_planet_log_static_limit(int n_planets) {
+  const long long lim = static_planet_log_limit(n_planets);
+  return lim < 0 ? GLISSE_EINVAL : lim;
+}
+
+// glisse_planet_log without an allocation: the kernel writes the caller's device buffer, its Jacobi-state
+// scratch is the static device array of planets.cu.  No cudaMalloc, cudaFree or allocating routine below.
+int glisse_planet_log_static(glisse_sim* s, long long n_steps, double* log) {
+  if (!s || n_steps < 0 || !log || (reinterpret_cast<uintptr_t>(log) & 15)) return GLISSE_EINVAL;
+  if (s->status != GLISSE_OK) return s->status;
+  if (s->planets_stale) return GLISSE_EINVAL;
+  if (n_steps > static_planet_log_limit(s->np)) return GLISSE_ELIMIT;
+  CKS(s, cudaSetDevice(s->device));
+  {
+    // the kernel writes `log` directly: it must be device memory of this device
+    cudaPointerAttributes at{};
+    if (cudaPointerGetAttributes(&at, log) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return GLISSE_EINVAL;
+    }
+    if (at.type != cudaMemoryTypeDevice || at.device != s->device) return GLISSE_EINVAL;
+  }
+  break_chain(s);
+  const int np = s->np;
+  const LogBuffer& B = s->buf[s->cur];
+  const long long off = s->step - B.start;
+  const long long no_fail = kNoPlanetFailure;
+  long long fail = kNoPlanetFailure;
+  CKS(s, cudaStreamWaitEvent(s->q, B.ready, 0));
+  // a scratch failure word: a failure somewhere in this look-ahead does not concern the sim's own clock
+  CKS(s, cudaMemcpyAsync(s->d_fail + 1, &no_fail, sizeof(no_fail), cudaMemcpyHostToDevice, s->q));
+  CKS(s, launch_planet_kernel_static(s->d_sys, np, B.jlog + static_cast<size_t>(off) * 6 * np, log,
+                                     static_cast<int>(n_steps), s->dt, s->step, s->d_fail + 1, s->q));
+  s->launches += 1;
+  CKS(s, cudaMemcpyAsync(&fail, s->d_fail + 1, sizeof(fail), cudaMemcpyDeviceToHost, s->q));
   const int st = sync_all(s);
   if (st != GLISSE_OK) return st;
   return fail < s->step + n_steps ? GLISSE_EPLANET : GLISSE_OK;   // not sticky: the sim itself is intact

@@ -129,6 +129,14 @@ cudaError_t launch_planet_init(const PlanetSystem* sys, const double* q, const d
 cudaError_t launch_planet_read(const PlanetSystem* sys, const double* jstate, double* q, double* qd,
                                cudaStream_t s);
 
+// The same kernel with its Jacobi-state scratch in a file-scope static __device__ array (planets.cu) instead of
+// caller memory: kStaticJlogDoubles doubles per device, shared by every call on that device.
+constexpr size_t kStaticJlogDoubles = size_t(1) << 18;   // 2 MiB
+// largest nsteps the static scratch holds for np planets (-1: np out of range)
+long long static_planet_log_limit(int np);
+cudaError_t launch_planet_kernel_static(const PlanetSystem* sys, int np, const double* jin, double* log, int nsteps,
+                                        double dt, long long step0, long long* fail_step, cudaStream_t s);
+
 // planet log records by cubic Hermite interpolation of a sparse history (all pointers device)
 cudaError_t launch_interpolate_log(const PlanetSystem* sys, long long n_samples, const double* sample_time,
                                    const double* sample_pos, const double* sample_vel, double t_first, double dt_record,

@@ -12,6 +12,8 @@
 //   kick:  v'_k += h (eta_k/eta_{k-1}) [ gm0 r'_k/|r'_k|^3 + A_k + (1/eta_k) sum_{i>k} gm_i A_i ]
 //          A_i = − gm0 q_i/|q_i|^3 − sum_{j != i} gm_j (q_i − q_j)/|q_i − q_j|^3
 //   drift: two-body motion of (r'_k, v'_k) about mu_k = gm0 eta_k/eta_{k-1}
+#include <mutex>
+
 #include "glisse_internal.cuh"
 #include "kepler.cuh"
 
@@ -371,6 +373,53 @@ cudaError_t launch_interpolate_log(const PlanetSystem* sys, long long n_samples,
   interpolate_log_kernel<<<static_cast<unsigned>((n_records + 127) / 128), 128, 0, s>>>(
       sys, n_samples, sample_time, sample_pos, sample_vel, t_first, dt_record, n_records, log);
   return cudaGetLastError();
+}
+
+// ---- the planet log without any allocation (include/glisse.h: glisse_planet_log_static) --------------------
+// The planet-history kernel writes, beside the log, the Jacobi state at every record (so that any step can be
+// resumed from): for glisse_planet_log that is scratch, which it gets from cudaMalloc.  Here the scratch is a
+// file-scope array in device memory of a fixed size, for callers that may not allocate.  Every GPU that loads
+// the library holds these 2 MiB until the process exits; every call on a device shares them.
+static __device__ __align__(256) double g_static_jlog[kStaticJlogDoubles];
+
+namespace {
+std::mutex g_static_mu;
+double* g_static_jlog_addr[64] = {};   // per device: the array's DEVICE address (its name is a host-side stand-in)
+}  // namespace
+
+// Device address of the static scratch on the CURRENT device, looked up once per device.
+static cudaError_t static_jlog_address(double** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_jlog_addr[dev]) {
+    double* ptr = nullptr;
+    e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_static_jlog);
+    if (e != cudaSuccess) return e;
+    if (!ptr) return cudaErrorInvalidSymbol;
+    g_static_jlog_addr[dev] = ptr;
+  }
+  *out = g_static_jlog_addr[dev];
+  return cudaSuccess;
+}
+
+long long static_planet_log_limit(int np) {
+  if (np < 0 || np > kMaxPlanets) return -1;
+  const long long per_record = np > 0 ? 6LL * np : 1;
+  return static_cast<long long>(kStaticJlogDoubles) / per_record - 1;   // records = steps + 1
+}
+
+cudaError_t launch_planet_kernel_static(const PlanetSystem* sys, int np, const double* jin, double* log, int nsteps,
+                                        double dt, long long step0, long long* fail_step, cudaStream_t s) {
+  if (nsteps < 0 || nsteps > static_planet_log_limit(np)) return cudaErrorInvalidValue;   // (the caller checks first)
+  double* jlog = nullptr;
+  cudaError_t e = static_jlog_address(&jlog);
+  if (e != cudaSuccess) return e;
+  // Nothing in the scratch has to start at zero: the kernel writes every Jacobi record of this call before
+  // anything could read it, and nothing of an earlier call is read.
+  return launch_planet_kernel(sys, np, jin, log, jlog, nsteps, dt, step0, fail_step, 0, s);
 }
 
 }  // namespace glisse
