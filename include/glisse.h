@@ -18,7 +18,9 @@
  *  - Units: the library is unit-agnostic; G is folded into the masses (gm = G·m).  The
  *    benchmark configurations use AU, days, solar masses with G = k² (Gaussian constant).
  *  - Pointers marked "host or device" are handed to cudaMemcpyAsync with cudaMemcpyDefault: the
- *    driver's unified addressing tells host from device, the library never classifies them itself.
+ *    driver's unified addressing tells host from device, the library never classifies them itself
+ *    (one exception: glisse_planet_log_static, whose kernel writes the caller's buffer directly,
+ *    asks cudaPointerGetAttributes whether it is device memory).
  *    Host buffers should be pinned for the copies to overlap; pageable ones work and serialise.
  *  - Ownership: inputs are copied during glisse_create (the caller keeps its buffers); outputs
  *    are caller-allocated.  The library owns its internal device state until glisse_destroy.
