@@ -370,7 +370,8 @@ void glisse_destroy(glisse_sim* sim);
  * The result of every particle is what a single simulation over all of them returns, bit for bit, when
  * params fixes guess_order (1 or 3); with guess_order = 0 each part chooses its Kepler starting point from
  * its own particles, as every rank of a multi-GPU run does (a roundoff-level difference).  Arguments and
- * statuses otherwise as glisse_create.  Synchronous.
+ * statuses otherwise as glisse_create (a caller's params->stream is then shared by all parts, whose particle
+ * kernels no longer overlap: leave it NULL here).  Synchronous.
  */
 int glisse_run(double gm_star, int n_planets, const double* gm_planet, const double* planet_pos,
                const double* planet_vel, const double* planet_rcrit, long long n_particles,
